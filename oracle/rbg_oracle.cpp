@@ -1,0 +1,499 @@
+// rbg_oracle.cpp -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+//
+// Plain, slow, scalar CPU oracle for the Monte Carlo evaluation of the relativistic 2->2
+// Boltzmann collision term C_a[f](x,p1) (Eq. 16; quantum factor Eq. 18
+// PAPER.md:192-197; species sum and symmetry factor Eq. 19).
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+// build, load or call this file.  It shares no code, header, table or constant generator with
+// the CUDA path under paper_2308_04869_b200/csrc and neither includes the other.
+//
+// What it computes.  Eq. 16 for "a(k1)+b(k2)->c(k3)+d(p)" with the grid particle d(p)==p1, its
+// partner c(k3)==p2 and the other pair (k1,k2)==(p3,p4).  Integrating d3p3 d3p4 delta4/(E3 E4) by
+// two-body phase space (= |p*|/sqrt(s) dOmega*) leaves the reduced form (R) of DESIGN.md section 2:
+//
+//   C_role(x,p1) = sym * Int_box(s2) d3p2 Int_4pi dOmega*  |M|^2 |p*_34| / (64 pi^2 E1 E2 sqrt(s))
+//                        * [ f3 f4 F1 F2  -  f1 f2 F3 F4 ],          F = 1 + theta (2 pi hbar)^3 f / g
+//
+// which is estimated with N samples: p2 uniform in the species-2 momentum box (volume V2), the
+// CM direction n uniform on the sphere, so C_role ~= sym V2 4pi / N * Sum integrand
+//          = sym V2 / (16 pi E1 N) * Sum  w (gain - loss),   w = |M|^2 |p*| / (E2 sqrt(s)).
+//
+// The paper leaves sampler, RNG and arithmetic order to an external package, so
+// the step-by-step chain below (O0..O14) is the reading fixed in DESIGN.md section 4; every
+// floating-point operation up to a cell-index decision is written as ONE IEEE operation
+// (fma() = one rounding; every other operator one rounding; no contraction: build with
+// -ffp-contract=off) so that an independent implementation can reproduce the decisions exactly.
+//
+// Pins (tests/test_oracle_*.py): Philox known answers, per-sample kinematic invariants, the
+// massless closed form, a scipy quadrature of the loss rate, exact detailed balance for
+// MJ/FD/BE inputs, the paper's own 5-D form Eq. 37 (oracle/eq37.py), number/energy conservation,
+// deterministic brute-force quadrature of (R) (oracle/quadrature.py), H-theorem sign,
+// thread-count independence.  No function here is "parity unpinned".
+#include <cmath>
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <limits>
+#include <string>
+#include <type_traits>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+// ---------------------------------------------------------------------------------------------
+// O1. Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11).  Counter-based: out = P(key, counter).
+// ---------------------------------------------------------------------------------------------
+struct U4 { uint32_t v[4]; };
+
+inline U4 philox4x32_10(uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3) {
+    const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;   // round multipliers
+    const uint32_t W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;   // Weyl key increments
+    for (int round = 0; round < 10; ++round) {
+        const uint64_t prod0 = (uint64_t)M0 * c0;
+        const uint64_t prod1 = (uint64_t)M1 * c2;
+        const uint32_t hi0 = (uint32_t)(prod0 >> 32), lo0 = (uint32_t)prod0;
+        const uint32_t hi1 = (uint32_t)(prod1 >> 32), lo1 = (uint32_t)prod1;
+        const uint32_t n0 = hi1 ^ c1 ^ k0;
+        const uint32_t n1 = lo1;
+        const uint32_t n2 = hi0 ^ c3 ^ k1;
+        const uint32_t n3 = lo0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += W0; k1 += W1;
+    }
+    return U4{{c0, c1, c2, c3}};
+}
+
+// ---------------------------------------------------------------------------------------------
+// Problem description (mirrors what the caller passes; plain structs, C layout)
+// ---------------------------------------------------------------------------------------------
+struct Species { double mass, charge; int stat; double g; };
+struct Grid    { int n[3]; double pmin[3], pmax[3]; };
+struct Process { int a, b, c, d; int kind; double par[4]; double sym; };
+
+enum Kind { M2_CONST = 0, M2_COULOMB_SCREENED = 1, M2_TCHAN_S2 = 2 };
+
+// A role = one process seen from one grid species: particle 1 is the grid
+// particle, 2 its sampled partner, (3,4) the other pair.
+struct Role { int s[4]; int kind; double par[4]; double sym; int process; };
+
+typedef double (*FCallback)(int species, const double* p, void* user);
+
+// Built-in analytic input family for analytic-f mode (an INPUT, not part of the method):
+//   f_s(p) = scale / ( exp((sqrt(|p-u|^2 + m^2) - mu)/T) - theta ),  8 doubles per species in
+// `user`: scale, T, mu, m, theta, ux, uy, uz.  theta=0: Maxwell-Juttner (Eq. 11),
+// -1/+1: Fermi-Dirac / Bose-Einstein occupation times scale.
+extern "C" double orc_builtin_thermal(int species, const double* p, void* user) {
+    const double* q = (const double*)user + 8 * species;
+    const double dx = p[0] - q[5], dy = p[1] - q[6], dz = p[2] - q[7];
+    const double E = std::sqrt(dx * dx + dy * dy + dz * dz + q[3] * q[3]);
+    return q[0] / (std::exp((E - q[2]) / q[1]) - q[4]);
+}
+
+struct Handle {
+    int nx = 0;
+    std::vector<Species> sp;
+    std::vector<Grid> grid;
+    std::vector<Role> roles;
+    std::vector<size_t> sp_off;     // offset of species s in the f / C arrays
+    std::vector<size_t> np;         // momentum cells of species s
+    std::vector<size_t> role_off;   // offset of role r in the per-role detail arrays
+    double hbar = 1.0;
+    int use_float = 0;
+    std::string err;
+};
+
+// Per-sample record for tests (oracle-only).
+struct Trace {
+    double p1[3], p2[3], p3[3], p4[3];
+    double E1, E2, E3, s, t, pf, w, f1, f2, f3, f4, gain, loss;
+    int j2, j3, j4;            // linear momentum cell, -1 = outside the box
+    int status;                // 0 ok, 1 skipped at O4 (h<=0), 2 below threshold, 3 no direction
+    int draws;                 // Philox calls consumed
+};
+
+template <typename R> inline R rfma(R a, R b, R c);
+template <> inline double rfma<double>(double a, double b, double c) { return std::fma(a, b, c); }
+template <> inline float  rfma<float>(float a, float b, float c) { return std::fmaf(a, b, c); }
+
+// u32 -> uniform real in [0,1): double keeps all 32 bits, float the top 24; both exact.
+template <typename R> inline R u01(uint32_t x);
+template <> inline double u01<double>(uint32_t x) { return (double)x * 0x1p-32; }
+template <> inline float  u01<float>(uint32_t x) { return (float)(x >> 8) * 0x1p-24f; }
+// u32 -> uniform real in [-1,1): exact in both types.
+template <typename R> inline R usym(uint32_t x);
+template <> inline double usym<double>(uint32_t x) { return (double)x * 0x1p-31 - 1.0; }
+template <> inline float  usym<float>(uint32_t x) { return (float)(x >> 8) * 0x1p-23f - 1.0f; }
+
+template <typename R> struct RoleConst {
+    R m[4], msq[4];
+    R m1m2, msum2, Mth, Mdf, dm34;
+    R pmin[4][3], L[4][3], invD[4][3], off[4][3];   // per particle slot (its species' grid)
+    int n[4][3];
+    R theta_kappa[4];
+    R par0, mD2, g4;
+};
+
+template <typename R> inline R dot3(const R* a, const R* b) {
+    return rfma<R>(a[2], b[2], rfma<R>(a[1], b[1], a[0] * b[0]));
+}
+
+struct Accum { double G = 0, Ls = 0, Lin = 0, Q = 0; };
+
+template <typename R>
+struct Evaluator {
+    const Handle& H; const Role& role; int irole;
+    RoleConst<R> k;
+    FCallback fcb; void* user; int box_cut;   // analytic-f mode when fcb != nullptr
+
+    Evaluator(const Handle& h, int ir, FCallback cb, void* u, int cut)
+        : H(h), role(h.roles[ir]), irole(ir), fcb(cb), user(u), box_cut(cut) {
+        // Role constants: computed in double by the formulas below, then rounded to R.
+        double m[4];
+        for (int i = 0; i < 4; ++i) m[i] = H.sp[role.s[i]].mass;
+        for (int i = 0; i < 4; ++i) { k.m[i] = (R)m[i]; k.msq[i] = (R)(m[i] * m[i]); }
+        const double msum = m[0] + m[1], m34 = m[2] + m[3], md = m[2] - m[3];
+        k.m1m2  = (R)(m[0] * m[1]);
+        k.msum2 = (R)(msum * msum);
+        k.Mth   = (R)(msum * msum - m34 * m34);
+        k.Mdf   = (R)(md * md);
+        k.dm34  = (R)(m[2] * m[2] - m[3] * m[3]);
+        const double twopihbar = 2.0 * M_PI * H.hbar;
+        for (int i = 0; i < 4; ++i) {
+            const Grid& g = H.grid[role.s[i]];
+            for (int d = 0; d < 3; ++d) {
+                const double L = g.pmax[d] - g.pmin[d];
+                const double invD = (double)g.n[d] / L;
+                k.n[i][d] = g.n[d];
+                k.pmin[i][d] = (R)g.pmin[d];
+                k.L[i][d] = (R)L;
+                k.invD[i][d] = (R)invD;
+                k.off[i][d] = (R)(-g.pmin[d] * invD);
+            }
+            const Species& S = H.sp[role.s[i]];
+            k.theta_kappa[i] = (R)((double)S.stat * (twopihbar * twopihbar * twopihbar) / S.g);
+        }
+        k.par0 = (R)role.par[0];
+        k.mD2  = (R)(role.par[1] * role.par[1]);
+        const double g2 = role.par[0] * role.par[0];
+        k.g4   = (R)(g2 * g2);
+    }
+
+    // O10.  Nearest-cell gather: tau_d = fma(p_d, invDelta_d, -pmin_d*invDelta_d); inside iff
+    // 0 <= floor(tau_d) < n_d for all d; zero outside the box (north_star).  Returns cell or -1.
+    inline int cell_of(int slot, const R* p) const {
+        int j[3];
+        for (int d = 0; d < 3; ++d) {
+            const R tau = rfma<R>(p[d], k.invD[slot][d], k.off[slot][d]);
+            const R fl = std::floor(tau);
+            if (!(fl >= (R)0) || !(fl < (R)k.n[slot][d])) return -1;
+            j[d] = (int)fl;
+        }
+        return (j[0] * k.n[slot][1] + j[1]) * k.n[slot][2] + j[2];
+    }
+
+    // One p1: N samples.  The f value of species s, spatial cell ix, momentum cell j is
+    // f_all[sp_off[s] + ix*np[s] + j] (layout of DESIGN.md section 5).
+    void eval_p1(const double* f_all, int ix, int ip1, int N, uint64_t seed, Accum& acc, Trace* trace,
+                 int trace_n) const {
+        const uint32_t key0 = (uint32_t)seed, key1 = (uint32_t)(seed >> 32);
+        // species table base pointers at this spatial cell (index = sp_off[s] + ix*np[s])
+        auto fval = [&](int slot, int cell, const R* p) -> R {
+            if (fcb) {
+                if (box_cut && cell < 0) return (R)0;
+                const double pd[3] = {(double)p[0], (double)p[1], (double)p[2]};
+                return (R)fcb(role.s[slot], pd, user);
+            }
+            if (cell < 0) return (R)0;
+            const int s = role.s[slot];
+            return (R)f_all[H.sp_off[s] + (size_t)ix * H.np[s] + (size_t)cell];
+        };
+
+        // ---- O0: per-p1 setup -------------------------------------------------------------
+        const Grid& g1 = H.grid[role.s[0]];
+        int i1[3];
+        i1[2] = ip1 % g1.n[2]; i1[1] = (ip1 / g1.n[2]) % g1.n[1]; i1[0] = ip1 / (g1.n[2] * g1.n[1]);
+        R p1[3];
+        for (int d = 0; d < 3; ++d) {
+            const R delta = (R)((g1.pmax[d] - g1.pmin[d]) / (double)g1.n[d]);
+            p1[d] = rfma<R>((R)i1[d] + (R)0.5, delta, k.pmin[0][d]);
+        }
+        const R q1 = dot3<R>(p1, p1);
+        const R E1 = std::sqrt(q1 + k.msq[0]);
+        const R T1 = q1 / (E1 + k.m[0]);        // kinetic energy E1-m1, cancellation-free (float chain)
+        const R f1 = fval(0, ip1, p1);
+        const R F1 = rfma<R>(k.theta_kappa[0], f1, (R)1);
+
+        for (int n = 0; n < N; ++n) {
+            Trace tr; std::memset(&tr, 0, sizeof tr);
+            const bool want = trace && n == trace_n;
+            const uint32_t cw = ((uint32_t)irole << 8);
+            // ---- O1/O2: partner momentum, uniform in the species-2 box --------------------
+            const U4 r0 = philox4x32_10(key0, key1, (uint32_t)n, (uint32_t)ip1, (uint32_t)ix, cw | 0u);
+            R p2[3]; int j2d[3];
+            for (int d = 0; d < 3; ++d) {
+                const R u = u01<R>(r0.v[d]);
+                p2[d] = rfma<R>(u, k.L[1][d], k.pmin[1][d]);
+                j2d[d] = (int)(((uint64_t)r0.v[d] * (uint64_t)k.n[1][d]) >> 32);   // = floor(x n / 2^32)
+            }
+            const int j2 = (j2d[0] * k.n[1][1] + j2d[1]) * k.n[1][2] + j2d[2];
+            int status = 0, draws = 1;
+            R E2 = 0, s = 0, t = 0, pf = 0, w = 0, E3 = 0, f2 = 0, f3 = 0, f4 = 0, gain = 0, loss = 0;
+            R p3[3] = {0, 0, 0}, p4[3] = {0, 0, 0};
+            int j3 = -1, j4 = -1;
+            do {
+                // ---- O3: partner energy ---------------------------------------------------
+                const R q2 = dot3<R>(p2, p2);
+                E2 = std::sqrt(q2 + k.msq[1]);
+                // ---- O4: s via h = E1 E2 - m1 m2 - p1.p2 = (s - (m1+m2)^2)/2 --------------
+                const R d12 = dot3<R>(p1, p2);
+                R Kk;
+                if (std::is_same<R, float>::value) {
+                    // float chain: E1E2 - m1m2 = T1 T2 + m1 T2 + m2 T1 with T = q/(E+m) (no cancellation)
+                    const R T2 = q2 / (E2 + k.m[1]);
+                    Kk = rfma<R>(T1, T2, rfma<R>(k.m[0], T2, k.m[1] * T1));
+                } else {
+                    Kk = rfma<R>(E1, E2, -k.m1m2);
+                }
+                const R h = Kk - d12;
+                if (!(h > (R)0)) { status = 1; break; }
+                s = rfma<R>((R)2, h, k.msum2);
+                const R rs = std::sqrt(s);
+                const R irs = (R)1 / rs;
+                const R hirs = (R)0.5 * irs;
+                // ---- O5: threshold, outgoing CM momentum and CM energy of particle 3 ------
+                const R a34 = rfma<R>((R)2, h, k.Mth);          // s - (m3+m4)^2
+                if (!(a34 > (R)0)) { status = 2; break; }
+                const R b34 = s - k.Mdf;                        // s - (m3-m4)^2
+                pf = std::sqrt(a34 * b34) * hirs;               // |p*_34|
+                const R E3s = (s + k.dm34) * hirs;              // (s + m3^2 - m4^2) / (2 sqrt s)
+                // ---- O6: direction, Marsaglia (1972) disk rejection, trig-free -------------
+                R nh[3]; bool have = false;
+                for (uint32_t kd = 1; kd <= 15u && !have; ++kd) {
+                    const U4 rd = philox4x32_10(key0, key1, (uint32_t)n, (uint32_t)ip1, (uint32_t)ix, cw | kd);
+                    ++draws;
+                    for (int att = 0; att < 2 && !have; ++att) {
+                        const R a = usym<R>(rd.v[2 * att]), b = usym<R>(rd.v[2 * att + 1]);
+                        const R S = rfma<R>(a, a, b * b);
+                        if (S < (R)1) {
+                            const R r2 = (R)2 * std::sqrt((R)1 - S);
+                            nh[0] = a * r2; nh[1] = b * r2; nh[2] = rfma<R>((R)-2, S, (R)1);
+                            have = true;
+                        }
+                    }
+                }
+                if (!have) { status = 3; break; }
+                // ---- O7: boost the CM momentum of particle 3 to the lab ---------------------
+                R p3s[3], P[3];
+                for (int d = 0; d < 3; ++d) { p3s[d] = pf * nh[d]; P[d] = p1[d] + p2[d]; }
+                const R Et = E1 + E2;
+                const R dPn = dot3<R>(P, p3s);
+                E3 = rfma<R>(Et, E3s, dPn) * irs;               // gamma (E3* + beta.p3*)
+                const R c = (E3 + E3s) / (Et + rs);             // p3 = p3* + P (E3+E3*)/(Et+sqrt s)
+                for (int d = 0; d < 3; ++d) { p3[d] = rfma<R>(P[d], c, p3s[d]); p4[d] = P[d] - p3[d]; }
+                // ---- O8/O9/O12: t = (p1-p3)^2 and the weight as one quotient ---------------
+                const R ers = E2 * rs;
+                if (role.kind == M2_CONST) {
+                    w = (k.par0 * pf) / ers;
+                } else {
+                    R dl[3];
+                    for (int d = 0; d < 3; ++d) dl[d] = p1[d] - p3[d];
+                    const R dl2 = dot3<R>(dl, dl);
+                    const R dE = E1 - E3;
+                    t = rfma<R>(dE, dE, -dl2);
+                    const R D = t - k.mD2;
+                    const R den = (D * D) * ers;
+                    if (role.kind == M2_COULOMB_SCREENED) w = (k.par0 * pf) / den;
+                    else                                  w = ((k.g4 * (s * s)) * pf) / den;
+                }
+                // ---- O10: gathers ------------------------------------------------------------
+                j3 = cell_of(2, p3); j4 = cell_of(3, p4);
+                f2 = fval(1, j2, p2); f3 = fval(2, j3, p3); f4 = fval(3, j4, p4);
+                // ---- O11: statistics and integrand (Eq. 16 bracket, Eq. 18) -----------------
+                const R F2 = rfma<R>(k.theta_kappa[1], f2, (R)1);
+                const R F3 = rfma<R>(k.theta_kappa[2], f3, (R)1);
+                const R F4 = rfma<R>(k.theta_kappa[3], f4, (R)1);
+                gain = (f3 * f4) * (F1 * F2);
+                loss = (f1 * f2) * (F3 * F4);
+                // ---- O12: accumulate in double ---------------------------------------------
+                const double wg = (double)(w * gain), wl = (double)(w * loss);
+                acc.G += wg; acc.Ls += wl;
+                if (j3 >= 0 && j4 >= 0) acc.Lin += wl;
+                acc.Q += (wg - wl) * (wg - wl);
+            } while (false);
+            if (want) {
+                for (int d = 0; d < 3; ++d) { tr.p1[d] = p1[d]; tr.p2[d] = p2[d]; tr.p3[d] = p3[d]; tr.p4[d] = p4[d]; }
+                tr.E1 = E1; tr.E2 = E2; tr.E3 = E3; tr.s = s; tr.t = t; tr.pf = pf; tr.w = w;
+                tr.f1 = f1; tr.f2 = f2; tr.f3 = f3; tr.f4 = f4; tr.gain = gain; tr.loss = loss;
+                tr.j2 = j2; tr.j3 = j3; tr.j4 = j4; tr.status = status; tr.draws = draws;
+                *trace = tr;
+            }
+        }
+        (void)T1;
+    }
+
+    // O13: scale.  C_role = sym V2 / (16 pi E1 N) (G - Ls), in double.
+    double prefactor(int ip1, int N) const {
+        const Grid& g1 = H.grid[role.s[0]];
+        int i1[3];
+        i1[2] = ip1 % g1.n[2]; i1[1] = (ip1 / g1.n[2]) % g1.n[1]; i1[0] = ip1 / (g1.n[2] * g1.n[1]);
+        R p1[3];
+        for (int d = 0; d < 3; ++d) {
+            const R delta = (R)((g1.pmax[d] - g1.pmin[d]) / (double)g1.n[d]);
+            p1[d] = rfma<R>((R)i1[d] + (R)0.5, delta, k.pmin[0][d]);
+        }
+        const R E1 = std::sqrt(dot3<R>(p1, p1) + k.msq[0]);
+        const Grid& g2 = H.grid[role.s[1]];
+        const double V2 = (g2.pmax[0] - g2.pmin[0]) * (g2.pmax[1] - g2.pmin[1]) * (g2.pmax[2] - g2.pmin[2]);
+        return (role.sym * V2) / (16.0 * M_PI * (double)E1 * (double)N);
+    }
+};
+
+template <typename R>
+int run_collision(const Handle& H, const double* f, double* C, int N, uint64_t seed, int ix_begin, int ix_end,
+                  int ix_stride, double* dG, double* dL, double* dLin, double* dQ, FCallback cb, void* user,
+                  int box_cut) {
+    // C is zeroed for the spatial cells visited, then roles are added in ascending order (O14).
+    for (size_t s = 0; s < H.sp.size(); ++s)
+        for (int ix = ix_begin; ix < ix_end; ix += ix_stride)
+            for (size_t j = 0; j < H.np[s]; ++j) C[H.sp_off[s] + (size_t)ix * H.np[s] + j] = 0.0;
+    for (int ir = 0; ir < (int)H.roles.size(); ++ir) {
+        Evaluator<R> ev(H, ir, cb, user, box_cut);
+        const int s1 = H.roles[ir].s[0];
+        const long np1 = (long)H.np[s1];
+        const long ncell = (ix_end - ix_begin + ix_stride - 1) / ix_stride;
+        const bool serial = cb != nullptr && cb != orc_builtin_thermal;   // Python callbacks are not thread-safe
+#pragma omp parallel for schedule(static) if (!serial)
+        for (long idx = 0; idx < ncell * np1; ++idx) {
+            const int ix = ix_begin + (int)(idx / np1) * ix_stride;
+            const int ip1 = (int)(idx % np1);
+            Accum acc;
+            ev.eval_p1(f, ix, ip1, N, seed, acc, nullptr, -1);
+            const double pref = ev.prefactor(ip1, N);
+            C[H.sp_off[s1] + (size_t)ix * np1 + ip1] += pref * (acc.G - acc.Ls);
+            const size_t o = H.role_off[ir] + (size_t)ix * np1 + ip1;
+            if (dG) dG[o] = pref * acc.G;
+            if (dL) dL[o] = pref * acc.Ls;
+            if (dLin) dLin[o] = pref * acc.Lin;
+            if (dQ) dQ[o] = pref * pref * acc.Q;
+        }
+    }
+    return 0;
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------
+// C entry points (ctypes-friendly)
+// ---------------------------------------------------------------------------------------------
+extern "C" {
+
+void orc_philox4x32_10(const uint32_t key[2], const uint32_t ctr[4], uint32_t out[4]) {
+    const U4 r = philox4x32_10(key[0], key[1], ctr[0], ctr[1], ctr[2], ctr[3]);
+    for (int i = 0; i < 4; ++i) out[i] = r.v[i];
+}
+
+void* orc_create(int nx, int n_species, const Species* sp, const Grid* grid, int n_process, const Process* pr,
+                 double hbar, int use_float) {
+    Handle* H = new Handle;
+    H->nx = nx; H->hbar = hbar; H->use_float = use_float;
+    H->sp.assign(sp, sp + n_species);
+    H->grid.assign(grid, grid + n_species);
+    size_t off = 0;
+    for (int s = 0; s < n_species; ++s) {
+        H->sp_off.push_back(off);
+        const size_t np = (size_t)grid[s].n[0] * grid[s].n[1] * grid[s].n[2];
+        H->np.push_back(np);
+        off += (size_t)nx * np;
+    }
+    // Role expansion (Eq. 19): process a+b->c+d contributes to C of every
+    // distinct external species when that species is placed on the grid leg.  By the symmetry of
+    // |M|^2 under crossing the labels of a 2->2 process we treat:
+    //   grid particle = a : role (a,b,c,d)      grid particle = b : role (b,a,d,c)   (if b != a)
+    // For the elastic processes (c==a, d==b) these are the gain/loss pair of Eq. 16 with the
+    // forward and reverse reaction being the same process.  sym: <0 => paper rule (0.5 iff a==b).
+    size_t roff = 0;
+    for (int i = 0; i < n_process; ++i) {
+        const Process& p = pr[i];
+        if (p.c != p.a || p.d != p.b) { delete H; return nullptr; }   // elastic roles only (R15)
+        const double sym = p.sym < 0 ? (p.a == p.b ? 0.5 : 1.0) : p.sym;
+        Role r; r.kind = p.kind; std::memcpy(r.par, p.par, sizeof r.par); r.sym = sym; r.process = i;
+        r.s[0] = p.a; r.s[1] = p.b; r.s[2] = p.c; r.s[3] = p.d;
+        H->roles.push_back(r); H->role_off.push_back(roff); roff += (size_t)nx * H->np[p.a];
+        if (p.b != p.a) {
+            r.s[0] = p.b; r.s[1] = p.a; r.s[2] = p.d; r.s[3] = p.c;
+            H->roles.push_back(r); H->role_off.push_back(roff); roff += (size_t)nx * H->np[p.b];
+        }
+    }
+    H->role_off.push_back(roff);
+    return H;
+}
+
+void orc_destroy(void* h) { delete (Handle*)h; }
+size_t orc_f_elems(const void* h) { const Handle* H = (const Handle*)h; return H->sp_off.back() + (size_t)H->nx * H->np.back(); }
+size_t orc_species_offset(const void* h, int s) { return ((const Handle*)h)->sp_off[s]; }
+int orc_n_roles(const void* h) { return (int)((const Handle*)h)->roles.size(); }
+size_t orc_detail_elems(const void* h) { return ((const Handle*)h)->role_off.back(); }
+size_t orc_role_offset(const void* h, int r) { return ((const Handle*)h)->role_off[r]; }
+void orc_role_info(const void* h, int r, int s_out[4], int* kind, double* sym, int* process) {
+    const Role& R = ((const Handle*)h)->roles[r];
+    for (int i = 0; i < 4; ++i) s_out[i] = R.s[i];
+    *kind = R.kind; *sym = R.sym; *process = R.process;
+}
+int orc_threads() {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+// Full sweep over spatial cells ix_begin, ix_begin+stride, ... < ix_end.  C has orc_f_elems
+// doubles (only the visited cells are written).  detail arrays (may be null) have
+// orc_detail_elems doubles: scaled gain, loss, in-box loss and the sum of squared per-sample
+// contributions (for the Monte Carlo standard error), per (role, ix, p1).
+// fcb != null switches to analytic-f mode: every f value comes from fcb(species, p, user);
+// box_cut != 0 keeps the "zero outside the momentum box" rule in that mode.
+int orc_collision(void* h, const double* f, double* C, int n_samples, uint64_t seed, int ix_begin, int ix_end,
+                  int ix_stride, double* dG, double* dL, double* dLin, double* dQ, FCallback fcb, void* user,
+                  int box_cut) {
+    Handle* H = (Handle*)h;
+    if (n_samples <= 0 || ix_begin < 0 || ix_end > H->nx || ix_stride <= 0) return -1;
+    if (H->use_float)
+        return run_collision<float>(*H, f, C, n_samples, seed, ix_begin, ix_end, ix_stride, dG, dL, dLin, dQ, fcb, user, box_cut);
+    return run_collision<double>(*H, f, C, n_samples, seed, ix_begin, ix_end, ix_stride, dG, dL, dLin, dQ, fcb, user, box_cut);
+}
+
+// One p1 only (analytic or grid mode): returns scaled G, Ls, Lin, Q for (role, ix, ip1).
+int orc_collision_point(void* h, const double* f, int role, int ix, int ip1, int n_samples, uint64_t seed,
+                        double out[4], FCallback fcb, void* user, int box_cut) {
+    Handle* H = (Handle*)h;
+    Accum acc; double pref;
+    if (H->use_float) { Evaluator<float> ev(*H, role, fcb, user, box_cut); ev.eval_p1(f, ix, ip1, n_samples, seed, acc, nullptr, -1); pref = ev.prefactor(ip1, n_samples); }
+    else { Evaluator<double> ev(*H, role, fcb, user, box_cut); ev.eval_p1(f, ix, ip1, n_samples, seed, acc, nullptr, -1); pref = ev.prefactor(ip1, n_samples); }
+    out[0] = pref * acc.G; out[1] = pref * acc.Ls; out[2] = pref * acc.Lin; out[3] = pref * pref * acc.Q;
+    return 0;
+}
+
+// Kinematics of sample n of (role, ix, ip1): 27 doubles + 5 ints, see struct Trace.
+int orc_trace(void* h, const double* f, int role, int ix, int ip1, int n, uint64_t seed, double* dout, int* iout,
+              FCallback fcb, void* user, int box_cut) {
+    Handle* H = (Handle*)h;
+    Trace tr; Accum acc;
+    if (H->use_float) { Evaluator<float> ev(*H, role, fcb, user, box_cut); ev.eval_p1(f, ix, ip1, n + 1, seed, acc, &tr, n); }
+    else { Evaluator<double> ev(*H, role, fcb, user, box_cut); ev.eval_p1(f, ix, ip1, n + 1, seed, acc, &tr, n); }
+    std::memcpy(dout, &tr, 25 * sizeof(double));
+    iout[0] = tr.j2; iout[1] = tr.j3; iout[2] = tr.j4; iout[3] = tr.status; iout[4] = tr.draws;
+    return 0;
+}
+
+// O-update (Eq. 27; positivity PAPER.md:263): f_out = f + dt*C, count f_out < 0.
+long orc_update(size_t n, const double* f, const double* C, double dt, double* f_out) {
+    long neg = 0;
+    for (size_t i = 0; i < n; ++i) { f_out[i] = f[i] + dt * C[i]; if (f_out[i] < 0.0) ++neg; }
+    return neg;
+}
+
+}  // extern "C"

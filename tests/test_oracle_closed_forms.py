@@ -1,0 +1,69 @@
+"""P3 / P4: the oracle's loss rate against a closed form and against a scipy quadrature
+(Eq. 20-22: loss = f1 * Int f2 sigma_tot v_Moller)."""
+import math
+
+import numpy as np
+import pytest
+from scipy import integrate
+
+import oracle
+from conftest import read_golden
+
+
+def _one_species(m, n, lo, hi, kind=0, par=(1.0,), sym=-1.0):
+    return dict(nx=1, species=[dict(mass=m, charge=0, stat=0, g=1.0)],
+                grids=[dict(n=[n] * 3, pmin=[lo] * 3, pmax=[hi] * 3)],
+                processes=[dict(a=0, b=0, c=0, d=0, kind=kind, par=list(par), sym=sym)], hbar=1.0)
+
+
+def _loss_with_error(o, ip1, fcb, seed, batches=16, n=1 << 20):
+    """Mean and empirical standard error of the scaled loss over independent Philox keys."""
+    Ls = np.array([o.point(None, 0, 0, ip1, n, seed + 1000 * i, fcb=fcb, box_cut=False)[1] for i in range(batches)])
+    return Ls.mean(), Ls.std(ddof=1) / math.sqrt(batches)
+
+
+def test_p3_massless_closed_form():
+    """Massless, classical, constant |M|^2, f2 = exp(-|p|/T): rate/f1 = sym |M|^2 T^2 / (8 E1)."""
+    T, M2 = 0.5, 2.5
+    prob = _one_species(0.0, 24, -6.0, 6.0, par=(M2,))          # sym=-1 -> paper rule 1/2 (a == b)
+    o = oracle.Oracle(prob)
+    thermal = ("thermal", [[1.0, T, 0.0, 0.0, 0.0, 0, 0, 0]])
+    for ip1 in ((13 * 24 + 9) * 24 + 16, (11 * 24 + 12) * 24 + 12):
+        tr = o.trace(None, 0, 0, ip1, 0, 1, fcb=thermal, box_cut=False)
+        exact = 0.5 * M2 * T * T / (8 * tr["E1"]) * tr["f1"]
+        L, se = _loss_with_error(o, ip1, thermal, 4242 + ip1)
+        assert se < 0.02 * exact
+        assert abs(L - exact) < 4 * se + 1e-3 * exact, (L, exact, se)
+
+
+def _rate_quadrature(p1, m, T):
+    """Int d3p2 exp(-E2/T) |p*| / (16 pi E1 E2 sqrt s), spherical coordinates about p1."""
+    a1 = math.sqrt(p1 @ p1)
+    E1 = math.sqrt(a1 * a1 + m * m)
+
+    def integrand(c, q):
+        E2 = math.sqrt(q * q + m * m)
+        s = 2 * m * m + 2 * (E1 * E2 - a1 * q * c)
+        pst = math.sqrt(max(s * (s - 4 * m * m), 0.0)) / (2 * math.sqrt(s))
+        return 2 * math.pi * q * q * math.exp(-E2 / T) * pst / (16 * math.pi * E1 * E2 * math.sqrt(s))
+    val, err = integrate.dblquad(integrand, 0.0, 40.0 * T, -1.0, 1.0, epsabs=1e-12, epsrel=1e-10)
+    return val
+
+
+def test_p4_golden_value_reproduced_by_scipy():
+    gold = float(read_golden("closed_forms.txt")["p4_rate_over_f1"])
+    assert _rate_quadrature(np.array([0.3, -0.7, 1.1]), 1.0, 1.0) == pytest.approx(gold, rel=2e-6)
+
+
+def test_p4_massive_loss_rate_matches_scipy():
+    m, T = 1.0, 0.8
+    prob = _one_species(m, 120, -12.0, 12.0, sym=1.0)
+    o = oracle.Oracle(prob)
+    thermal = ("thermal", [[1.0, T, 0.0, m, 0.0, 0, 0, 0]])
+    ip1 = (61 * 120 + 56) * 120 + 65
+    tr = o.trace(None, 0, 0, ip1, 0, 1, fcb=thermal, box_cut=False)
+    assert np.allclose(tr["p1"], [0.3, -0.7, 1.1], atol=1e-12)
+    ref = _rate_quadrature(tr["p1"], m, T) * tr["f1"]
+    L, se = _loss_with_error(o, ip1, thermal, 777)
+    assert se < 0.02 * ref
+    assert abs(L - ref) < 4 * se + 1e-3 * ref, (L, ref, se)
