@@ -1,0 +1,130 @@
+/*
+ * rbg.h -- C ABI of the B200-native collision-term library (librbg.so).
+ *
+ * One thing is computed: the Monte Carlo evaluation of the relativistic 2->2 Boltzmann collision
+ * term C_a[f](x,p1) at every phase-space cell -- Eq. 16 of arXiv 2308.04869
+ * with the quantum factors of Eq. 18, summed over processes with the symmetry
+ * factor of Eq. 19 -- and, optionally, the explicit collision update
+ * f += dt*C of Eq. 27 with a count of cells that went negative.
+ * The paper hands this integral to an external GPU Monte Carlo package; the
+ * estimator, sampler and arithmetic order implemented here are fixed in DESIGN.md sections 2-4.
+ *
+ * Conventions
+ *   - hbar = c = 1 (as in the paper's own collision test); `hbar` below enters only
+ *     the occupation number nbar = (2 pi hbar)^3 f / g of Eq. 18.
+ *   - All pointers named *_dev are DEVICE pointers (cudaMalloc / torch CUDA tensors); pointers
+ *     named *_host are HOST pointers; everything else (structs, out-params) is host memory.
+ *   - Layout of f, C, f_out: one contiguous array of doubles, species-major, then spatial cell,
+ *     then momentum cell with pz fastest:
+ *         index(s, ix, ipx, ipy, ipz) = off(s) + ix*Np(s) + (ipx*n_y(s) + ipy)*n_z(s) + ipz,
+ *         off(s) = sum_{s'<s} Nx*Np(s'),   Np(s) = n_x(s) n_y(s) n_z(s),   Nx = nx*ny*nz,
+ *     i.e. the paper's [nx,ny,nz,npx,npy,npz] array per species,
+ *     concatenated over species.  Momentum cell centres: p_d = pmin_d + (i_d + 1/2) (pmax_d-pmin_d)/n_d.
+ *   - Ownership: the caller owns every buffer it passes and must keep device buffers alive until
+ *     the work queued on `cuda_stream` has completed.  The handle owns only its own scratch.
+ *   - Calls that take a stream are asynchronous on that stream (a cudaStream_t passed as void*;
+ *     NULL = the legacy default stream).  rbg_collision_host is synchronous.
+ *   - Errors: every int-returning entry point returns RBG_OK (0) or a negative RBG_E_* code; the
+ *     text is available from rbg_last_error().  No exception crosses this boundary.  There is no
+ *     CPU fallback: anything the CUDA path does not support is an error, never a slow path.
+ *   - Determinism: the result is a pure function of (f, the rbg_create arguments, n_samples, seed);
+ *     it does not depend on the stream, the launch geometry (rbg_set_option) or how spatial cells
+ *     are partitioned across calls or GPUs (the sample stream is keyed by the global cell index).
+ */
+#ifndef RBG_H_
+#define RBG_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RBG_OK             0
+#define RBG_E_INVALID_ARG (-1)
+#define RBG_E_UNSUPPORTED (-2)
+#define RBG_E_CUDA        (-3)
+
+/* rbg_create flags */
+#define RBG_FP64            0   /* sampling, kinematics and accumulation in fp64 (configs 1-4)        */
+#define RBG_FP32_KINEMATICS 1   /* fp32 sampling + kinematics, fp64 accumulation (config 5)           */
+
+typedef struct rbg_handle rbg_handle;   /* opaque; created by rbg_create, freed by rbg_destroy */
+
+/* Only the number of spatial cells matters: Eq. 16 is local in x (all four distributions are taken
+ * at the same (t,x)).  ix_offset is added to the local cell index when keying
+ * the sample stream, so that a shard holding cells [ix_offset, ix_offset+nx*ny*nz) of a larger
+ * domain reproduces the single-GPU result. */
+typedef struct { int nx, ny, nz; int ix_offset; } rbg_spatial_grid;
+
+/* Uniform, cell-centred Cartesian momentum grid of one species. */
+typedef struct { int n[3]; double pmin[3]; double pmax[3]; } rbg_momentum_grid;
+
+/* stat: 0 Boltzmann, +1 Bose-Einstein, -1 Fermi-Dirac (theta of Eq. 18); g: degrees of freedom
+ * (Eq. 18: electrons 2, photons 1, quarks 6, gluons 16).  charge is carried for completeness; the
+ * collision term does not use it. */
+typedef struct { double mass; double charge; int stat; double g; } rbg_species;
+
+typedef enum {
+    RBG_M2_CONST            = 0,  /* |M|^2 = par[0]                                   */
+    RBG_M2_COULOMB_SCREENED = 1,  /* |M|^2 = par[0] / (t - par[1]^2)^2                */
+    RBG_M2_TCHAN_S2         = 2   /* |M|^2 = par[0]^4 s^2 / (t - par[1]^2)^2   (Table III t-channel
+                                     form with regulator)          */
+} rbg_m2_kind;
+
+/* Process a + b -> c + d (species indices).  Only elastic processes (c == a, d == b) are
+ * implemented; anything else is RBG_E_UNSUPPORTED.  sym < 0 selects the paper's rule
+ * (PAPER.md:208): 1/2 if a == b, else 1. */
+typedef struct { int a, b, c, d; int kind; double par[4]; double sym; } rbg_process;
+
+/* Create a handle.  Returns RBG_OK and stores the handle in *out, or a negative code (then *out
+ * is NULL and rbg_last_error(NULL) has the text).  Rejects: non-positive grid counts,
+ * pmax <= pmin, negative mass, stat not in {0,+1,-1}, g <= 0, species index out of range,
+ * unknown kind or flags, inelastic processes, more than 255 roles, no CUDA device. */
+int rbg_create(rbg_handle** out, const rbg_spatial_grid* grid, int n_species, const rbg_species* species,
+               const rbg_momentum_grid* momentum_grids /* [n_species] */, int n_process,
+               const rbg_process* processes, double hbar, int flags);
+
+/* C_dev[all cells] = collision term of f_dev (C_dev is overwritten, not accumulated into).
+ * n_samples Monte Carlo samples per (role, spatial cell, momentum cell); seed keys the Philox
+ * streams.  f_dev and C_dev hold rbg_f_elems() doubles and must not overlap. */
+int rbg_collision(rbg_handle* h, const double* f_dev, double* C_dev, int n_samples, uint64_t seed,
+                  void* cuda_stream);
+
+/* Fused explicit Euler step of Eq. 27: f_out_dev = f_dev + dt * C[f_dev].  *neg_flag_dev (one int in
+ * device memory, zeroed by the caller) is incremented by the number of cells with f_out < 0; f_out
+ * is stored unclamped (policy is the caller's).  f_out_dev must not alias f_dev. */
+int rbg_collision_update(rbg_handle* h, const double* f_dev, double* f_out_dev, double dt, int* neg_flag_dev,
+                         int n_samples, uint64_t seed, void* cuda_stream);
+
+/* Same as rbg_collision with HOST buffers: copies f_host to the device (handle-owned scratch),
+ * runs the kernels, copies C back, synchronises.  Pinned host memory makes the copies faster but
+ * is not required. */
+int rbg_collision_host(rbg_handle* h, const double* f_host, double* C_host, int n_samples, uint64_t seed);
+
+/* Number of doubles in f / C / f_out. */
+size_t rbg_f_elems(const rbg_handle* h);
+/* Number of roles (a process seen from one grid species; a+b with a != b gives two). */
+int rbg_n_roles(const rbg_handle* h);
+/* roles * Nx * Np * n_samples summed over roles: the "collision samples" one sweep evaluates. */
+uint64_t rbg_sample_evals(const rbg_handle* h, int n_samples);
+/* Kernels launched by the most recent rbg_collision* call on this handle. */
+int rbg_last_launch_count(const rbg_handle* h);
+/* Launch geometry / gather path knobs (results do not depend on them).  key: "warps_per_cta"
+ * (1..32), "p1_per_cta" (momentum cells per CTA, >= 1), "gather" (0 auto, 1 shared memory,
+ * 2 global/L2).  Returns RBG_E_INVALID_ARG for an unknown key or bad value. */
+int rbg_set_option(rbg_handle* h, const char* key, int value);
+/* Text of the last error on this handle (or of the last failed rbg_create if h is NULL). */
+const char* rbg_last_error(const rbg_handle* h);
+void rbg_destroy(rbg_handle* h);
+
+/* Measurement helper: runs a register-resident chain of independent FMAs on every SM and reports
+ * the achieved rate.  what: 0 = fp64 FMA, 1 = fp32 FMA, 2 = int32 multiply-add.  *ops_per_s counts
+ * one FMA as one operation.  Used by bench.py for the live roofline denominator. */
+int rbg_probe_alu_peak(int what, int iters, double* ops_per_s, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RBG_H_ */

@@ -1,0 +1,184 @@
+"""ctypes marshalling for librbg.so; names follow include/rbg.h one to one."""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+
+KIND_CONST, KIND_COULOMB_SCREENED, KIND_TCHAN_S2 = 0, 1, 2
+RBG_FP64, RBG_FP32_KINEMATICS = 0, 1
+
+_PKG = Path(__file__).resolve().parent
+_LIB_PATH = _PKG / "librbg.so"
+_lib = None
+
+
+class RbgError(RuntimeError):
+    pass
+
+
+class _SpatialGrid(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("ix_offset", C.c_int)]
+
+
+class _MomentumGrid(C.Structure):
+    _fields_ = [("n", C.c_int * 3), ("pmin", C.c_double * 3), ("pmax", C.c_double * 3)]
+
+
+class _Species(C.Structure):
+    _fields_ = [("mass", C.c_double), ("charge", C.c_double), ("stat", C.c_int), ("g", C.c_double)]
+
+
+class _Process(C.Structure):
+    _fields_ = [("a", C.c_int), ("b", C.c_int), ("c", C.c_int), ("d", C.c_int), ("kind", C.c_int),
+                ("par", C.c_double * 4), ("sym", C.c_double)]
+
+
+# every symbol include/rbg.h declares
+_SIGNATURES = {
+    "rbg_create": (C.c_int, [C.POINTER(C.c_void_p), C.POINTER(_SpatialGrid), C.c_int, C.POINTER(_Species),
+                             C.POINTER(_MomentumGrid), C.c_int, C.POINTER(_Process), C.c_double, C.c_int]),
+    "rbg_collision": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_uint64, C.c_void_p]),
+    "rbg_collision_update": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_int,
+                                       C.c_uint64, C.c_void_p]),
+    "rbg_collision_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_uint64]),
+    "rbg_f_elems": (C.c_size_t, [C.c_void_p]),
+    "rbg_n_roles": (C.c_int, [C.c_void_p]),
+    "rbg_sample_evals": (C.c_uint64, [C.c_void_p, C.c_int]),
+    "rbg_last_launch_count": (C.c_int, [C.c_void_p]),
+    "rbg_set_option": (C.c_int, [C.c_void_p, C.c_char_p, C.c_int]),
+    "rbg_last_error": (C.c_char_p, [C.c_void_p]),
+    "rbg_destroy": (None, [C.c_void_p]),
+    "rbg_probe_alu_peak": (C.c_int, [C.c_int, C.c_int, C.POINTER(C.c_double), C.c_void_p]),
+}
+
+
+def exported_symbols():
+    return sorted(_SIGNATURES)
+
+
+def load_library():
+    """Load librbg.so; raises RbgError if it has not been built (no fallback of any kind)."""
+    global _lib
+    if _lib is None:
+        if not _LIB_PATH.exists():
+            raise RbgError(f"{_LIB_PATH} is missing: run `python -m paper_2308_04869_b200.build` "
+                           "(there is no CPU fallback)")
+        lib = C.CDLL(str(_LIB_PATH))
+        for name, (res, args) in _SIGNATURES.items():
+            fn = getattr(lib, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = lib
+    return _lib
+
+
+def _check(rc, handle=None):
+    if rc != 0:
+        msg = load_library().rbg_last_error(handle)
+        raise RbgError(f"librbg error {rc}: {msg.decode() if msg else ''}")
+
+
+def probe_alu_peak(what: int, iters: int = 1 << 16, stream=None) -> float:
+    """FMA/s (one FMA = one op) of a register-resident chain: 0 fp64, 1 fp32, 2 int32."""
+    out = C.c_double()
+    _check(load_library().rbg_probe_alu_peak(what, iters, C.byref(out), _stream_ptr(stream)))
+    return out.value
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    return C.c_void_p(getattr(stream, "cuda_stream", stream))
+
+
+class Collision:
+    """One problem (spatial cells, species, momentum grids, processes) on the current CUDA device.
+
+    ``problem`` is a plain dict: nx (number of spatial cells, or (nx,ny,nz)), species [dict(mass,
+    charge, stat, g)], grids [dict(n, pmin, pmax)], processes [dict(a,b,c,d,kind,par,sym)], hbar.
+    """
+
+    def __init__(self, problem: dict, fp32_kinematics: bool = False, ix_offset: int = 0):
+        lib = load_library()
+        nx = problem["nx"]
+        nxyz = (int(nx), 1, 1) if np.isscalar(nx) else tuple(int(v) for v in nx)
+        sg = _SpatialGrid(*nxyz, int(ix_offset))
+        sp, gr, pr = problem["species"], problem["grids"], problem["processes"]
+        S = (_Species * len(sp))(*[_Species(s["mass"], s.get("charge", 0.0), s["stat"], s.get("g", 1.0)) for s in sp])
+        G = (_MomentumGrid * len(gr))(*[_MomentumGrid((C.c_int * 3)(*g["n"]), (C.c_double * 3)(*g["pmin"]),
+                                                      (C.c_double * 3)(*g["pmax"])) for g in gr])
+        P = (_Process * max(len(pr), 1))(*[_Process(p["a"], p["b"], p["c"], p["d"], p["kind"],
+                                                    (C.c_double * 4)(*(list(p["par"]) + [0.0] * 4)[:4]),
+                                                    p.get("sym", -1.0)) for p in pr])
+        h = C.c_void_p()
+        _check(lib.rbg_create(C.byref(h), C.byref(sg), len(sp), S, G, len(pr), P, float(problem.get("hbar", 1.0)),
+                              RBG_FP32_KINEMATICS if fp32_kinematics else RBG_FP64))
+        self._h = h
+        self.f_elems = int(lib.rbg_f_elems(h))
+        self.n_roles = int(lib.rbg_n_roles(h))
+
+    def __del__(self):
+        h = getattr(self, "_h", None)
+        if h:
+            load_library().rbg_destroy(h)
+            self._h = None
+
+    # -- helpers ---------------------------------------------------------------------------------
+    def _dev(self, t, name):
+        import torch
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+                and t.numel() == self.f_elems):
+            raise RbgError(f"{name} must be a contiguous float64 CUDA tensor with {self.f_elems} elements")
+        return C.c_void_p(t.data_ptr())
+
+    def sample_evals(self, n_samples: int) -> int:
+        return int(load_library().rbg_sample_evals(self._h, int(n_samples)))
+
+    def last_launch_count(self) -> int:
+        return int(load_library().rbg_last_launch_count(self._h))
+
+    def set_option(self, key: str, value: int):
+        _check(load_library().rbg_set_option(self._h, key.encode(), int(value)), self._h)
+
+    # -- the hot path ----------------------------------------------------------------------------
+    def collision(self, f, n_samples: int, seed: int, out=None, stream=None):
+        """rbg_collision: C[f] for every cell (torch CUDA tensors; asynchronous on the stream)."""
+        import torch
+        if out is None:
+            out = torch.empty_like(f)
+        _check(load_library().rbg_collision(self._h, self._dev(f, "f"), self._dev(out, "out"), int(n_samples),
+                                            int(seed), _stream_ptr(stream)), self._h)
+        return out
+
+    def collision_update(self, f, dt: float, n_samples: int, seed: int, out=None, neg_flag=None, stream=None):
+        """rbg_collision_update: f_out = f + dt*C[f]; neg_flag (int32 CUDA tensor) += #cells with f_out < 0."""
+        import torch
+        if out is None:
+            out = torch.empty_like(f)
+        if neg_flag is None:
+            neg_flag = torch.zeros(1, dtype=torch.int32, device=f.device)
+        _check(load_library().rbg_collision_update(self._h, self._dev(f, "f"), self._dev(out, "out"), float(dt),
+                                                   C.c_void_p(neg_flag.data_ptr()), int(n_samples), int(seed),
+                                                   _stream_ptr(stream)), self._h)
+        return out, neg_flag
+
+    def collision_host(self, f_host, n_samples: int, seed: int, out=None):
+        """rbg_collision_host: host buffers in, host buffers out (numpy float64 or pinned CPU tensors)."""
+        import torch
+        def ptr(a, name):
+            if isinstance(a, torch.Tensor):
+                ok = (not a.is_cuda) and a.dtype == torch.float64 and a.is_contiguous() and a.numel() == self.f_elems
+                p = a.data_ptr()
+            else:
+                ok = a.dtype == np.float64 and a.flags.c_contiguous and a.size == self.f_elems
+                p = a.ctypes.data
+            if not ok:
+                raise RbgError(f"{name} must be a contiguous float64 host array with {self.f_elems} elements")
+            return C.c_void_p(p)
+        if out is None:
+            out = torch.empty_like(f_host) if isinstance(f_host, torch.Tensor) else np.empty_like(f_host)
+        _check(load_library().rbg_collision_host(self._h, ptr(f_host, "f_host"), ptr(out, "out"), int(n_samples),
+                                                 int(seed)), self._h)
+        return out

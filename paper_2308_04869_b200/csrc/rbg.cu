@@ -1,0 +1,358 @@
+// rbg.cu -- host side of librbg.so: the C ABI of include/rbg.h over the kernels in rbg_kernels.cuh.
+//
+// Validation, role expansion (Eq. 19), role constants, launch
+// geometry.  No CPU fallback: every step of the path runs in the CUDA kernels; this file only
+// marshals.  Shares no code with oracle/.
+#include "../../include/rbg.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "rbg_kernels.cuh"
+
+namespace {
+
+thread_local std::string g_create_error;
+
+struct Role {
+    int s1, s2;            // grid species, partner species (elastic: s3 = s1, s4 = s2)
+    int kind;
+    double par[4];
+    double sym;
+    int index;             // global role index
+};
+
+}  // namespace
+
+struct rbg_handle {
+    int nx = 0, ix_offset = 0;
+    int n_species = 0;
+    std::vector<rbg_species> species;
+    std::vector<rbg_momentum_grid> grids;
+    std::vector<size_t> np, sp_off;
+    std::vector<Role> roles;
+    size_t f_elems = 0;
+    double hbar = 1.0;
+    int flags = 0;
+    int device = 0;
+    int sm_count = 148;
+    int max_smem_optin = 0;
+    // options
+    int opt_warps = 0, opt_p1_per_cta = 0, opt_gather = 0;
+    int last_launches = 0;
+    // scratch for the host entry point
+    double *scratch_f = nullptr, *scratch_c = nullptr;
+    size_t scratch_elems = 0;
+    mutable std::string err;
+};
+
+namespace {
+
+int fail(rbg_handle* h, int code, const std::string& msg) {
+    if (h) h->err = msg; else g_create_error = msg;
+    return code;
+}
+
+#define RBG_CUDA(h, call)                                                                          \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(h, RBG_E_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_));        \
+    } while (0)
+
+// Role constants: the formulas of DESIGN.md section 4 ("role constants"), evaluated in double and then
+// rounded to R.
+template <typename R>
+rbg::RoleParams<R> make_role_params(const rbg_handle& H, const Role& r) {
+    rbg::RoleParams<R> k;
+    std::memset(&k, 0, sizeof k);
+    const int sl[4] = {r.s1, r.s2, r.s1, r.s2};
+    double m[4];
+    for (int i = 0; i < 4; ++i) m[i] = H.species[sl[i]].mass;
+    const double msum = m[0] + m[1], m34 = m[2] + m[3], md = m[2] - m[3];
+    k.m1 = (R)m[0]; k.m2 = (R)m[1];
+    k.msq1 = (R)(m[0] * m[0]); k.msq2 = (R)(m[1] * m[1]);
+    k.m1m2 = (R)(m[0] * m[1]);
+    k.msum2 = (R)(msum * msum);
+    k.Mth = (R)(msum * msum - m34 * m34);
+    k.Mdf = (R)(md * md);
+    k.dm34 = (R)(m[2] * m[2] - m[3] * m[3]);
+    const rbg_momentum_grid& g1 = H.grids[r.s1];
+    const rbg_momentum_grid& g2 = H.grids[r.s2];
+    double V2 = 1.0;
+    for (int d = 0; d < 3; ++d) {
+        const double L1 = g1.pmax[d] - g1.pmin[d], L2 = g2.pmax[d] - g2.pmin[d];
+        const double invD1 = (double)g1.n[d] / L1, invD2 = (double)g2.n[d] / L2;
+        k.pmin1[d] = (R)g1.pmin[d];
+        k.delta1[d] = (R)(L1 / (double)g1.n[d]);
+        k.pmin2[d] = (R)g2.pmin[d];
+        k.L2[d] = (R)L2;
+        k.invD3[d] = (R)invD1; k.off3[d] = (R)(-g1.pmin[d] * invD1);
+        k.invD4[d] = (R)invD2; k.off4[d] = (R)(-g2.pmin[d] * invD2);
+        k.n1[d] = k.n3[d] = g1.n[d];
+        k.n2[d] = k.n4[d] = g2.n[d];
+    }
+    V2 = (g2.pmax[0] - g2.pmin[0]) * (g2.pmax[1] - g2.pmin[1]) * (g2.pmax[2] - g2.pmin[2]);
+    const double tph = 2.0 * M_PI * H.hbar;
+    const double tk1 = (double)H.species[r.s1].stat * (tph * tph * tph) / H.species[r.s1].g;
+    const double tk2 = (double)H.species[r.s2].stat * (tph * tph * tph) / H.species[r.s2].g;
+    k.tk1 = k.tk3 = (R)tk1;
+    k.tk2 = k.tk4 = (R)tk2;
+    k.par0 = (R)r.par[0];
+    k.mD2 = (R)(r.par[1] * r.par[1]);
+    const double g2c = r.par[0] * r.par[0];
+    k.g4 = (R)(g2c * g2c);
+    k.symV2 = r.sym * V2;
+    k.np1 = (int)H.np[r.s1]; k.np2 = (int)H.np[r.s2]; k.np3 = k.np1;
+    k.role = r.index;
+    k.same_species = r.s1 == r.s2;
+    return k;
+}
+
+template <typename R, int KIND, bool Q, bool SMEM>
+cudaError_t launch_one(const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp, int grid, int threads, size_t smem,
+                       cudaStream_t st) {
+    auto kern = rbg::collision_role_kernel<R, KIND, Q, SMEM>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    kern<<<grid, threads, smem, st>>>(rp, lp);
+    return cudaGetLastError();
+}
+
+template <typename R, int KIND>
+cudaError_t launch_kq(bool q, bool smem_path, const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp, int grid,
+                      int threads, size_t smem, cudaStream_t st) {
+    if (q) return smem_path ? launch_one<R, KIND, true, true>(rp, lp, grid, threads, smem, st)
+                            : launch_one<R, KIND, true, false>(rp, lp, grid, threads, smem, st);
+    return smem_path ? launch_one<R, KIND, false, true>(rp, lp, grid, threads, smem, st)
+                     : launch_one<R, KIND, false, false>(rp, lp, grid, threads, smem, st);
+}
+
+template <typename R>
+int run_roles(rbg_handle* h, const double* f, double* out, bool update, double dt, int* neg_flag, int n_samples,
+              uint64_t seed, cudaStream_t st) {
+    h->last_launches = 0;
+    // last role per species (update mode counts negatives there); species with no role: C = 0 / f_out = f
+    std::vector<int> first_role(h->n_species, -1), last_role(h->n_species, -1);
+    for (size_t i = 0; i < h->roles.size(); ++i) {
+        if (first_role[h->roles[i].s1] < 0) first_role[h->roles[i].s1] = (int)i;
+        last_role[h->roles[i].s1] = (int)i;
+    }
+    for (int s = 0; s < h->n_species; ++s) {
+        if (first_role[s] >= 0) continue;
+        const size_t n = (size_t)h->nx * h->np[s];
+        if (update) {
+            rbg::copy_count_kernel<<<h->sm_count * 4, 256, 0, st>>>(f + h->sp_off[s], out + h->sp_off[s], n, neg_flag);
+            RBG_CUDA(h, cudaGetLastError());
+            ++h->last_launches;
+        } else {
+            RBG_CUDA(h, cudaMemsetAsync(out + h->sp_off[s], 0, n * sizeof(double), st));
+        }
+    }
+    for (size_t i = 0; i < h->roles.size(); ++i) {
+        const Role& r = h->roles[i];
+        const rbg::RoleParams<R> rp = make_role_params<R>(*h, r);
+        const int warps = h->opt_warps > 0 ? h->opt_warps : 16;
+        long work = (long)h->nx * rp.np1;
+        int T = h->opt_p1_per_cta > 0 ? h->opt_p1_per_cta : (int)std::min<long>(512, std::max<long>(warps, work / ((long)h->sm_count * 8)));
+        T = std::min(T, rp.np1);
+        // shared memory: [16 B mbarrier][T doubles][table2][table1 if species differ]
+        const size_t tab2 = (((size_t)rp.np2 + 3) & ~(size_t)3) * sizeof(R);
+        const size_t tab1 = rp.same_species ? 0 : (size_t)rp.np1 * sizeof(R);
+        const size_t head = 16 + (((size_t)T * 8 + 15) & ~(size_t)15);
+        bool smem_path = head + tab2 + tab1 <= (size_t)h->max_smem_optin;
+        if (h->opt_gather == 1 && !smem_path) return fail(h, RBG_E_UNSUPPORTED, "gather=1 (shared memory) requested but the f tables do not fit");
+        if (h->opt_gather == 2) smem_path = false;
+        const size_t smem = head + (smem_path ? tab2 + tab1 : 0);
+        rbg::LaunchParams lp;
+        std::memset(&lp, 0, sizeof lp);
+        lp.f1_base = f + h->sp_off[r.s1];
+        lp.f2_base = f + h->sp_off[r.s2];
+        lp.out_base = out + h->sp_off[r.s1];
+        lp.nx_local = h->nx; lp.ix_offset = h->ix_offset; lp.n_samples = n_samples;
+        lp.key0 = (uint32_t)seed; lp.key1 = (uint32_t)(seed >> 32);
+        lp.p1_per_cta = T; lp.tiles = (rp.np1 + T - 1) / T;
+        lp.accumulate = first_role[r.s1] != (int)i;
+        lp.update = update; lp.dt = dt; lp.neg_flag = neg_flag;
+        lp.count_negative = update && last_role[r.s1] == (int)i;
+        const long grid = (long)lp.tiles * h->nx;
+        if (grid > 0x7fffffffL) return fail(h, RBG_E_UNSUPPORTED, "grid too large; raise p1_per_cta");
+        const bool q = h->species[r.s1].stat != 0 || h->species[r.s2].stat != 0;
+        cudaError_t e;
+        switch (r.kind) {
+            case RBG_M2_CONST: e = launch_kq<R, rbg::KIND_CONST>(q, smem_path, rp, lp, (int)grid, warps * 32, smem, st); break;
+            case RBG_M2_COULOMB_SCREENED: e = launch_kq<R, rbg::KIND_COULOMB>(q, smem_path, rp, lp, (int)grid, warps * 32, smem, st); break;
+            default: e = launch_kq<R, rbg::KIND_TCHAN_S2>(q, smem_path, rp, lp, (int)grid, warps * 32, smem, st); break;
+        }
+        if (e != cudaSuccess) return fail(h, RBG_E_CUDA, std::string("kernel launch: ") + cudaGetErrorString(e));
+        ++h->last_launches;
+    }
+    return RBG_OK;
+}
+
+int run(rbg_handle* h, const double* f, double* out, bool update, double dt, int* neg_flag, int n_samples, uint64_t seed,
+        void* stream) {
+    if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
+    if (!f || !out) return fail(h, RBG_E_INVALID_ARG, "null buffer");
+    if (f == out) return fail(h, RBG_E_INVALID_ARG, "output must not alias f");
+    if (n_samples <= 0) return fail(h, RBG_E_INVALID_ARG, "n_samples must be positive");
+    if (update && !neg_flag) return fail(h, RBG_E_INVALID_ARG, "null neg_flag_dev");
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = -1;
+    RBG_CUDA(h, cudaGetDevice(&dev));
+    if (dev != h->device) RBG_CUDA(h, cudaSetDevice(h->device));
+    int rc = (h->flags & RBG_FP32_KINEMATICS) ? run_roles<float>(h, f, out, update, dt, neg_flag, n_samples, seed, st)
+                                               : run_roles<double>(h, f, out, update, dt, neg_flag, n_samples, seed, st);
+    if (dev != h->device && dev >= 0) cudaSetDevice(dev);
+    return rc;
+}
+
+}  // namespace
+
+extern "C" {
+
+int rbg_create(rbg_handle** out, const rbg_spatial_grid* grid, int n_species, const rbg_species* species,
+               const rbg_momentum_grid* mg, int n_process, const rbg_process* processes, double hbar, int flags) {
+    if (!out) return fail(nullptr, RBG_E_INVALID_ARG, "out is null");
+    *out = nullptr;
+    if (!grid || !species || !mg || (n_process > 0 && !processes)) return fail(nullptr, RBG_E_INVALID_ARG, "null argument");
+    if (grid->nx <= 0 || grid->ny <= 0 || grid->nz <= 0 || grid->ix_offset < 0)
+        return fail(nullptr, RBG_E_INVALID_ARG, "spatial grid counts must be positive");
+    if ((long)grid->nx * grid->ny * grid->nz > 0x7fffffffL) return fail(nullptr, RBG_E_INVALID_ARG, "too many spatial cells");
+    if (n_species <= 0 || n_process < 0) return fail(nullptr, RBG_E_INVALID_ARG, "bad species/process count");
+    if (!(hbar > 0.0)) return fail(nullptr, RBG_E_INVALID_ARG, "hbar must be positive");
+    if (flags != RBG_FP64 && flags != RBG_FP32_KINEMATICS) return fail(nullptr, RBG_E_INVALID_ARG, "unknown flags");
+    rbg_handle* h = new rbg_handle;
+    h->nx = grid->nx * grid->ny * grid->nz;
+    h->ix_offset = grid->ix_offset;
+    h->n_species = n_species; h->hbar = hbar; h->flags = flags;
+    size_t off = 0;
+    for (int s = 0; s < n_species; ++s) {
+        const rbg_species& S = species[s];
+        const rbg_momentum_grid& G = mg[s];
+        std::string why;
+        if (!(S.mass >= 0.0)) why = "negative mass";
+        else if (S.stat != 0 && S.stat != 1 && S.stat != -1) why = "stat must be 0, +1 or -1";
+        else if (!(S.g > 0.0)) why = "g must be positive";
+        for (int d = 0; d < 3 && why.empty(); ++d) {
+            if (G.n[d] <= 0) why = "momentum grid counts must be positive";
+            else if (!(G.pmax[d] > G.pmin[d])) why = "pmax must exceed pmin";
+        }
+        const double npd = (double)G.n[0] * G.n[1] * G.n[2];
+        if (why.empty() && npd > 0x7fffffff) why = "too many momentum cells";
+        if (!why.empty()) { delete h; return fail(nullptr, RBG_E_INVALID_ARG, "species " + std::to_string(s) + ": " + why); }
+        h->species.push_back(S); h->grids.push_back(G);
+        h->np.push_back((size_t)npd); h->sp_off.push_back(off);
+        off += (size_t)h->nx * (size_t)npd;
+    }
+    h->f_elems = off;
+    for (int i = 0; i < n_process; ++i) {
+        const rbg_process& p = processes[i];
+        const int idx[4] = {p.a, p.b, p.c, p.d};
+        for (int j = 0; j < 4; ++j)
+            if (idx[j] < 0 || idx[j] >= n_species) { delete h; return fail(nullptr, RBG_E_INVALID_ARG, "process " + std::to_string(i) + ": species index out of range"); }
+        if (p.kind < RBG_M2_CONST || p.kind > RBG_M2_TCHAN_S2) { delete h; return fail(nullptr, RBG_E_INVALID_ARG, "process " + std::to_string(i) + ": unknown |M|^2 kind"); }
+        if (p.c != p.a || p.d != p.b) { delete h; return fail(nullptr, RBG_E_UNSUPPORTED, "process " + std::to_string(i) + ": only elastic processes (c==a, d==b) are implemented"); }
+        Role r;
+        r.kind = p.kind; std::memcpy(r.par, p.par, sizeof r.par);
+        r.sym = p.sym < 0 ? (p.a == p.b ? 0.5 : 1.0) : p.sym;
+        r.s1 = p.a; r.s2 = p.b; r.index = (int)h->roles.size();
+        h->roles.push_back(r);
+        if (p.b != p.a) { r.s1 = p.b; r.s2 = p.a; r.index = (int)h->roles.size(); h->roles.push_back(r); }
+    }
+    if (h->roles.size() > 255) { delete h; return fail(nullptr, RBG_E_UNSUPPORTED, "more than 255 roles"); }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { delete h; return fail(nullptr, RBG_E_CUDA, "no CUDA device (there is no CPU fallback)"); }
+    cudaGetDevice(&h->device);
+    cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, h->device);
+    cudaDeviceGetAttribute(&h->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device);
+    *out = h;
+    return RBG_OK;
+}
+
+int rbg_collision(rbg_handle* h, const double* f_dev, double* C_dev, int n_samples, uint64_t seed, void* cuda_stream) {
+    return run(h, f_dev, C_dev, false, 0.0, nullptr, n_samples, seed, cuda_stream);
+}
+
+int rbg_collision_update(rbg_handle* h, const double* f_dev, double* f_out_dev, double dt, int* neg_flag_dev,
+                         int n_samples, uint64_t seed, void* cuda_stream) {
+    return run(h, f_dev, f_out_dev, true, dt, neg_flag_dev, n_samples, seed, cuda_stream);
+}
+
+int rbg_collision_host(rbg_handle* h, const double* f_host, double* C_host, int n_samples, uint64_t seed) {
+    if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
+    if (!f_host || !C_host) return fail(h, RBG_E_INVALID_ARG, "null buffer");
+    if (h->scratch_elems < h->f_elems) {
+        cudaFree(h->scratch_f); cudaFree(h->scratch_c); h->scratch_f = h->scratch_c = nullptr; h->scratch_elems = 0;
+        RBG_CUDA(h, cudaMalloc(&h->scratch_f, h->f_elems * sizeof(double)));
+        RBG_CUDA(h, cudaMalloc(&h->scratch_c, h->f_elems * sizeof(double)));
+        h->scratch_elems = h->f_elems;
+    }
+    RBG_CUDA(h, cudaMemcpyAsync(h->scratch_f, f_host, h->f_elems * sizeof(double), cudaMemcpyHostToDevice, 0));
+    int rc = run(h, h->scratch_f, h->scratch_c, false, 0.0, nullptr, n_samples, seed, nullptr);
+    if (rc != RBG_OK) return rc;
+    RBG_CUDA(h, cudaMemcpyAsync(C_host, h->scratch_c, h->f_elems * sizeof(double), cudaMemcpyDeviceToHost, 0));
+    RBG_CUDA(h, cudaStreamSynchronize(0));
+    return RBG_OK;
+}
+
+size_t rbg_f_elems(const rbg_handle* h) { return h ? h->f_elems : 0; }
+int rbg_n_roles(const rbg_handle* h) { return h ? (int)h->roles.size() : 0; }
+uint64_t rbg_sample_evals(const rbg_handle* h, int n_samples) {
+    if (!h) return 0;
+    uint64_t t = 0;
+    for (const Role& r : h->roles) t += (uint64_t)h->nx * h->np[r.s1] * (uint64_t)n_samples;
+    return t;
+}
+int rbg_last_launch_count(const rbg_handle* h) { return h ? h->last_launches : 0; }
+
+int rbg_set_option(rbg_handle* h, const char* key, int value) {
+    if (!h || !key) return fail(h, RBG_E_INVALID_ARG, "null argument");
+    const std::string k(key);
+    if (k == "warps_per_cta") { if (value < 0 || value > 16) return fail(h, RBG_E_INVALID_ARG, "warps_per_cta must be 0 (auto) or 1..16"); h->opt_warps = value; }
+    else if (k == "p1_per_cta") { if (value < 0) return fail(h, RBG_E_INVALID_ARG, "p1_per_cta must be >= 0 (0 = auto)"); h->opt_p1_per_cta = value; }
+    else if (k == "gather") { if (value < 0 || value > 2) return fail(h, RBG_E_INVALID_ARG, "gather must be 0, 1 or 2"); h->opt_gather = value; }
+    else return fail(h, RBG_E_INVALID_ARG, "unknown option " + k);
+    return RBG_OK;
+}
+
+const char* rbg_last_error(const rbg_handle* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+void rbg_destroy(rbg_handle* h) {
+    if (!h) return;
+    cudaFree(h->scratch_f); cudaFree(h->scratch_c);
+    delete h;
+}
+
+int rbg_probe_alu_peak(int what, int iters, double* ops_per_s, void* cuda_stream) {
+    if (!ops_per_s || iters <= 0 || what < 0 || what > 2) return fail(nullptr, RBG_E_INVALID_ARG, "bad probe arguments");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    RBG_CUDA(nullptr, cudaGetDevice(&dev));
+    RBG_CUDA(nullptr, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int ctas = sms * 8, threads = 256;
+    void* buf = nullptr;
+    RBG_CUDA(nullptr, cudaMalloc(&buf, (size_t)ctas * threads * 8));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {            // rep 0 warms clocks and instruction cache
+        cudaEventRecord(e0, st);
+        if (what == 0) rbg::alu_probe_kernel<double><<<ctas, threads, 0, st>>>((double*)buf, 1.0000001, 1e-9, iters);
+        else if (what == 1) rbg::alu_probe_kernel<float><<<ctas, threads, 0, st>>>((float*)buf, 1.0000001f, 1e-9f, iters);
+        else rbg::alu_probe_kernel<unsigned><<<ctas, threads, 0, st>>>((unsigned*)buf, 2654435761u, 12345u, iters);
+        cudaEventRecord(e1, st);
+        cudaError_t e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) { cudaFree(buf); return fail(nullptr, RBG_E_CUDA, cudaGetErrorString(e)); }
+        float ms = 0; cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(buf);
+    *ops_per_s = (double)ctas * threads * 8.0 * (double)iters / (best * 1e-3);
+    return RBG_OK;
+}
+
+}  // extern "C"

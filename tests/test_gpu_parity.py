@@ -1,0 +1,221 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element on the same
+seeded inputs.  Bar (north_star): |C_gpu - C_oracle| <= 1e-10 (|gain| + |loss|) per cell in fp64;
+1e-4 of the same scale for the fp32-kinematics variant against the oracle's float chain."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-10
+TOL32 = 1e-4
+
+
+def _rbg():
+    import paper_2308_04869_b200 as rbg
+    return rbg
+
+
+def oracle_C_and_scale(orc, f, n_samples, seed, **kw):
+    """Oracle C and the per-cell tolerance scale sum_roles (G + L)."""
+    C_ref, d = orc.collision(f, n_samples, seed, detail=True, **kw)
+    mag = np.zeros_like(C_ref)
+    for r in range(orc.n_roles):
+        s1 = orc.roles[r]["s"][0]
+        n = orc.nx * orc.np[s1]
+        mag[orc.sp_off[s1]:orc.sp_off[s1] + n] += (d["G"] + d["L"])[orc.role_off[r]:orc.role_off[r] + n]
+    return C_ref, mag
+
+
+def gpu_C(problem, f, n_samples, seed, fp32=False, options=(), ix_offset=0):
+    rbg = _rbg()
+    col = rbg.Collision(problem, fp32_kinematics=fp32, ix_offset=ix_offset)
+    for k, v in options:
+        col.set_option(k, v)
+    ft = torch.from_numpy(np.ascontiguousarray(f)).cuda()
+    C = col.collision(ft, n_samples, seed)
+    torch.cuda.synchronize()
+    return C.cpu().numpy(), col
+
+
+def assert_parity(C, C_ref, mag, tol, what):
+    err = np.abs(C - C_ref)
+    bad = err > tol * mag
+    worst = np.max(err / np.maximum(mag, 1e-300))
+    assert not bad.any(), f"{what}: {bad.sum()} cells off, worst err/(G+L) = {worst:.3e}"
+    assert np.any(C_ref != 0), what
+
+
+CASES = [
+    # (config, overrides): sizes the oracle finishes in seconds that still span several p1 tiles,
+    # ragged tile tails, sample counts that are not a multiple of the warp size, odd grid sizes
+    # (7^3 = 343 cells: table size not a multiple of 16 bytes -> non-TMA staging path)
+    (1, dict()),                                             # BASELINE configs[0] at full size
+    (1, dict(nx=3, np_side=7, n_samples=100)),
+    (2, dict(nx=3, np_side=20, n_samples=64)),
+    (2, dict(nx=2, np_side=7, n_samples=33)),
+    (3, dict(nx=2, np_side=8, n_samples=96)),
+    (3, dict(nx=1, np_side=20, n_samples=16)),
+    (4, dict(nx=5, np_side=20, n_samples=100)),
+]
+
+
+@pytest.mark.parametrize("cfg,kw", CASES)
+def test_parity_fp64(cfg, kw):
+    w = workloads.make(cfg, **kw)
+    orc = oracle.Oracle(w["problem"])
+    C_ref, mag = oracle_C_and_scale(orc, w["f"], w["n_samples"], w["seed"])
+    C, col = gpu_C(w["problem"], w["f"], w["n_samples"], w["seed"])
+    assert_parity(C, C_ref, mag, TOL64, f"cfg{cfg} {kw}")
+    assert col.last_launch_count() == orc.n_roles
+    assert col.sample_evals(w["n_samples"]) == workloads.configs.sample_evals(w["problem"], w["n_samples"])
+
+
+@pytest.mark.parametrize("cfg,kw", [(1, dict(nx=2, np_side=8, n_samples=128)), (2, dict(nx=2, np_side=10, n_samples=64)),
+                                    (3, dict(nx=1, np_side=8, n_samples=64))])
+def test_parity_fp32_kinematics(cfg, kw):
+    w = workloads.make(cfg, **kw)
+    orc = oracle.Oracle(w["problem"], use_float=True)
+    C_ref, mag = oracle_C_and_scale(orc, w["f"], w["n_samples"], w["seed"])
+    C, _ = gpu_C(w["problem"], w["f"], w["n_samples"], w["seed"], fp32=True)
+    assert_parity(C, C_ref, mag, TOL32, f"fp32 cfg{cfg}")
+
+
+def test_result_independent_of_launch_geometry_and_gather_path():
+    """Determinism contract of include/rbg.h: each p1 is reduced by one warp in a fixed lane order, so
+    the result is bit-identical for any tile size, CTA size and gather path."""
+    w = workloads.make(2, nx=2, np_side=12, n_samples=80)
+    base, _ = gpu_C(w["problem"], w["f"], w["n_samples"], w["seed"])
+    for opts in ([("warps_per_cta", 3), ("p1_per_cta", 5)], [("warps_per_cta", 8), ("p1_per_cta", 1000)],
+                 [("gather", 2)], [("gather", 2), ("warps_per_cta", 1), ("p1_per_cta", 1)]):
+        other, _ = gpu_C(w["problem"], w["f"], w["n_samples"], w["seed"], options=opts)
+        assert np.array_equal(base, other), opts
+
+
+def test_spatial_sharding_reproduces_the_single_device_result():
+    """Section 8(e): spatial cells are independent; the stream is keyed by the global cell index."""
+    w = workloads.make(2, nx=5, np_side=8, n_samples=48)
+    full, _ = gpu_C(w["problem"], w["f"], w["n_samples"], w["seed"])
+    offs, total = workloads.f_layout(w["problem"])
+    for lo, hi in ((0, 2), (2, 5)):
+        prob = dict(w["problem"], nx=hi - lo)
+        parts_in, parts_ref = [], []
+        for s, g in enumerate(w["problem"]["grids"]):
+            npc = int(np.prod(g["n"]))
+            blk = w["f"][offs[s]:offs[s] + 5 * npc].reshape(5, npc)
+            parts_in.append(blk[lo:hi].reshape(-1))
+            parts_ref.append(full[offs[s]:offs[s] + 5 * npc].reshape(5, npc)[lo:hi].reshape(-1))
+        shard, _ = gpu_C(prob, np.concatenate(parts_in), w["n_samples"], w["seed"], ix_offset=lo)
+        assert np.array_equal(shard, np.concatenate(parts_ref))
+
+
+def test_fused_update_and_negativity_flag():
+    """rbg_collision_update: f_out = f + dt*C (Eq. 27) and the count of negative cells."""
+    rbg = _rbg()
+    w = workloads.make(2, nx=2, np_side=8, n_samples=64)
+    orc = oracle.Oracle(w["problem"])
+    C_ref, mag = oracle_C_and_scale(orc, w["f"], w["n_samples"], w["seed"])
+    col = rbg.Collision(w["problem"])
+    f = torch.from_numpy(w["f"]).cuda()
+    for dt in (1e-3, 5e3):                      # the large step drives some cells negative
+        ref, neg_ref = oracle.update(w["f"], C_ref, dt)
+        out, flag = col.collision_update(f, dt, w["n_samples"], w["seed"])
+        torch.cuda.synchronize()
+        got = out.cpu().numpy()
+        assert np.all(np.abs(got - ref) <= dt * TOL64 * mag + 4 * np.finfo(float).eps * np.abs(ref))
+        margin = dt * TOL64 * mag + 4 * np.finfo(float).eps * np.abs(ref)
+        sure_neg = int(np.sum(ref < -margin)); maybe_neg = int(np.sum(ref < margin))
+        assert sure_neg <= int(flag.item()) <= maybe_neg
+        assert int(flag.item()) == int(np.sum(got < 0))
+        if dt > 1:
+            assert neg_ref > 0 and flag.item() > 0
+        else:
+            assert flag.item() == 0
+    # the flag accumulates (caller zeroes it)
+    out, flag2 = col.collision_update(f, 5e3, w["n_samples"], w["seed"], neg_flag=flag.clone())
+    torch.cuda.synchronize()
+    assert flag2.item() == 2 * flag.item()
+    with pytest.raises(rbg.RbgError):
+        col.collision_update(f, 1e-3, 8, 1, out=f)          # f_out must not alias f
+
+
+def test_host_entry_point_matches_device_entry_point():
+    w = workloads.make(1, nx=2, np_side=8, n_samples=64)
+    C_dev, col = gpu_C(w["problem"], w["f"], w["n_samples"], w["seed"])
+    C_host = col.collision_host(w["f"], w["n_samples"], w["seed"])
+    assert np.array_equal(C_dev, C_host)
+    pinned = torch.from_numpy(w["f"]).pin_memory()
+    assert np.array_equal(col.collision_host(pinned, w["n_samples"], w["seed"]).numpy(), C_dev)
+
+
+def test_edge_cases():
+    rbg = _rbg()
+    # single sample; fewer samples than lanes; one momentum cell; a species that takes part in no process
+    w = workloads.make(2, nx=1, np_side=4, n_samples=1)
+    for N in (1, 5, 31, 32, 33):
+        orc = oracle.Oracle(w["problem"])
+        C_ref, mag = oracle_C_and_scale(orc, w["f"], N, 77)
+        C, _ = gpu_C(w["problem"], w["f"], N, 77)
+        assert_parity(C, C_ref, mag, TOL64, f"N={N}")
+    prob = dict(w["problem"], processes=[w["problem"]["processes"][0]])      # only e-e: H+ has no role
+    orc = oracle.Oracle(prob)
+    C_ref, mag = oracle_C_and_scale(orc, w["f"], 16, 3)
+    C, col = gpu_C(prob, w["f"], 16, 3)
+    assert_parity(C, C_ref, mag, TOL64, "idle species")
+    assert np.all(C[orc.sp_off[1]:] == 0)
+    out, flag = col.collision_update(torch.from_numpy(w["f"]).cuda(), 1e-3, 16, 3)
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy()[orc.sp_off[1]:], w["f"][orc.sp_off[1]:])
+    # one-cell momentum grid and no processes at all
+    one = dict(nx=2, species=[dict(mass=1.0, charge=0, stat=0, g=1.0)],
+               grids=[dict(n=[1, 1, 1], pmin=[-1.0] * 3, pmax=[1.0] * 3)],
+               processes=[dict(a=0, b=0, c=0, d=0, kind=0, par=[1.0], sym=-1.0)], hbar=1.0)
+    f1 = np.array([0.5, 0.25])
+    orc = oracle.Oracle(one)
+    C_ref, mag = oracle_C_and_scale(orc, f1, 64, 1)
+    C, _ = gpu_C(one, f1, 64, 1)
+    assert_parity(C, C_ref, mag, TOL64, "1-cell grid")
+    none = dict(one, processes=[])
+    C, col = gpu_C(none, f1, 64, 1)
+    assert np.all(C == 0) and col.n_roles == 0
+    # massless species (T = q/(E+0), h > 0 guard)
+    w0 = workloads.make(3, nx=1, np_side=6, n_samples=40)
+    w0["problem"]["species"][3]["mass"] = 0.0
+    orc = oracle.Oracle(w0["problem"])
+    C_ref, mag = oracle_C_and_scale(orc, w0["f"], 40, 5)
+    C, _ = gpu_C(w0["problem"], w0["f"], 40, 5)
+    assert_parity(C, C_ref, mag, TOL64, "massless")
+
+
+def test_argument_errors():
+    rbg = _rbg()
+    w = workloads.make(1, np_side=4)
+    P = w["problem"]
+    bads = [dict(P, nx=0),
+            dict(P, species=[dict(mass=-1.0, charge=0, stat=0, g=1.0)]),
+            dict(P, species=[dict(mass=1.0, charge=0, stat=2, g=1.0)]),
+            dict(P, species=[dict(mass=1.0, charge=0, stat=0, g=0.0)]),
+            dict(P, grids=[dict(n=[4, 0, 4], pmin=[-1.0] * 3, pmax=[1.0] * 3)]),
+            dict(P, grids=[dict(n=[4, 4, 4], pmin=[1.0] * 3, pmax=[1.0] * 3)]),
+            dict(P, processes=[dict(a=0, b=1, c=0, d=1, kind=0, par=[1.0], sym=-1.0)]),
+            dict(P, processes=[dict(a=0, b=0, c=0, d=0, kind=9, par=[1.0], sym=-1.0)])]
+    for bad in bads:
+        with pytest.raises(rbg.RbgError):
+            rbg.Collision(bad)
+    with pytest.raises(rbg.RbgError, match="elastic"):
+        two = dict(P, species=P["species"] * 2, grids=P["grids"] * 2,
+                   processes=[dict(a=0, b=0, c=1, d=1, kind=0, par=[1.0], sym=-1.0)])
+        rbg.Collision(two)
+    col = rbg.Collision(P)
+    f = torch.from_numpy(w["f"]).cuda()
+    with pytest.raises(rbg.RbgError):
+        col.collision(f, 0, 1)
+    with pytest.raises(rbg.RbgError):
+        col.collision(f[:-1], 8, 1)
+    with pytest.raises(rbg.RbgError):
+        col.set_option("no_such_option", 1)
+    with pytest.raises(rbg.RbgError):
+        col.set_option("warps_per_cta", 99)
