@@ -112,7 +112,7 @@ uint64_t rbg_sample_evals(const rbg_handle* h, int n_samples);
 /* Kernels launched by the most recent rbg_collision* call on this handle. */
 int rbg_last_launch_count(const rbg_handle* h);
 /* Launch geometry / gather path knobs (results do not depend on them).  key: "warps_per_cta"
- * (1..32), "p1_per_cta" (momentum cells per CTA, >= 1), "gather" (0 auto, 1 shared memory,
+ * (1..16), "p1_per_cta" (momentum cells per CTA, >= 1), "gather" (0 auto, 1 shared memory,
  * 2 global/L2).  Returns RBG_E_INVALID_ARG for an unknown key or bad value. */
 int rbg_set_option(rbg_handle* h, const char* key, int value);
 /* Text of the last error on this handle (or of the last failed rbg_create if h is NULL). */
@@ -123,6 +123,12 @@ void rbg_destroy(rbg_handle* h);
  * the achieved rate.  what: 0 = fp64 FMA, 1 = fp32 FMA, 2 = int32 multiply-add.  *ops_per_s counts
  * one FMA as one operation.  Used by bench.py for the live roofline denominator. */
 int rbg_probe_alu_peak(int what, int iters, double* ops_per_s, void* cuda_stream);
+
+/* Diagnostic: compares the kernels' own fp64 divide / reciprocal / square-root sequences (the
+ * round-to-nearest fast paths without range checks) bit for bit with the CUDA
+ * library operators on n_operands random operand pairs (5 comparisons each); *mismatches must come
+ * back 0.  Synchronous, default stream. */
+int rbg_selftest_math(uint64_t n_operands, uint32_t seed, uint64_t* mismatches);
 
 #ifdef __cplusplus
 }

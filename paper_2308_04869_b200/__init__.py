@@ -9,5 +9,5 @@ from __future__ import annotations
 
 from .binding import (  # noqa: F401
     Collision, RbgError, KIND_CONST, KIND_COULOMB_SCREENED, KIND_TCHAN_S2, load_library, probe_alu_peak,
-    exported_symbols,
+    exported_symbols, selftest_math,
 )

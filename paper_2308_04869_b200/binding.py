@@ -51,6 +51,7 @@ _SIGNATURES = {
     "rbg_last_error": (C.c_char_p, [C.c_void_p]),
     "rbg_destroy": (None, [C.c_void_p]),
     "rbg_probe_alu_peak": (C.c_int, [C.c_int, C.c_int, C.POINTER(C.c_double), C.c_void_p]),
+    "rbg_selftest_math": (C.c_int, [C.c_uint64, C.c_uint32, C.POINTER(C.c_uint64)]),
 }
 
 
@@ -84,6 +85,13 @@ def probe_alu_peak(what: int, iters: int = 1 << 16, stream=None) -> float:
     out = C.c_double()
     _check(load_library().rbg_probe_alu_peak(what, iters, C.byref(out), _stream_ptr(stream)))
     return out.value
+
+
+def selftest_math(n_operands: int, seed: int = 1) -> int:
+    """rbg_selftest_math: number of bitwise mismatches (must be 0)."""
+    out = C.c_uint64()
+    _check(load_library().rbg_selftest_math(int(n_operands), int(seed), C.byref(out)))
+    return int(out.value)
 
 
 def _stream_ptr(stream):

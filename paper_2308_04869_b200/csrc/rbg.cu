@@ -174,6 +174,10 @@ int run_roles(rbg_handle* h, const double* f, double* out, bool update, double d
         lp.out_base = out + h->sp_off[r.s1];
         lp.nx_local = h->nx; lp.ix_offset = h->ix_offset; lp.n_samples = n_samples;
         lp.key0 = (uint32_t)seed; lp.key1 = (uint32_t)(seed >> 32);
+        for (int rr = 0; rr < 10; ++rr) {
+            lp.rk[2 * rr] = lp.key0 + (uint32_t)rr * 0x9E3779B9u;
+            lp.rk[2 * rr + 1] = lp.key1 + (uint32_t)rr * 0xBB67AE85u;
+        }
         lp.p1_per_cta = T; lp.tiles = (rp.np1 + T - 1) / T;
         lp.accumulate = first_role[r.s1] != (int)i;
         lp.update = update; lp.dt = dt; lp.neg_flag = neg_flag;
@@ -325,6 +329,23 @@ void rbg_destroy(rbg_handle* h) {
     if (!h) return;
     cudaFree(h->scratch_f); cudaFree(h->scratch_c);
     delete h;
+}
+
+int rbg_selftest_math(uint64_t n_operands, uint32_t seed, uint64_t* mismatches) {
+    if (!mismatches) return fail(nullptr, RBG_E_INVALID_ARG, "null argument");
+    unsigned long long* d = nullptr;
+    RBG_CUDA(nullptr, cudaMalloc(&d, 8));
+    RBG_CUDA(nullptr, cudaMemset(d, 0, 8));
+    const int ctas = 592, threads = 256;
+    const unsigned long long per = (n_operands + (uint64_t)ctas * threads - 1) / ((uint64_t)ctas * threads);
+    rbg::math_selftest_kernel<<<ctas, threads>>>(per, seed, d);
+    cudaError_t e = cudaDeviceSynchronize();
+    unsigned long long hbad = 0;
+    if (e == cudaSuccess) e = cudaMemcpy(&hbad, d, 8, cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    if (e != cudaSuccess) return fail(nullptr, RBG_E_CUDA, cudaGetErrorString(e));
+    *mismatches = hbad;
+    return RBG_OK;
 }
 
 int rbg_probe_alu_peak(int what, int iters, double* ops_per_s, void* cuda_stream) {
