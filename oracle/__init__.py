@@ -90,6 +90,7 @@ def lib():
         L.orc_update.restype = C.c_long
         L.orc_update.argtypes = [C.c_size_t, dp, dp, C.c_double, dp]
         L.orc_philox4x32_10.argtypes = [C.POINTER(C.c_uint32)] * 3
+        L.orc_direction.argtypes = [C.POINTER(C.c_uint32), C.c_int, dp]
         _lib = L
     return _lib
 
@@ -100,6 +101,14 @@ def philox4x32_10(key, ctr):
     o = (C.c_uint32 * 4)()
     lib().orc_philox4x32_10(k, c, o)
     return tuple(int(v) for v in o)
+
+
+def direction(words, use_float=False):
+    """O6 of the chain: the unit vector made from the four words of one Philox call."""
+    x = (C.c_uint32 * 4)(*[int(w) for w in words])
+    out = np.zeros(3)
+    lib().orc_direction(x, int(use_float), _dp(out))
+    return out
 
 
 def threads() -> int:

@@ -110,22 +110,79 @@ struct Trace {
     double p1[3], p2[3], p3[3], p4[3];
     double E1, E2, E3, s, t, pf, w, f1, f2, f3, f4, gain, loss;
     int j2, j3, j4;            // linear momentum cell, -1 = outside the box
-    int status;                // 0 ok, 1 skipped at O4 (h<=0), 2 below threshold, 3 no direction
-    int draws;                 // Philox calls consumed
+    int status;                // 0 ok, 1 skipped at O4 (h<=0), 2 below threshold
+    int draws;                 // Philox calls consumed (always 1)
 };
 
 template <typename R> inline R rfma(R a, R b, R c);
 template <> inline double rfma<double>(double a, double b, double c) { return std::fma(a, b, c); }
 template <> inline float  rfma<float>(float a, float b, float c) { return std::fmaf(a, b, c); }
 
-// u32 -> uniform real in [0,1): double keeps all 32 bits, float the top 24; both exact.
-template <typename R> inline R u01(uint32_t x);
-template <> inline double u01<double>(uint32_t x) { return (double)x * 0x1p-32; }
-template <> inline float  u01<float>(uint32_t x) { return (float)(x >> 8) * 0x1p-24f; }
-// u32 -> uniform real in [-1,1): exact in both types.
+// O2: top 24 bits of a word -> uniform real in [0,1), exact in both types.
+template <typename R> inline R u01(uint32_t x) { return (R)(x >> 8) * (R)0x1p-24; }
+// O6: a word -> uniform real in [-1,1): double keeps all 32 bits, float the top 24; both exact.
 template <typename R> inline R usym(uint32_t x);
 template <> inline double usym<double>(uint32_t x) { return (double)x * 0x1p-31 - 1.0; }
 template <> inline float  usym<float>(uint32_t x) { return (float)(x >> 8) * 0x1p-23f - 1.0f; }
+
+// O6: cos and sin of an angle a in (0, pi/4) as fixed polynomials in z = a*a, Horner with fma.
+// The coefficients are part of the chain (table "direction polynomials"):
+// near-minimax fits of (sin(a)/a - 1)/z and (cos(a) - 1)/z on [0, (pi/4)^2]; absolute error
+// <= 3e-16 (double, 6 terms each) and <= 1.5e-7 (float, 3 and 4 terms).
+template <typename R> struct OctantPoly;
+template <> struct OctantPoly<double> {
+    static void eval(double a, double& ca, double& sa) {
+        const double S1 = -0x1.5555555555555p-3, S2 = 0x1.1111111110bb2p-7, S3 = -0x1.a01a019e83aaep-13,
+                     S4 = 0x1.71de37968a100p-19, S5 = -0x1.ae600b02b6262p-26, S6 = 0x1.5e0b19f8b1451p-33;
+        const double C1 = -0x1.ffffffffffffap-2, C2 = 0x1.5555555554137p-5, C3 = -0x1.6c16c1691d8abp-10,
+                     C4 = 0x1.a019fc7b4b9f6p-16, C5 = -0x1.27e0f5789db4bp-22, C6 = 0x1.1c064801aa169p-29;
+        const double z = a * a;
+        double ps = std::fma(S6, z, S5); ps = std::fma(ps, z, S4); ps = std::fma(ps, z, S3);
+        ps = std::fma(ps, z, S2); ps = std::fma(ps, z, S1);
+        sa = std::fma(a * z, ps, a);
+        double pc = std::fma(C6, z, C5); pc = std::fma(pc, z, C4); pc = std::fma(pc, z, C3);
+        pc = std::fma(pc, z, C2); pc = std::fma(pc, z, C1);
+        ca = std::fma(z, pc, 1.0);
+    }
+};
+template <> struct OctantPoly<float> {
+    static void eval(float a, float& ca, float& sa) {
+        const float S1 = -0x1.555552p-3f, S2 = 0x1.110c28p-7f, S3 = -0x1.9ac9bp-13f;
+        const float C1 = -0x1p-1f, C2 = 0x1.55554cp-5f, C3 = -0x1.6c0e08p-10f, C4 = 0x1.9a6f2cp-16f;
+        const float z = a * a;
+        float ps = std::fmaf(S3, z, S2); ps = std::fmaf(ps, z, S1);
+        sa = std::fmaf(a * z, ps, a);
+        float pc = std::fmaf(C4, z, C3); pc = std::fmaf(pc, z, C2); pc = std::fmaf(pc, z, C1);
+        ca = std::fmaf(z, pc, 1.0f);
+    }
+};
+
+// O6: unit vector, uniform on the sphere, from one word for cos(theta) and 24 bits for phi.
+//   nz = usym(x3);  sin(theta) = sqrt(1 - nz^2);
+//   phi = (k + 1/2) 2 pi / 2^24, k = 24-bit integer: quadrant q = k >> 22, second-half flag b = bit 21,
+//   in-octant index r = k & (2^21 - 1), folded r' = b ? 2^21 - 1 - r : r, a = (r' + 1/2)(pi/4)/2^21,
+//   (cos, sin) of the angle inside the quadrant = b ? (sin a, cos a) : (cos a, sin a), then the
+//   exact rotation by q * pi/2.
+template <typename R> inline void direction(uint32_t x3, uint32_t k24, R nh[3]) {
+    const R nz = usym<R>(x3);
+    const R st = std::sqrt(rfma<R>(-nz, nz, (R)1));
+    const uint32_t q = k24 >> 22, b = (k24 >> 21) & 1u, r = k24 & 0x1FFFFFu;
+    const uint32_t rf = b ? 0x1FFFFFu - r : r;
+    const R A1 = (R)0x1.921fb54442d18p-22;       // (pi/4) / 2^21
+    const R A0 = (R)0x1.921fb54442d18p-23;       // half a step
+    const R a = rfma<R>((R)rf, A1, A0);
+    R ca, sa;
+    OctantPoly<R>::eval(a, ca, sa);
+    const R c1 = b ? sa : ca, s1 = b ? ca : sa;  // angle in (0, pi/2)
+    R cphi, sphi;
+    switch (q) {
+        case 0:  cphi = c1;  sphi = s1;  break;
+        case 1:  cphi = -s1; sphi = c1;  break;
+        case 2:  cphi = -c1; sphi = -s1; break;
+        default: cphi = s1;  sphi = -c1; break;
+    }
+    nh[0] = st * cphi; nh[1] = st * sphi; nh[2] = nz;
+}
 
 template <typename R> struct RoleConst {
     R m[4], msq[4];
@@ -229,16 +286,18 @@ struct Evaluator {
         for (int n = 0; n < N; ++n) {
             Trace tr; std::memset(&tr, 0, sizeof tr);
             const bool want = trace && n == trace_n;
-            const uint32_t cw = ((uint32_t)irole << 8);
-            // ---- O1/O2: partner momentum, uniform in the species-2 box --------------------
-            const U4 r0 = philox4x32_10(key0, key1, (uint32_t)n, (uint32_t)ip1, (uint32_t)ix, cw | 0u);
+            // ---- O1/O2: one Philox call per sample; partner momentum uniform in the species-2 box
+            // from the top 24 bits of words 0..2; its cell from the same bits by integer arithmetic.
+            const U4 r0 = philox4x32_10(key0, key1, (uint32_t)n, (uint32_t)ip1, (uint32_t)ix, (uint32_t)irole);
             R p2[3]; int j2d[3];
             for (int d = 0; d < 3; ++d) {
                 const R u = u01<R>(r0.v[d]);
                 p2[d] = rfma<R>(u, k.L[1][d], k.pmin[1][d]);
-                j2d[d] = (int)(((uint64_t)r0.v[d] * (uint64_t)k.n[1][d]) >> 32);   // = floor(x n / 2^32)
+                j2d[d] = (int)(((uint64_t)(r0.v[d] >> 8) * (uint64_t)k.n[1][d]) >> 24);   // = floor(u n)
             }
             const int j2 = (j2d[0] * k.n[1][1] + j2d[1]) * k.n[1][2] + j2d[2];
+            // the low bytes of words 0..2 make the 24-bit azimuth index, word 3 gives cos(theta)
+            const uint32_t k24 = ((r0.v[0] & 255u) << 16) | ((r0.v[1] & 255u) << 8) | (r0.v[2] & 255u);
             int status = 0, draws = 1;
             R E2 = 0, s = 0, t = 0, pf = 0, w = 0, E3 = 0, f2 = 0, f3 = 0, f4 = 0, gain = 0, loss = 0;
             R p3[3] = {0, 0, 0}, p4[3] = {0, 0, 0};
@@ -269,29 +328,16 @@ struct Evaluator {
                 const R b34 = s - k.Mdf;                        // s - (m3-m4)^2
                 pf = std::sqrt(a34 * b34) * hirs;               // |p*_34|
                 const R E3s = (s + k.dm34) * hirs;              // (s + m3^2 - m4^2) / (2 sqrt s)
-                // ---- O6: direction, Marsaglia (1972) disk rejection, trig-free -------------
-                R nh[3]; bool have = false;
-                for (uint32_t kd = 1; kd <= 15u && !have; ++kd) {
-                    const U4 rd = philox4x32_10(key0, key1, (uint32_t)n, (uint32_t)ip1, (uint32_t)ix, cw | kd);
-                    ++draws;
-                    for (int att = 0; att < 2 && !have; ++att) {
-                        const R a = usym<R>(rd.v[2 * att]), b = usym<R>(rd.v[2 * att + 1]);
-                        const R S = rfma<R>(a, a, b * b);
-                        if (S < (R)1) {
-                            const R r2 = (R)2 * std::sqrt((R)1 - S);
-                            nh[0] = a * r2; nh[1] = b * r2; nh[2] = rfma<R>((R)-2, S, (R)1);
-                            have = true;
-                        }
-                    }
-                }
-                if (!have) { status = 3; break; }
+                // ---- O6: direction uniform on the sphere, rejection-free and libm-free -------------
+                R nh[3];
+                direction<R>(r0.v[3], k24, nh);
                 // ---- O7: boost the CM momentum of particle 3 to the lab ---------------------
                 R p3s[3], P[3];
                 for (int d = 0; d < 3; ++d) { p3s[d] = pf * nh[d]; P[d] = p1[d] + p2[d]; }
                 const R Et = E1 + E2;
                 const R dPn = dot3<R>(P, p3s);
                 E3 = rfma<R>(Et, E3s, dPn) * irs;               // gamma (E3* + beta.p3*)
-                const R c = (E3 + E3s) / (Et + rs);             // p3 = p3* + P (E3+E3*)/(Et+sqrt s)
+                const R c = (E3 + E3s) * ((R)1 / (Et + rs));    // p3 = p3* + P (E3+E3*)/(Et+sqrt s)
                 for (int d = 0; d < 3; ++d) { p3[d] = rfma<R>(P[d], c, p3s[d]); p4[d] = P[d] - p3[d]; }
                 // ---- O8/O9/O12: t = (p1-p3)^2 and the weight as one quotient ---------------
                 const R ers = E2 * rs;
@@ -393,6 +439,13 @@ extern "C" {
 void orc_philox4x32_10(const uint32_t key[2], const uint32_t ctr[4], uint32_t out[4]) {
     const U4 r = philox4x32_10(key[0], key[1], ctr[0], ctr[1], ctr[2], ctr[3]);
     for (int i = 0; i < 4; ++i) out[i] = r.v[i];
+}
+
+// O6 alone (pin: tests compare it with numpy's cos/sin): words x[0..3] of one Philox call -> n.
+void orc_direction(const uint32_t x[4], int use_float, double out[3]) {
+    const uint32_t k24 = ((x[0] & 255u) << 16) | ((x[1] & 255u) << 8) | (x[2] & 255u);
+    if (use_float) { float nh[3]; direction<float>(x[3], k24, nh); for (int d = 0; d < 3; ++d) out[d] = nh[d]; }
+    else { double nh[3]; direction<double>(x[3], k24, nh); for (int d = 0; d < 3; ++d) out[d] = nh[d]; }
 }
 
 void* orc_create(int nx, int n_species, const Species* sp, const Grid* grid, int n_process, const Process* pr,

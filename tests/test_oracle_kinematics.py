@@ -1,7 +1,11 @@
 """P2: per-sample kinematic invariants of the oracle's chain (O2-O9), the sampling distributions
 (p2 uniform in the box, CM direction uniform on the sphere) and the nearest-cell gather (O10)."""
 import math
+from fractions import Fraction
 
+import mpmath
+
+mpmath.mp.dps = 40
 import numpy as np
 import pytest
 
@@ -130,3 +134,31 @@ def test_threshold_and_degenerate_samples_contribute_zero():
     assert st.count(0) == 200
     # ... and the estimate stays finite
     assert np.all(np.isfinite(o.collision(f, 64, 1)))
+
+
+def test_direction_against_library_trigonometry():
+    """O6: the polynomial, libm-free direction equals
+    (sin(theta) cos(phi), sin(theta) sin(phi), cos(theta)) with mpmath's cos/sin (40 digits), for
+    cos(theta) = x3 2^-31 - 1 and phi = (k + 1/2) 2 pi / 2^24, k from the low bytes of x0..x2:
+    to 4e-16 in double and 3e-7 in float; exactly unit length to rounding; every octant, both ends
+    of every octant and the symmetric partner (k -> 2^24 - 1 - k mirrors phi -> -phi exactly)."""
+    rng = np.random.default_rng(7)
+    ks = [0, 1, 2 ** 21 - 1, 2 ** 21, 2 ** 22 - 1, 2 ** 22, 3 * 2 ** 21, 2 ** 23 - 1, 2 ** 23, 2 ** 24 - 1]
+    ks += [int(v) for v in rng.integers(0, 2 ** 24, 400)]
+    for k in ks:
+        for x3 in [0, 1, 2 ** 31, 2 ** 32 - 1] + [int(v) for v in rng.integers(0, 2 ** 32, 3)]:
+            hi = [int(v) << 8 for v in rng.integers(0, 2 ** 24, 3)]          # p2 bits: must not matter
+            words = [hi[0] | (k >> 16), hi[1] | ((k >> 8) & 255), hi[2] | (k & 255), x3]
+            phi = (mpmath.mpf(k) + 0.5) * 2 * mpmath.pi / 2 ** 24        # 40 digits: no rounding of the angle
+            cphi, sphi = float(mpmath.cos(phi)), float(mpmath.sin(phi))
+            for use_float, tol in ((False, 4e-16), (True, 3e-7)):
+                ct = (x3 >> 8) * 2.0 ** -23 - 1.0 if use_float else x3 * 2.0 ** -31 - 1.0
+                st = math.sqrt(float(1 - Fraction(ct) ** 2))              # 1 - ct^2 exactly, one rounding
+                want = np.array([st * cphi, st * sphi, ct])
+                got = oracle.direction(words, use_float)
+                assert np.all(np.abs(got - want) <= tol), (k, x3, use_float, got, want)
+                assert abs(got @ got - 1.0) <= 4 * tol
+                mirror = 2 ** 24 - 1 - k
+                wm = [hi[0] | (mirror >> 16), hi[1] | ((mirror >> 8) & 255), hi[2] | (mirror & 255), x3]
+                gm = oracle.direction(wm, use_float)
+                assert gm[0] == got[0] and gm[1] == -got[1] and gm[2] == got[2]
