@@ -81,7 +81,7 @@ typedef struct { int a, b, c, d; int kind; double par[4]; double sym; } rbg_proc
 /* Create a handle.  Returns RBG_OK and stores the handle in *out, or a negative code (then *out
  * is NULL and rbg_last_error(NULL) has the text).  Rejects: non-positive grid counts,
  * pmax <= pmin, negative mass, stat not in {0,+1,-1}, g <= 0, species index out of range,
- * unknown kind or flags, inelastic processes, more than 255 roles, no CUDA device. */
+ * unknown kind or flags, inelastic processes, no CUDA device. */
 int rbg_create(rbg_handle** out, const rbg_spatial_grid* grid, int n_species, const rbg_species* species,
                const rbg_momentum_grid* momentum_grids /* [n_species] */, int n_process,
                const rbg_process* processes, double hbar, int flags);
@@ -111,9 +111,10 @@ int rbg_n_roles(const rbg_handle* h);
 uint64_t rbg_sample_evals(const rbg_handle* h, int n_samples);
 /* Kernels launched by the most recent rbg_collision* call on this handle. */
 int rbg_last_launch_count(const rbg_handle* h);
-/* Launch geometry / gather path knobs (results do not depend on them).  key: "warps_per_cta"
- * (1..16), "p1_per_cta" (momentum cells per CTA, >= 1), "gather" (0 auto, 1 shared memory,
- * 2 global/L2).  Returns RBG_E_INVALID_ARG for an unknown key or bad value. */
+/* Launch geometry / gather path knobs (results do not depend on them; 0 = automatic).  key:
+ * "warps_per_cta" (1..32), "p1_per_cta" (momentum cells per CTA, >= 1), "samples_per_lane"
+ * (1 or 2: samples a lane evaluates per loop iteration; CTAs of more than 16 warps use 1),
+ * "gather" (1 shared memory, 2 global/L2).  Returns RBG_E_INVALID_ARG for an unknown key or value. */
 int rbg_set_option(rbg_handle* h, const char* key, int value);
 /* Text of the last error on this handle (or of the last failed rbg_create if h is NULL). */
 const char* rbg_last_error(const rbg_handle* h);

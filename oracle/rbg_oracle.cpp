@@ -158,13 +158,14 @@ template <> struct OctantPoly<float> {
 };
 
 // O6: unit vector, uniform on the sphere, from one word for cos(theta) and 24 bits for phi.
-//   nz = usym(x3);  sin(theta) = sqrt(1 - nz^2);
+//   nz = usym(x3 | odd), odd = lowest bit that usym keeps (so |nz| < 1 and the lattice is symmetric);
+//   sin(theta) = sqrt(1 - nz^2);
 //   phi = (k + 1/2) 2 pi / 2^24, k = 24-bit integer: quadrant q = k >> 22, second-half flag b = bit 21,
 //   in-octant index r = k & (2^21 - 1), folded r' = b ? 2^21 - 1 - r : r, a = (r' + 1/2)(pi/4)/2^21,
 //   (cos, sin) of the angle inside the quadrant = b ? (sin a, cos a) : (cos a, sin a), then the
 //   exact rotation by q * pi/2.
 template <typename R> inline void direction(uint32_t x3, uint32_t k24, R nh[3]) {
-    const R nz = usym<R>(x3);
+    const R nz = usym<R>(x3 | (sizeof(R) == 8 ? 1u : 0x100u));   // odd lattice: symmetric, never +-1
     const R st = std::sqrt(rfma<R>(-nz, nz, (R)1));
     const uint32_t q = k24 >> 22, b = (k24 >> 21) & 1u, r = k24 & 0x1FFFFFu;
     const uint32_t rf = b ? 0x1FFFFFu - r : r;

@@ -41,7 +41,7 @@ struct rbg_handle {
     int sm_count = 148;
     int max_smem_optin = 0;
     // options
-    int opt_warps = 0, opt_p1_per_cta = 0, opt_gather = 0;
+    int opt_warps = 0, opt_p1_per_cta = 0, opt_gather = 0, opt_spl = 0;
     int last_launches = 0;
     // scratch for the host entry point
     double *scratch_f = nullptr, *scratch_c = nullptr;
@@ -112,23 +112,33 @@ rbg::RoleParams<R> make_role_params(const rbg_handle& H, const Role& r) {
     return k;
 }
 
-template <typename R, int KIND, bool Q, bool SMEM>
+template <typename R, int KIND, bool Q, bool SMEM, int MAXT, int SPL>
 cudaError_t launch_one(const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp, int grid, int threads, size_t smem,
                        cudaStream_t st) {
-    auto kern = rbg::collision_role_kernel<R, KIND, Q, SMEM>;
+    auto kern = rbg::collision_role_kernel<R, KIND, Q, SMEM, MAXT, SPL>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kern<<<grid, threads, smem, st>>>(rp, lp);
     return cudaGetLastError();
 }
 
+// geometry variant: CTAs of up to 512 threads evaluate SPL = 1 or 2 samples per lane and iteration
+// (up to 128 registers per thread); CTAs of up to 1024 threads evaluate 1 (64 registers).
+template <typename R, int KIND, bool Q, bool SMEM>
+cudaError_t launch_geo(int spl, const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp, int grid, int threads,
+                       size_t smem, cudaStream_t st) {
+    if (threads > 512) return launch_one<R, KIND, Q, SMEM, 1024, 1>(rp, lp, grid, threads, smem, st);
+    if (spl == 2) return launch_one<R, KIND, Q, SMEM, 512, 2>(rp, lp, grid, threads, smem, st);
+    return launch_one<R, KIND, Q, SMEM, 512, 1>(rp, lp, grid, threads, smem, st);
+}
+
 template <typename R, int KIND>
-cudaError_t launch_kq(bool q, bool smem_path, const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp, int grid,
+cudaError_t launch_kq(bool q, bool smem_path, int spl, const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp, int grid,
                       int threads, size_t smem, cudaStream_t st) {
-    if (q) return smem_path ? launch_one<R, KIND, true, true>(rp, lp, grid, threads, smem, st)
-                            : launch_one<R, KIND, true, false>(rp, lp, grid, threads, smem, st);
-    return smem_path ? launch_one<R, KIND, false, true>(rp, lp, grid, threads, smem, st)
-                     : launch_one<R, KIND, false, false>(rp, lp, grid, threads, smem, st);
+    if (q) return smem_path ? launch_geo<R, KIND, true, true>(spl, rp, lp, grid, threads, smem, st)
+                            : launch_geo<R, KIND, true, false>(spl, rp, lp, grid, threads, smem, st);
+    return smem_path ? launch_geo<R, KIND, false, true>(spl, rp, lp, grid, threads, smem, st)
+                     : launch_geo<R, KIND, false, false>(spl, rp, lp, grid, threads, smem, st);
 }
 
 template <typename R>
@@ -156,6 +166,7 @@ int run_roles(rbg_handle* h, const double* f, double* out, bool update, double d
         const Role& r = h->roles[i];
         const rbg::RoleParams<R> rp = make_role_params<R>(*h, r);
         const int warps = h->opt_warps > 0 ? h->opt_warps : 16;
+        const int spl = h->opt_spl > 0 ? h->opt_spl : 2;
         long work = (long)h->nx * rp.np1;
         int T = h->opt_p1_per_cta > 0 ? h->opt_p1_per_cta : (int)std::min<long>(512, std::max<long>(warps, work / ((long)h->sm_count * 8)));
         T = std::min(T, rp.np1);
@@ -187,9 +198,9 @@ int run_roles(rbg_handle* h, const double* f, double* out, bool update, double d
         const bool q = h->species[r.s1].stat != 0 || h->species[r.s2].stat != 0;
         cudaError_t e;
         switch (r.kind) {
-            case RBG_M2_CONST: e = launch_kq<R, rbg::KIND_CONST>(q, smem_path, rp, lp, (int)grid, warps * 32, smem, st); break;
-            case RBG_M2_COULOMB_SCREENED: e = launch_kq<R, rbg::KIND_COULOMB>(q, smem_path, rp, lp, (int)grid, warps * 32, smem, st); break;
-            default: e = launch_kq<R, rbg::KIND_TCHAN_S2>(q, smem_path, rp, lp, (int)grid, warps * 32, smem, st); break;
+            case RBG_M2_CONST: e = launch_kq<R, rbg::KIND_CONST>(q, smem_path, spl, rp, lp, (int)grid, warps * 32, smem, st); break;
+            case RBG_M2_COULOMB_SCREENED: e = launch_kq<R, rbg::KIND_COULOMB>(q, smem_path, spl, rp, lp, (int)grid, warps * 32, smem, st); break;
+            default: e = launch_kq<R, rbg::KIND_TCHAN_S2>(q, smem_path, spl, rp, lp, (int)grid, warps * 32, smem, st); break;
         }
         if (e != cudaSuccess) return fail(h, RBG_E_CUDA, std::string("kernel launch: ") + cudaGetErrorString(e));
         ++h->last_launches;
@@ -267,7 +278,6 @@ int rbg_create(rbg_handle** out, const rbg_spatial_grid* grid, int n_species, co
         h->roles.push_back(r);
         if (p.b != p.a) { r.s1 = p.b; r.s2 = p.a; r.index = (int)h->roles.size(); h->roles.push_back(r); }
     }
-    if (h->roles.size() > 255) { delete h; return fail(nullptr, RBG_E_UNSUPPORTED, "more than 255 roles"); }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { delete h; return fail(nullptr, RBG_E_CUDA, "no CUDA device (there is no CPU fallback)"); }
     cudaGetDevice(&h->device);
@@ -316,7 +326,8 @@ int rbg_last_launch_count(const rbg_handle* h) { return h ? h->last_launches : 0
 int rbg_set_option(rbg_handle* h, const char* key, int value) {
     if (!h || !key) return fail(h, RBG_E_INVALID_ARG, "null argument");
     const std::string k(key);
-    if (k == "warps_per_cta") { if (value < 0 || value > 16) return fail(h, RBG_E_INVALID_ARG, "warps_per_cta must be 0 (auto) or 1..16"); h->opt_warps = value; }
+    if (k == "warps_per_cta") { if (value < 0 || value > 32) return fail(h, RBG_E_INVALID_ARG, "warps_per_cta must be 0 (auto) or 1..32"); h->opt_warps = value; }
+    else if (k == "samples_per_lane") { if (value < 0 || value > 2) return fail(h, RBG_E_INVALID_ARG, "samples_per_lane must be 0 (auto), 1 or 2"); h->opt_spl = value; }
     else if (k == "p1_per_cta") { if (value < 0) return fail(h, RBG_E_INVALID_ARG, "p1_per_cta must be >= 0 (0 = auto)"); h->opt_p1_per_cta = value; }
     else if (k == "gather") { if (value < 0 || value > 2) return fail(h, RBG_E_INVALID_ARG, "gather must be 0, 1 or 2"); h->opt_gather = value; }
     else return fail(h, RBG_E_INVALID_ARG, "unknown option " + k);

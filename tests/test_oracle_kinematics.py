@@ -139,7 +139,7 @@ def test_threshold_and_degenerate_samples_contribute_zero():
 def test_direction_against_library_trigonometry():
     """O6: the polynomial, libm-free direction equals
     (sin(theta) cos(phi), sin(theta) sin(phi), cos(theta)) with mpmath's cos/sin (40 digits), for
-    cos(theta) = x3 2^-31 - 1 and phi = (k + 1/2) 2 pi / 2^24, k from the low bytes of x0..x2:
+    cos(theta) = (x3|1) 2^-31 - 1 (odd lattice: never 0 or +-1) and phi = (k + 1/2) 2 pi / 2^24, k from the low bytes of x0..x2:
     to 4e-16 in double and 3e-7 in float; exactly unit length to rounding; every octant, both ends
     of every octant and the symmetric partner (k -> 2^24 - 1 - k mirrors phi -> -phi exactly)."""
     rng = np.random.default_rng(7)
@@ -152,7 +152,8 @@ def test_direction_against_library_trigonometry():
             phi = (mpmath.mpf(k) + 0.5) * 2 * mpmath.pi / 2 ** 24        # 40 digits: no rounding of the angle
             cphi, sphi = float(mpmath.cos(phi)), float(mpmath.sin(phi))
             for use_float, tol in ((False, 4e-16), (True, 3e-7)):
-                ct = (x3 >> 8) * 2.0 ** -23 - 1.0 if use_float else x3 * 2.0 ** -31 - 1.0
+                ct = ((x3 >> 8) | 1) * 2.0 ** -23 - 1.0 if use_float else (x3 | 1) * 2.0 ** -31 - 1.0
+                assert 0.0 < abs(ct) < 1.0
                 st = math.sqrt(float(1 - Fraction(ct) ** 2))              # 1 - ct^2 exactly, one rounding
                 want = np.array([st * cphi, st * sphi, ct])
                 got = oracle.direction(words, use_float)
