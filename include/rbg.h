@@ -125,10 +125,10 @@ void rbg_destroy(rbg_handle* h);
  * one FMA as one operation.  Used by bench.py for the live roofline denominator. */
 int rbg_probe_alu_peak(int what, int iters, double* ops_per_s, void* cuda_stream);
 
-/* Diagnostic: compares the kernels' own fp64 divide / reciprocal / square-root sequences (the
- * round-to-nearest fast paths without range checks) bit for bit with the CUDA
- * library operators on n_operands random operand pairs (5 comparisons each); *mismatches must come
- * back 0.  Synchronous, default stream. */
+/* Diagnostic: compares the kernels' own fp64 and fp32 divide / reciprocal / square-root sequences
+ * (the round-to-nearest fast paths without range checks) bit for bit with the
+ * CUDA library operators on n_operands random operand sets (10 comparisons each); *mismatches must
+ * come back 0.  Synchronous, default stream. */
 int rbg_selftest_math(uint64_t n_operands, uint32_t seed, uint64_t* mismatches);
 
 #ifdef __cplusplus

@@ -198,7 +198,7 @@ template <typename R> inline R dot3(const R* a, const R* b) {
     return rfma<R>(a[2], b[2], rfma<R>(a[1], b[1], a[0] * b[0]));
 }
 
-struct Accum { double G = 0, Ls = 0, Lin = 0, Q = 0; };
+struct Accum { double G = 0, Ls = 0, Lin = 0, Q = 0, D = 0; };   // D: float chain's sum of (float)(w gain - w loss)
 
 template <typename R>
 struct Evaluator {
@@ -367,6 +367,9 @@ struct Evaluator {
                 // ---- O12: accumulate in double ---------------------------------------------
                 const double wg = (double)(w * gain), wl = (double)(w * loss);
                 acc.G += wg; acc.Ls += wl;
+                // float chain only: the contribution to C is the difference rounded once to float,
+                // accumulated in double (O12); the double chain uses G - Ls
+                if (std::is_same<R, float>::value) acc.D += (double)(w * gain - w * loss);
                 if (j3 >= 0 && j4 >= 0) acc.Lin += wl;
                 acc.Q += (wg - wl) * (wg - wl);
             } while (false);
@@ -419,7 +422,7 @@ int run_collision(const Handle& H, const double* f, double* C, int N, uint64_t s
             Accum acc;
             ev.eval_p1(f, ix, ip1, N, seed, acc, nullptr, -1);
             const double pref = ev.prefactor(ip1, N);
-            C[H.sp_off[s1] + (size_t)ix * np1 + ip1] += pref * (acc.G - acc.Ls);
+            C[H.sp_off[s1] + (size_t)ix * np1 + ip1] += pref * (std::is_same<R, float>::value ? acc.D : acc.G - acc.Ls);
             const size_t o = H.role_off[ir] + (size_t)ix * np1 + ip1;
             if (dG) dG[o] = pref * acc.G;
             if (dL) dL[o] = pref * acc.Ls;
