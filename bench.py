@@ -34,6 +34,9 @@ METRIC, UNIT = "collision_samples_per_s", "samples/s"
 FLOPS_PER_SAMPLE = {0: 141.0, 1: 155.0, 2: 157.0}
 QUANTUM_EXTRA_FLOPS = 10.0
 FP64_LANES_PER_SM = 64          # FMA/clk/SM; confirmed by the live probe
+# dram__bytes_read.sum + dram__bytes_write.sum of one role launch from the committed `ncu --set full`
+# capture (profiles/r1b_chain_v2_cfg2.md: 32.84 MB + 1.64 MB, config 2 at full size); null elsewhere.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {2: 34.48e6}
 
 
 def flops_per_sweep(problem, n_samples):
@@ -141,7 +144,7 @@ def main():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5); 2 = configs[1]")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-cells", type=int, default=6, help="spatial cells per step of the reference arm")
-    ap.add_argument("--cpu-cells", type=int, default=24, help="spatial cells of the cpu_baseline leg")
+    ap.add_argument("--cpu-cells", type=int, default=48, help="spatial cells of the cpu_baseline leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--nx", type=int, default=None, help="override the number of spatial cells (profiling runs; "
                     "the JSON line then names the reduced workload)")
@@ -241,7 +244,8 @@ def main():
     if w["fp32"]:
         peak_nominal *= 2                       # 128 fp32 lanes per SM
     roof = {"bound": "alu", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s", "frac": achieved / peak_nominal,
-            "traffic": None, "peak_source": f"{sms} SM x {FP64_LANES_PER_SM * (2 if w['fp32'] else 1)} FMA/clk x 2 x "
+            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.config) if args.nx is None else None,
+            "traffic_unit": "bytes per launch (ncu capture, profiles/r1b_chain_v2_cfg2.md)", "peak_source": f"{sms} SM x {FP64_LANES_PER_SM * (2 if w['fp32'] else 1)} FMA/clk x 2 x "
                                             f"{max_mhz:.0f} MHz (DESIGN.md section 8)",
             "peak_probe_tflops": probe, "frac_of_probe": achieved / probe,
             "kernel": "rbg::collision_role_kernel", "launch_ms": t_launch * 1e3,
