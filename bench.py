@@ -31,7 +31,7 @@ METRIC, UNIT = "collision_samples_per_s", "samples/s"
 
 # Algorithmic FP64 work per sample of chain O1-O12 (FMA = 2 flops, every other
 # add/mul/compare/sqrt/divide = 1), by |M|^2 kind, classical statistics (+12 with quantum factors).
-FLOPS_PER_SAMPLE = {0: 141.0, 1: 155.0, 2: 157.0}
+FLOPS_PER_SAMPLE = {0: 141.0, 1: 155.0, 2: 157.0, 3: 142.0}
 QUANTUM_EXTRA_FLOPS = 10.0
 FP64_LANES_PER_SM = 64          # FMA/clk/SM; confirmed by the live probe
 # dram__bytes_read.sum + dram__bytes_write.sum of one role launch from the committed `ncu --set full`

@@ -69,8 +69,13 @@ typedef struct { double mass; double charge; int stat; double g; } rbg_species;
 typedef enum {
     RBG_M2_CONST            = 0,  /* |M|^2 = par[0]                                   */
     RBG_M2_COULOMB_SCREENED = 1,  /* |M|^2 = par[0] / (t - par[1]^2)^2                */
-    RBG_M2_TCHAN_S2         = 2   /* |M|^2 = par[0]^4 s^2 / (t - par[1]^2)^2   (Table III t-channel
+    RBG_M2_TCHAN_S2         = 2,  /* |M|^2 = par[0]^4 s^2 / (t - par[1]^2)^2   (Table III t-channel
                                      form with regulator)          */
+    RBG_M2_ISO_DSIGMA       = 3   /* |M|^2 = 64 pi^2 s par[0]: a constant differential cross section
+                                     dsigma/dOmega = par[0], isotropic in the CM frame -- how the paper's
+                                     collision test quotes its processes (Eq. 48, PAPER.md:493-500;
+                                     cross section <-> matrix element Eq. 20-22, PAPER.md:214-230;
+                                     DESIGN.md reading R17)                           */
 } rbg_m2_kind;
 
 /* Process a + b -> c + d (species indices).  Only elastic processes (c == a, d == b) are
@@ -97,6 +102,14 @@ int rbg_collision(rbg_handle* h, const double* f_dev, double* C_dev, int n_sampl
  * is stored unclamped (policy is the caller's).  f_out_dev must not alias f_dev. */
 int rbg_collision_update(rbg_handle* h, const double* f_dev, double* f_out_dev, double dt, int* neg_flag_dev,
                          int n_samples, uint64_t seed, void* cuda_stream);
+
+/* n_steps explicit Euler steps of Eq. 27 in a row (the paper's collision test runs 25 000 of them,
+ * PAPER.md:504): f <- f + dt * C[f], step k (k = 0 .. n_steps-1) drawing its samples with seed + k, i.e.
+ * exactly n_steps calls of rbg_collision_update ping-ponging between f_dev and scratch_dev (rbg_f_elems()
+ * doubles, caller-owned, must not overlap f_dev).  On return (stream order) f_dev holds the final state;
+ * scratch_dev is clobbered.  *neg_flag_dev accumulates the negative cells of every step.  n_steps >= 0. */
+int rbg_collision_evolve(rbg_handle* h, double* f_dev, double* scratch_dev, double dt, int n_steps,
+                         int* neg_flag_dev, int n_samples, uint64_t seed, void* cuda_stream);
 
 /* Same as rbg_collision with HOST buffers: copies f_host to the device (handle-owned scratch),
  * runs the kernels, copies C back, synchronises.  Pinned host memory makes the copies faster but

@@ -73,7 +73,11 @@ struct Species { double mass, charge; int stat; double g; };
 struct Grid    { int n[3]; double pmin[3], pmax[3]; };
 struct Process { int a, b, c, d; int kind; double par[4]; double sym; };
 
-enum Kind { M2_CONST = 0, M2_COULOMB_SCREENED = 1, M2_TCHAN_S2 = 2 };
+enum Kind { M2_CONST = 0, M2_COULOMB_SCREENED = 1, M2_TCHAN_S2 = 2,
+            // |M|^2 = 64 pi^2 s par0: a constant differential cross section dsigma/dOmega = par0, isotropic in
+            // the CM frame (the paper's collision test quotes its processes this way, Eq. 48 PAPER.md:493-500;
+            // relation cross section <-> matrix element: Eq. 20-22, reading R17)
+            M2_ISO_DSIGMA = 3 };
 
 // A role = one process seen from one grid species: particle 1 is the grid
 // particle, 2 its sampled partner, (3,4) the other pair.
@@ -191,7 +195,7 @@ template <typename R> struct RoleConst {
     R pmin[4][3], L[4][3], invD[4][3], off[4][3];   // per particle slot (its species' grid)
     int n[4][3];
     R theta_kappa[4];
-    R par0, mD2, g4;
+    R par0, mD2, g4, sig64;
 };
 
 template <typename R> inline R dot3(const R* a, const R* b) {
@@ -237,6 +241,7 @@ struct Evaluator {
         k.mD2  = (R)(role.par[1] * role.par[1]);
         const double g2 = role.par[0] * role.par[0];
         k.g4   = (R)(g2 * g2);
+        k.sig64 = (R)(64.0 * M_PI * M_PI * role.par[0]);     // M2_ISO_DSIGMA: |M|^2 = sig64 * s
     }
 
     // O10.  Nearest-cell gather: tau_d = fma(p_d, invDelta_d, -pmin_d*invDelta_d); inside iff
@@ -344,6 +349,8 @@ struct Evaluator {
                 const R ers = E2 * rs;
                 if (role.kind == M2_CONST) {
                     w = (k.par0 * pf) / ers;
+                } else if (role.kind == M2_ISO_DSIGMA) {
+                    w = ((k.sig64 * s) * pf) / ers;
                 } else {
                     R dl[3];
                     for (int d = 0; d < 3; ++d) dl[d] = p1[d] - p3[d];
@@ -475,6 +482,7 @@ void* orc_create(int nx, int n_species, const Species* sp, const Grid* grid, int
     for (int i = 0; i < n_process; ++i) {
         const Process& p = pr[i];
         if (p.c != p.a || p.d != p.b) { delete H; return nullptr; }   // elastic roles only (R15)
+        if (p.kind < M2_CONST || p.kind > M2_ISO_DSIGMA) { delete H; return nullptr; }
         const double sym = p.sym < 0 ? (p.a == p.b ? 0.5 : 1.0) : p.sym;
         Role r; r.kind = p.kind; std::memcpy(r.par, p.par, sizeof r.par); r.sym = sym; r.process = i;
         r.s[0] = p.a; r.s[1] = p.b; r.s[2] = p.c; r.s[3] = p.d;

@@ -6,7 +6,7 @@ from pathlib import Path
 
 import numpy as np
 
-KIND_CONST, KIND_COULOMB_SCREENED, KIND_TCHAN_S2 = 0, 1, 2
+KIND_CONST, KIND_COULOMB_SCREENED, KIND_TCHAN_S2, KIND_ISO_DSIGMA = 0, 1, 2, 3
 RBG_FP64, RBG_FP32_KINEMATICS = 0, 1
 
 _PKG = Path(__file__).resolve().parent
@@ -41,6 +41,8 @@ _SIGNATURES = {
                              C.POINTER(_MomentumGrid), C.c_int, C.POINTER(_Process), C.c_double, C.c_int]),
     "rbg_collision": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_uint64, C.c_void_p]),
     "rbg_collision_update": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_int,
+                                       C.c_uint64, C.c_void_p]),
+    "rbg_collision_evolve": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int, C.c_void_p, C.c_int,
                                        C.c_uint64, C.c_void_p]),
     "rbg_collision_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_uint64]),
     "rbg_f_elems": (C.c_size_t, [C.c_void_p]),
@@ -171,6 +173,19 @@ class Collision:
                                                    C.c_void_p(neg_flag.data_ptr()), int(n_samples), int(seed),
                                                    _stream_ptr(stream)), self._h)
         return out, neg_flag
+
+    def collision_evolve(self, f, dt: float, n_steps: int, n_samples: int, seed: int, scratch=None, neg_flag=None,
+                         stream=None):
+        """rbg_collision_evolve: n_steps Euler steps f <- f + dt*C[f] in place (step k uses seed + k)."""
+        import torch
+        if scratch is None:
+            scratch = torch.empty_like(f)
+        if neg_flag is None:
+            neg_flag = torch.zeros(1, dtype=torch.int32, device=f.device)
+        _check(load_library().rbg_collision_evolve(self._h, self._dev(f, "f"), self._dev(scratch, "scratch"), float(dt),
+                                                   int(n_steps), C.c_void_p(neg_flag.data_ptr()), int(n_samples),
+                                                   int(seed), _stream_ptr(stream)), self._h)
+        return f, neg_flag
 
     def collision_host(self, f_host, n_samples: int, seed: int, out=None):
         """rbg_collision_host: host buffers in, host buffers out (numpy float64 or pinned CPU tensors)."""

@@ -8,6 +8,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <utility>
 #include <string>
 #include <vector>
 
@@ -101,7 +102,7 @@ rbg::RoleParams<R> make_role_params(const rbg_handle& H, const Role& r) {
     const double tk2 = (double)H.species[r.s2].stat * (tph * tph * tph) / H.species[r.s2].g;
     k.tk1 = k.tk3 = (R)tk1;
     k.tk2 = k.tk4 = (R)tk2;
-    k.par0 = (R)r.par[0];
+    k.par0 = (R)(r.kind == RBG_M2_ISO_DSIGMA ? 64.0 * M_PI * M_PI * r.par[0] : r.par[0]);
     k.mD2 = (R)(r.par[1] * r.par[1]);
     const double g2c = r.par[0] * r.par[0];
     k.g4 = (R)(g2c * g2c);
@@ -200,7 +201,8 @@ int run_roles(rbg_handle* h, const double* f, double* out, bool update, double d
         switch (r.kind) {
             case RBG_M2_CONST: e = launch_kq<R, rbg::KIND_CONST>(q, smem_path, spl, rp, lp, (int)grid, warps * 32, smem, st); break;
             case RBG_M2_COULOMB_SCREENED: e = launch_kq<R, rbg::KIND_COULOMB>(q, smem_path, spl, rp, lp, (int)grid, warps * 32, smem, st); break;
-            default: e = launch_kq<R, rbg::KIND_TCHAN_S2>(q, smem_path, spl, rp, lp, (int)grid, warps * 32, smem, st); break;
+            case RBG_M2_TCHAN_S2: e = launch_kq<R, rbg::KIND_TCHAN_S2>(q, smem_path, spl, rp, lp, (int)grid, warps * 32, smem, st); break;
+            default: e = launch_kq<R, rbg::KIND_ISO_DSIGMA>(q, smem_path, spl, rp, lp, (int)grid, warps * 32, smem, st); break;
         }
         if (e != cudaSuccess) return fail(h, RBG_E_CUDA, std::string("kernel launch: ") + cudaGetErrorString(e));
         ++h->last_launches;
@@ -269,7 +271,7 @@ int rbg_create(rbg_handle** out, const rbg_spatial_grid* grid, int n_species, co
         const int idx[4] = {p.a, p.b, p.c, p.d};
         for (int j = 0; j < 4; ++j)
             if (idx[j] < 0 || idx[j] >= n_species) { delete h; return fail(nullptr, RBG_E_INVALID_ARG, "process " + std::to_string(i) + ": species index out of range"); }
-        if (p.kind < RBG_M2_CONST || p.kind > RBG_M2_TCHAN_S2) { delete h; return fail(nullptr, RBG_E_INVALID_ARG, "process " + std::to_string(i) + ": unknown |M|^2 kind"); }
+        if (p.kind < RBG_M2_CONST || p.kind > RBG_M2_ISO_DSIGMA) { delete h; return fail(nullptr, RBG_E_INVALID_ARG, "process " + std::to_string(i) + ": unknown |M|^2 kind"); }
         if (p.c != p.a || p.d != p.b) { delete h; return fail(nullptr, RBG_E_UNSUPPORTED, "process " + std::to_string(i) + ": only elastic processes (c==a, d==b) are implemented"); }
         Role r;
         r.kind = p.kind; std::memcpy(r.par, p.par, sizeof r.par);
@@ -294,6 +296,27 @@ int rbg_collision(rbg_handle* h, const double* f_dev, double* C_dev, int n_sampl
 int rbg_collision_update(rbg_handle* h, const double* f_dev, double* f_out_dev, double dt, int* neg_flag_dev,
                          int n_samples, uint64_t seed, void* cuda_stream) {
     return run(h, f_dev, f_out_dev, true, dt, neg_flag_dev, n_samples, seed, cuda_stream);
+}
+
+int rbg_collision_evolve(rbg_handle* h, double* f_dev, double* scratch_dev, double dt, int n_steps, int* neg_flag_dev,
+                         int n_samples, uint64_t seed, void* cuda_stream) {
+    if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
+    if (n_steps < 0) return fail(h, RBG_E_INVALID_ARG, "n_steps must be >= 0");
+    if (!f_dev || !scratch_dev) return fail(h, RBG_E_INVALID_ARG, "null buffer");
+    const size_t bytes = h->f_elems * sizeof(double);
+    const char *a = (const char*)f_dev, *b = (const char*)scratch_dev;
+    if (a < b + bytes && b < a + bytes) return fail(h, RBG_E_INVALID_ARG, "scratch_dev overlaps f_dev");
+    double *cur = f_dev, *nxt = scratch_dev;
+    int launches = 0;
+    for (int k = 0; k < n_steps; ++k) {
+        const int rc = run(h, cur, nxt, true, dt, neg_flag_dev, n_samples, seed + (uint64_t)k, cuda_stream);
+        if (rc != RBG_OK) return rc;
+        launches += h->last_launches;
+        std::swap(cur, nxt);
+    }
+    if (cur != f_dev) RBG_CUDA(h, cudaMemcpyAsync(f_dev, cur, bytes, cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
+    h->last_launches = launches;
+    return RBG_OK;
 }
 
 int rbg_collision_host(rbg_handle* h, const double* f_host, double* C_host, int n_samples, uint64_t seed) {

@@ -57,3 +57,34 @@ def test_fullsize_config5_fused_update_fp32():
             ref = w["f"][sl] + w["dt"] * C_ref[sl]
             assert np.all(np.abs(got[sl] - ref) <= w["dt"] * TOL32 * mag[sl] + 4e-16 * np.abs(ref))
     assert int(flag.item()) == int((out < 0).sum().item())
+
+
+def test_paper_collision_test_thermalises_species_b():
+    """The paper's own collision workload at its full grid (35^3) through
+    rbg_collision_evolve: species b (dsigma/dOmega = 20) reaches exp(-E/T) with the T its conserved energy per
+    particle dictates, species a (dsigma/dOmega = 1) is still far from it (Fig. 9)."""
+    import paper_2308_04869_b200 as rbg
+    from test_oracle_thermalisation import boltzmann_fit, temperature_from_energy_per_particle
+    from workloads.configs import cell_centres
+    w = workloads.make(6)
+    col = rbg.Collision(w["problem"])
+    P = cell_centres(w["problem"]["grids"][0])
+    E = np.sqrt((P * P).sum(1) + 0.3 ** 2)
+    npc, dp3 = P.shape[0], (4.0 / 35) ** 3
+    f0 = w["f"]
+    f = torch.from_numpy(f0).cuda()
+    _, flag = col.collision_evolve(f, w["dt"], 60, w["n_samples"], w["seed"])
+    torch.cuda.synchronize()
+    got = f.cpu().numpy()
+    assert int(flag.item()) == int((got < 0).sum()) == 0
+    fa, fb = got[:npc], got[npc:]
+    (Ta, rms_a), (Tb, rms_b) = boltzmann_fit(fa, E), boltzmann_fit(fb, E)
+    T_pred = temperature_from_energy_per_particle((f0[npc:] * E).sum() / f0[npc:].sum(), 0.3)
+    assert rms_b < 0.12 and rms_a > 4 * rms_b, (rms_a, rms_b)
+    assert abs(Tb - T_pred) < 0.05 * T_pred, (Tb, T_pred)
+    assert abs(fa.sum() / f0[:npc].sum() - 1) < 5e-3
+    assert 0.93 < fb.sum() / f0[npc:].sum() < 1.01
+    # one step of it against the oracle, on the cells the oracle is asked for (every cell: nx = 1)
+    C = col.collision(torch.from_numpy(f0).cuda(), 16, w["seed"])
+    torch.cuda.synchronize()
+    _check_cells(dict(w, n_samples=16), C.cpu().numpy(), (0,), False)

@@ -60,6 +60,8 @@ CASES = [
     (3, dict(nx=2, np_side=8, n_samples=96)),
     (3, dict(nx=1, np_side=20, n_samples=16)),
     (4, dict(nx=5, np_side=20, n_samples=100)),
+    (6, dict(nx=2, np_side=9, n_samples=64)),               # kind ISO_DSIGMA (the paper's collision test)
+    (6, dict(n_samples=16)),                                # 35^3 tables (343 KB each): global/L2 gather path
 ]
 
 
@@ -75,7 +77,7 @@ def test_parity_fp64(cfg, kw):
 
 
 @pytest.mark.parametrize("cfg,kw", [(1, dict(nx=2, np_side=8, n_samples=128)), (2, dict(nx=2, np_side=10, n_samples=64)),
-                                    (3, dict(nx=1, np_side=8, n_samples=64))])
+                                    (3, dict(nx=1, np_side=8, n_samples=64)), (6, dict(nx=1, np_side=10, n_samples=64))])
 def test_parity_fp32_kinematics(cfg, kw):
     w = workloads.make(cfg, **kw)
     orc = oracle.Oracle(w["problem"], use_float=True)
@@ -219,3 +221,37 @@ def test_argument_errors():
         col.set_option("no_such_option", 1)
     with pytest.raises(rbg.RbgError):
         col.set_option("warps_per_cta", 99)
+
+
+def test_evolve_is_repeated_update():
+    """rbg_collision_evolve = n_steps x rbg_collision_update with seeds seed + k, result in place."""
+    rbg = _rbg()
+    w = workloads.make(6, nx=2, np_side=8, n_samples=48)
+    orc = oracle.Oracle(w["problem"])
+    dt = 5e-3
+    ref, mags = w["f"].copy(), []
+    for k in range(3):
+        C_ref, mag = oracle_C_and_scale(orc, ref, w["n_samples"], w["seed"] + k)
+        ref, _ = oracle.update(ref, C_ref, dt)
+        mags.append(mag)
+    col = rbg.Collision(w["problem"])
+    for steps in (3, 2, 1, 0):
+        f = torch.from_numpy(w["f"]).cuda()
+        got, flag = col.collision_evolve(f, dt, steps, w["n_samples"], w["seed"])
+        torch.cuda.synchronize()
+        assert got.data_ptr() == f.data_ptr()
+        assert col.last_launch_count() == steps * orc.n_roles
+        chain = torch.from_numpy(w["f"]).cuda()
+        for k in range(steps):
+            chain, _ = col.collision_update(chain, dt, w["n_samples"], w["seed"] + k)
+        torch.cuda.synchronize()
+        assert torch.equal(got, chain), steps
+        if steps == 3:
+            # each step's C agrees to TOL64 (G + L); a 1e-16 difference in f after step k feeds into step k+1
+            tol = dt * TOL64 * sum(mags) + 1e-13 * np.abs(ref).max()
+            assert np.all(np.abs(got.cpu().numpy() - ref) <= tol)
+    f = torch.from_numpy(w["f"]).cuda()
+    with pytest.raises(rbg.RbgError):
+        col.collision_evolve(f, dt, 1, 8, 1, scratch=f)
+    with pytest.raises(rbg.RbgError):
+        col.collision_evolve(f, dt, -1, 8, 1)

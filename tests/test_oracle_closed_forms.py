@@ -67,3 +67,43 @@ def test_p4_massive_loss_rate_matches_scipy():
     L, se = _loss_with_error(o, ip1, thermal, 777)
     assert se < 0.02 * ref
     assert abs(L - ref) < 4 * se + 1e-3 * ref, (L, ref, se)
+
+
+def _sigma_rate_quadrature(p1, m1, m2, T, dsigma):
+    """Eq. 20-21: loss rate / f1 = Int d3p2 f2 sigma_tot I / (E1 E2) with the invariant flux
+    I = sqrt((p1.p2)^2 - m1^2 m2^2) and sigma_tot = 4 pi dsigma/dOmega for an isotropic cross section."""
+    a1 = math.sqrt(p1 @ p1)
+    E1 = math.sqrt(a1 * a1 + m1 * m1)
+
+    def integrand(c, q):
+        E2 = math.sqrt(q * q + m2 * m2)
+        k12 = E1 * E2 - a1 * q * c                          # four-product p1.p2
+        flux = math.sqrt(max(k12 * k12 - (m1 * m2) ** 2, 0.0))
+        return 2 * math.pi * q * q * math.exp(-E2 / T) * 4 * math.pi * dsigma * flux / (E1 * E2)
+    val, err = integrate.dblquad(integrand, 0.0, 40.0 * T, -1.0, 1.0, epsabs=1e-12, epsrel=1e-10)
+    return val
+
+
+def test_iso_dsigma_kind_loss_rate_is_sigma_times_flux():
+    """Kind 3, |M|^2 = 64 pi^2 s dsigma/dOmega: the loss rate is f1 Int f2 sigma_tot v_Moller with
+    sigma_tot = 4 pi dsigma/dOmega (Eq. 20-22), for unequal masses."""
+    m1, m2, T, dsig = 0.3, 0.7, 0.6, 2.5
+    prob = dict(nx=1, species=[dict(mass=m1, charge=0, stat=0, g=1.0), dict(mass=m2, charge=0, stat=0, g=1.0)],
+                grids=[dict(n=[60] * 3, pmin=[-6.0] * 3, pmax=[6.0] * 3), dict(n=[60] * 3, pmin=[-9.0] * 3, pmax=[9.0] * 3)],
+                processes=[dict(a=0, b=1, c=0, d=1, kind=3, par=[dsig], sym=-1.0)], hbar=1.0)
+    o = oracle.Oracle(prob)
+    thermal = ("thermal", [[1.0, T, 0.0, m1, 0.0, 0, 0, 0], [1.0, T, 0.0, m2, 0.0, 0, 0, 0]])
+    ip1 = (33 * 60 + 26) * 60 + 35
+    tr = o.trace(None, 0, 0, ip1, 0, 1, fcb=thermal, box_cut=False)
+    ref = _sigma_rate_quadrature(tr["p1"], m1, m2, T, dsig) * tr["f1"]
+    L, se = _loss_with_error(o, ip1, thermal, 999)
+    assert se < 0.02 * ref
+    assert abs(L - ref) < 4 * se + 1e-3 * ref, (L, ref, se)
+    # per sample: the weight is the CONST-kind weight times 64 pi^2 s dsigma
+    prob0 = dict(prob, processes=[dict(a=0, b=1, c=0, d=1, kind=0, par=[1.0], sym=-1.0)])
+    o0 = oracle.Oracle(prob0)
+    for n in range(20):
+        a = o.trace(None, 0, 0, ip1, n, 5, fcb=thermal, box_cut=False)
+        b = o0.trace(None, 0, 0, ip1, n, 5, fcb=thermal, box_cut=False)
+        assert a["w"] == pytest.approx(b["w"] * 64 * math.pi ** 2 * a["s"] * dsig, rel=1e-14)
+        assert np.array_equal(a["p3"], b["p3"])

@@ -11,6 +11,7 @@ import numpy as np
 KIND_CONST = 0              # |M|^2 = par[0]
 KIND_COULOMB_SCREENED = 1   # |M|^2 = par[0] / (t - par[1]^2)^2
 KIND_TCHAN_S2 = 2           # |M|^2 = par[0]^4 s^2 / (t - par[1]^2)^2
+KIND_ISO_DSIGMA = 3         # |M|^2 = 64 pi^2 s par[0]  (constant CM-frame dsigma/dOmega = par[0])
 
 INPUT_SEED_BASE = 0x5EED0000
 MC_SEED_BASE = 20230810
@@ -121,6 +122,25 @@ def make(cfg: int, nx: int | None = None, n_samples: int | None = None, np_side:
         dens = 1.0 + 0.1 * (2.0 * rng.random(nx) - 1.0)
         fs = [dens[:, None] * prof[None, :]]
         name = "cfg4: 1 classical species, two counter-streaming beams, const |M|^2"
+    elif cfg == 6:
+        # The paper's own collision test (Eq. 46-48, Fig. 9): two classical species of
+        # mass 0.3, 1x1x1 spatial cell, 35^3 momentum cells on [-2,2]^3, step-function input with Q_s = 1,
+        # f_0 = 0.2 / 0.4, constant differential cross sections 1 (aa), 20 (bb), 0.01 (ab),
+        # dt = 0.0002/0.197, 25 000 steps.  Readings (R17-R19): the cross sections are taken as
+        # CM-frame isotropic; the occupied region is |p| < Q_s (Eq. 46-47 print the opposite inequality,
+        # which would fill the box to its corners); samples per cell and step are not stated (256 here).
+        nxd, N, side = 1, 256, 35
+        nx = nxd if nx is None else nx
+        side = side if np_side is None else np_side
+        species = [dict(mass=0.3, charge=0.0, stat=0, g=1.0), dict(mass=0.3, charge=0.0, stat=0, g=1.0)]
+        grids = [_grid(side, -2.0, 2.0), _grid(side, -2.0, 2.0)]
+        procs = [_elastic(0, 0, KIND_ISO_DSIGMA, [1.0]), _elastic(1, 1, KIND_ISO_DSIGMA, [20.0]),
+                 _elastic(0, 1, KIND_ISO_DSIGMA, [0.01])]
+        P = cell_centres(grids[0])
+        inside = ((P * P).sum(1) < 1.0).astype(np.float64)
+        fs = [np.tile(f0 * inside, (nx, 1)) for f0 in (0.2, 0.4)]
+        dt = 0.0002 / 0.197
+        name = "cfg6: paper's collision test (Eq. 46-48): 2 classical species m=0.3, const dsigma/dOmega 1/20/0.01"
     else:
         raise ValueError(f"unknown config {cfg}")
     problem = dict(nx=int(nx), species=species, grids=grids, processes=procs, hbar=1.0)
