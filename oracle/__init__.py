@@ -54,7 +54,7 @@ class _Grid(C.Structure):
 
 class _Process(C.Structure):
     _fields_ = [("a", C.c_int), ("b", C.c_int), ("c", C.c_int), ("d", C.c_int), ("kind", C.c_int),
-                ("par", C.c_double * 4), ("sym", C.c_double)]
+                ("par", C.c_double * 4), ("sym", C.c_double), ("sampler", C.c_int)]
 
 
 FCALLBACK = C.CFUNCTYPE(C.c_double, C.c_int, C.POINTER(C.c_double), C.c_void_p)
@@ -137,10 +137,10 @@ class Oracle:
                                       (C.c_double * 3)(*g["pmax"])) for g in gr])
         P = (_Process * len(pr))(*[_Process(p["a"], p["b"], p["c"], p["d"], p["kind"],
                                             (C.c_double * 4)(*(list(p["par"]) + [0.0] * 4)[:4]),
-                                            p.get("sym", -1.0)) for p in pr])
+                                            p.get("sym", -1.0), int(p.get("sampler", 0))) for p in pr])
         self._h = L.orc_create(self.nx, len(sp), S, G, len(pr), P, float(problem.get("hbar", 1.0)), int(use_float))
         if not self._h:
-            raise ValueError("oracle: unsupported problem (only elastic processes c==a, d==b)")
+            raise ValueError("oracle: unsupported problem (only elastic processes c==a, d==b; sampler 1 needs a t-channel kind)")
         self.n_species = len(sp)
         self.np = [int(np.prod(g["n"])) for g in gr]
         self.f_elems = int(L.orc_f_elems(self._h))

@@ -71,7 +71,7 @@ inline U4 philox4x32_10(uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1, uint
 // ---------------------------------------------------------------------------------------------
 struct Species { double mass, charge; int stat; double g; };
 struct Grid    { int n[3]; double pmin[3], pmax[3]; };
-struct Process { int a, b, c, d; int kind; double par[4]; double sym; };
+struct Process { int a, b, c, d; int kind; double par[4]; double sym; int sampler; };
 
 enum Kind { M2_CONST = 0, M2_COULOMB_SCREENED = 1, M2_TCHAN_S2 = 2,
             // |M|^2 = 64 pi^2 s par0: a constant differential cross section dsigma/dOmega = par0, isotropic in
@@ -81,7 +81,11 @@ enum Kind { M2_CONST = 0, M2_COULOMB_SCREENED = 1, M2_TCHAN_S2 = 2,
 
 // A role = one process seen from one grid species: particle 1 is the grid
 // particle, 2 its sampled partner, (3,4) the other pair.
-struct Role { int s[4]; int kind; double par[4]; double sym; int process; };
+// sampler: how the CM scattering direction is drawn.  0 = uniform on the sphere (O6); 1 = polar angle
+// about the CM direction of particle 1 drawn from the t-channel shape 1/(t - mD^2)^2 by its inverse CDF
+// (steps S1..S7 below), azimuth uniform.  Both estimate the same integral (R).
+enum Sampler { SAMPLER_UNIFORM = 0, SAMPLER_TCHANNEL = 1 };
+struct Role { int s[4]; int kind; double par[4]; double sym; int process; int sampler; };
 
 typedef double (*FCallback)(int species, const double* p, void* user);
 
@@ -117,6 +121,7 @@ struct Trace {
     int status;                // 0 ok, 1 skipped at O4 (h<=0), 2 below threshold
     int draws;                 // Philox calls consumed (always 1)
 };
+
 
 template <typename R> inline R rfma(R a, R b, R c);
 template <> inline double rfma<double>(double a, double b, double c) { return std::fma(a, b, c); }
@@ -168,9 +173,7 @@ template <> struct OctantPoly<float> {
 //   in-octant index r = k & (2^21 - 1), folded r' = b ? 2^21 - 1 - r : r, a = (r' + 1/2)(pi/4)/2^21,
 //   (cos, sin) of the angle inside the quadrant = b ? (sin a, cos a) : (cos a, sin a), then the
 //   exact rotation by q * pi/2.
-template <typename R> inline void direction(uint32_t x3, uint32_t k24, R nh[3]) {
-    const R nz = usym<R>(x3 | (sizeof(R) == 8 ? 1u : 0x100u));   // odd lattice: symmetric, never +-1
-    const R st = std::sqrt(rfma<R>(-nz, nz, (R)1));
+template <typename R> inline void azimuth(uint32_t k24, R& cphi, R& sphi) {
     const uint32_t q = k24 >> 22, b = (k24 >> 21) & 1u, r = k24 & 0x1FFFFFu;
     const uint32_t rf = b ? 0x1FFFFFu - r : r;
     const R A1 = (R)0x1.921fb54442d18p-22;       // (pi/4) / 2^21
@@ -179,15 +182,26 @@ template <typename R> inline void direction(uint32_t x3, uint32_t k24, R nh[3]) 
     R ca, sa;
     OctantPoly<R>::eval(a, ca, sa);
     const R c1 = b ? sa : ca, s1 = b ? ca : sa;  // angle in (0, pi/2)
-    R cphi, sphi;
     switch (q) {
         case 0:  cphi = c1;  sphi = s1;  break;
         case 1:  cphi = -s1; sphi = c1;  break;
         case 2:  cphi = -c1; sphi = -s1; break;
         default: cphi = s1;  sphi = -c1; break;
     }
+}
+template <typename R> inline void direction(uint32_t x3, uint32_t k24, R nh[3]) {
+    const R nz = usym<R>(x3 | (sizeof(R) == 8 ? 1u : 0x100u));   // odd lattice: symmetric, never +-1
+    const R st = std::sqrt(rfma<R>(-nz, nz, (R)1));
+    R cphi, sphi;
+    azimuth<R>(k24, cphi, sphi);
     nh[0] = st * cphi; nh[1] = st * sphi; nh[2] = nz;
 }
+
+// S2 (t-channel sampler): a word -> uniform real in (0,1) on the half-integer lattice, exact in both types:
+// double (x + 1/2) 2^-32, float ((x >> 8) + 1/2) 2^-24.  uhalf(~x) = 1 - uhalf(x) exactly.
+template <typename R> inline R uhalf(uint32_t x);
+template <> inline double uhalf<double>(uint32_t x) { return std::fma((double)x, 0x1p-32, 0x1p-33); }
+template <> inline float  uhalf<float>(uint32_t x) { return std::fmaf((float)(x >> 8), 0x1p-24f, 0x1p-25f); }
 
 template <typename R> struct RoleConst {
     R m[4], msq[4];
@@ -195,7 +209,7 @@ template <typename R> struct RoleConst {
     R pmin[4][3], L[4][3], invD[4][3], off[4][3];   // per particle slot (its species' grid)
     int n[4][3];
     R theta_kappa[4];
-    R par0, mD2, g4, sig64;
+    R par0, mD2, twomD2, g4, sig64;
 };
 
 template <typename R> inline R dot3(const R* a, const R* b) {
@@ -239,6 +253,7 @@ struct Evaluator {
         }
         k.par0 = (R)role.par[0];
         k.mD2  = (R)(role.par[1] * role.par[1]);
+        k.twomD2 = (R)(2.0 * (role.par[1] * role.par[1]));
         const double g2 = role.par[0] * role.par[0];
         k.g4   = (R)(g2 * g2);
         k.sig64 = (R)(64.0 * M_PI * M_PI * role.par[0]);     // M2_ISO_DSIGMA: |M|^2 = sig64 * s
@@ -334,20 +349,63 @@ struct Evaluator {
                 const R b34 = s - k.Mdf;                        // s - (m3-m4)^2
                 pf = std::sqrt(a34 * b34) * hirs;               // |p*_34|
                 const R E3s = (s + k.dm34) * hirs;              // (s + m3^2 - m4^2) / (2 sqrt s)
-                // ---- O6: direction uniform on the sphere, rejection-free and libm-free -------------
-                R nh[3];
-                direction<R>(r0.v[3], k24, nh);
-                // ---- O7: boost the CM momentum of particle 3 to the lab ---------------------
                 R p3s[3], P[3];
-                for (int d = 0; d < 3; ++d) { p3s[d] = pf * nh[d]; P[d] = p1[d] + p2[d]; }
+                for (int d = 0; d < 3; ++d) P[d] = p1[d] + p2[d];
                 const R Et = E1 + E2;
+                const R ig = (R)1 / (Et + rs);
+                const R ers = E2 * rs;
+                bool weight_done = false;
+                if (role.sampler == SAMPLER_TCHANNEL) {
+                    // ---- S1: CM momentum of particle 1 (inverse of the boost of O7; E1* = E3* for elastic roles)
+                    const R cb = (E1 + E3s) * ig;
+                    R v1[3];
+                    for (int d = 0; d < 3; ++d) v1[d] = rfma<R>(-P[d], cb, p1[d]);
+                    // ---- S2: om = 1 - cos(theta*) from the inverse CDF of 1/(t - mD^2)^2, t = -2 pf^2 om:
+                    //      om = 2 mD^2 v / (mD^2 + 4 (1 - v) pf^2),  v uniform in (0,1)
+                    const R v = uhalf<R>(r0.v[3]), vb = uhalf<R>(~r0.v[3]);
+                    const R q = pf * pf;
+                    const R den = rfma<R>((R)4 * vb, q, k.mD2);
+                    const R om = (k.twomD2 * v) / den;
+                    // ---- S3: polar angle
+                    const R st = std::sqrt(om * ((R)2 - om));
+                    const R ct = (R)1 - om;
+                    // ---- S4: azimuth (same lattice and polynomials as O6)
+                    R cphi, sphi;
+                    azimuth<R>(k24, cphi, sphi);
+                    const R A = st * cphi, B = st * sphi;
+                    // ---- S5: frame about v1 (Duff et al. 2017 orthonormal basis, scaled by |v1| = pf):
+                    //      pf e1 = (pf - sg x xa, -sg x ya, -sg x),  pf e2 = (-x ya, sg pf - y ya, -y),
+                    //      sg = sign(z), xa = x / (sg pf + z), ya = y / (sg pf + z)
+                    const R sg = v1[2] >= (R)0 ? (R)1 : (R)-1;
+                    const R ia = (R)1 / rfma<R>(sg, pf, v1[2]);
+                    const R xa = v1[0] * ia, ya = v1[1] * ia;
+                    const R sx = sg * v1[0];
+                    const R e1x = rfma<R>(-sx, xa, pf), e1y = -(sx * ya), e1z = -sx;
+                    const R e2x = -(v1[0] * ya), e2y = rfma<R>(-v1[1], ya, sg * pf), e2z = -v1[1];
+                    p3s[0] = rfma<R>(ct, v1[0], rfma<R>(B, e2x, A * e1x));
+                    p3s[1] = rfma<R>(ct, v1[1], rfma<R>(B, e2y, A * e1y));
+                    p3s[2] = rfma<R>(ct, v1[2], rfma<R>(B, e2z, A * e1z));
+                    // ---- S7: weight = |M|^2 pf / (E2 sqrt s) times the importance ratio
+                    //      (1/2) / pdf(om) = D^2 / (mD^2 (mD^2 + 4 pf^2)), D = mD^2 - t: the angular factor cancels
+                    t = -((R)2 * q) * om;
+                    const R zn = k.mD2 * rfma<R>((R)4, q, k.mD2);
+                    if (role.kind == M2_COULOMB_SCREENED) w = (k.par0 * pf) / (zn * ers);
+                    else                                  w = ((k.g4 * (s * s)) * pf) / (zn * ers);
+                    weight_done = true;
+                } else {
+                    // ---- O6: direction uniform on the sphere, rejection-free and libm-free ---------
+                    R nh[3];
+                    direction<R>(r0.v[3], k24, nh);
+                    for (int d = 0; d < 3; ++d) p3s[d] = pf * nh[d];
+                }
+                // ---- O7: boost the CM momentum of particle 3 to the lab ---------------------
                 const R dPn = dot3<R>(P, p3s);
                 E3 = rfma<R>(Et, E3s, dPn) * irs;               // gamma (E3* + beta.p3*)
-                const R c = (E3 + E3s) * ((R)1 / (Et + rs));    // p3 = p3* + P (E3+E3*)/(Et+sqrt s)
+                const R c = (E3 + E3s) * ig;                    // p3 = p3* + P (E3+E3*)/(Et+sqrt s)
                 for (int d = 0; d < 3; ++d) { p3[d] = rfma<R>(P[d], c, p3s[d]); p4[d] = P[d] - p3[d]; }
                 // ---- O8/O9/O12: t = (p1-p3)^2 and the weight as one quotient ---------------
-                const R ers = E2 * rs;
-                if (role.kind == M2_CONST) {
+                if (weight_done) {
+                } else if (role.kind == M2_CONST) {
                     w = (k.par0 * pf) / ers;
                 } else if (role.kind == M2_ISO_DSIGMA) {
                     w = ((k.sig64 * s) * pf) / ers;
@@ -483,8 +541,11 @@ void* orc_create(int nx, int n_species, const Species* sp, const Grid* grid, int
         const Process& p = pr[i];
         if (p.c != p.a || p.d != p.b) { delete H; return nullptr; }   // elastic roles only (R15)
         if (p.kind < M2_CONST || p.kind > M2_ISO_DSIGMA) { delete H; return nullptr; }
+        if (p.sampler != SAMPLER_UNIFORM && p.sampler != SAMPLER_TCHANNEL) { delete H; return nullptr; }
+        // the t-channel sampler needs a t-channel kind with a non-zero regulator
+        if (p.sampler == SAMPLER_TCHANNEL && !((p.kind == M2_COULOMB_SCREENED || p.kind == M2_TCHAN_S2) && p.par[1] != 0.0)) { delete H; return nullptr; }
         const double sym = p.sym < 0 ? (p.a == p.b ? 0.5 : 1.0) : p.sym;
-        Role r; r.kind = p.kind; std::memcpy(r.par, p.par, sizeof r.par); r.sym = sym; r.process = i;
+        Role r; r.kind = p.kind; std::memcpy(r.par, p.par, sizeof r.par); r.sym = sym; r.process = i; r.sampler = p.sampler;
         r.s[0] = p.a; r.s[1] = p.b; r.s[2] = p.c; r.s[3] = p.d;
         H->roles.push_back(r); H->role_off.push_back(roff); roff += (size_t)nx * H->np[p.a];
         if (p.b != p.a) {
