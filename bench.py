@@ -33,6 +33,8 @@ METRIC, UNIT = "collision_samples_per_s", "samples/s"
 # add/mul/compare/sqrt/divide = 1), by |M|^2 kind, classical statistics (+12 with quantum factors).
 FLOPS_PER_SAMPLE = {0: 141.0, 1: 155.0, 2: 157.0, 3: 142.0}
 QUANTUM_EXTRA_FLOPS = 10.0
+# the same count for the t-channel importance sampler (steps S1-S7), kinds 1 and 2
+FLOPS_PER_SAMPLE_TCHANNEL = {1: 185.0, 2: 187.0}
 FP64_LANES_PER_SM = 64          # FMA/clk/SM; confirmed by the live probe
 # dram__bytes_read.sum + dram__bytes_write.sum of one role launch from the committed `ncu --set full`
 # capture (profiles/r1b_chain_v2_cfg2.md: 32.84 MB + 1.64 MB, config 2 at full size); null elsewhere.
@@ -43,7 +45,8 @@ def flops_per_sweep(problem, n_samples):
     tot = 0.0
     for p in problem["processes"]:
         q = any(problem["species"][s]["stat"] != 0 for s in (p["a"], p["b"]))
-        per = FLOPS_PER_SAMPLE[p["kind"]] + (QUANTUM_EXTRA_FLOPS if q else 0.0)
+        table = FLOPS_PER_SAMPLE_TCHANNEL if p.get("sampler", 0) == 1 else FLOPS_PER_SAMPLE
+        per = table[p["kind"]] + (QUANTUM_EXTRA_FLOPS if q else 0.0)
         for s in ([p["a"]] if p["a"] == p["b"] else [p["a"], p["b"]]):
             tot += per * problem["nx"] * int(np.prod(problem["grids"][s]["n"])) * n_samples
     return tot
@@ -113,7 +116,7 @@ def run_reference(args):
     """--impl reference: the oracle on this box's host cores, same config/metric (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    w = workloads.make(args.config)
+    w = workloads.make(args.config, sampler=args.sampler)
     nx = w["problem"]["nx"]
     ncell = max(1, min(nx, args.ref_cells))
     cells = [int(i) for i in np.linspace(0, nx - 1, ncell).astype(int)]
@@ -148,6 +151,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--nx", type=int, default=None, help="override the number of spatial cells (profiling runs; "
                     "the JSON line then names the reduced workload)")
+    ap.add_argument("--sampler", type=int, default=0, choices=[0, 1], help="1: t-channel importance sampler on the "
+                    "t-channel processes (configs 2, 3, 5); the JSON line then names it")
     ap.add_argument("--opt", action="append", default=[], help="librbg option key=value (launch geometry)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -167,7 +172,7 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
-    w = workloads.make(args.config, nx=args.nx)
+    w = workloads.make(args.config, nx=args.nx, sampler=args.sampler)
     if args.nx is not None:
         w["name"] += f" [nx overridden to {args.nx}]"
     prob = w["problem"]
@@ -244,7 +249,7 @@ def main():
     if w["fp32"]:
         peak_nominal *= 2                       # 128 fp32 lanes per SM
     roof = {"bound": "alu", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s", "frac": achieved / peak_nominal,
-            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.config) if args.nx is None else None,
+            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.config) if args.nx is None and not args.sampler else None,
             "traffic_unit": "bytes per launch (ncu capture, profiles/r1b_chain_v2_cfg2.md)", "peak_source": f"{sms} SM x {FP64_LANES_PER_SM * (2 if w['fp32'] else 1)} FMA/clk x 2 x "
                                             f"{max_mhz:.0f} MHz (DESIGN.md section 8)",
             "peak_probe_tflops": probe, "frac_of_probe": achieved / probe,

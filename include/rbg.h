@@ -78,15 +78,25 @@ typedef enum {
                                      DESIGN.md reading R17)                           */
 } rbg_m2_kind;
 
+/* How the CM scattering direction of a process is drawn (both estimate the same integral):
+ *   RBG_SAMPLER_UNIFORM   uniform on the sphere;
+ *   RBG_SAMPLER_TCHANNEL  polar angle about the CM direction of the grid particle drawn from the shape
+ *                         1/(t - par[1]^2)^2 of the screened t-channel kinds by its inverse CDF, azimuth
+ *                         uniform; the angular factor of |M|^2 then cancels in the weight (DESIGN.md
+ *                         section 4b).  Only with RBG_M2_COULOMB_SCREENED / RBG_M2_TCHAN_S2 and par[1] != 0;
+ *                         removes the (p* / par[1])^2-sized variance of sampling a forward peak uniformly. */
+#define RBG_SAMPLER_UNIFORM  0
+#define RBG_SAMPLER_TCHANNEL 1
+
 /* Process a + b -> c + d (species indices).  Only elastic processes (c == a, d == b) are
  * implemented; anything else is RBG_E_UNSUPPORTED.  sym < 0 selects the paper's rule
  * (PAPER.md:208): 1/2 if a == b, else 1. */
-typedef struct { int a, b, c, d; int kind; double par[4]; double sym; } rbg_process;
+typedef struct { int a, b, c, d; int kind; double par[4]; double sym; int sampler; } rbg_process;
 
 /* Create a handle.  Returns RBG_OK and stores the handle in *out, or a negative code (then *out
  * is NULL and rbg_last_error(NULL) has the text).  Rejects: non-positive grid counts,
  * pmax <= pmin, negative mass, stat not in {0,+1,-1}, g <= 0, species index out of range,
- * unknown kind or flags, inelastic processes, no CUDA device. */
+ * unknown kind, sampler or flags, a sampler that does not fit the kind, inelastic processes, no CUDA device. */
 int rbg_create(rbg_handle** out, const rbg_spatial_grid* grid, int n_species, const rbg_species* species,
                const rbg_momentum_grid* momentum_grids /* [n_species] */, int n_process,
                const rbg_process* processes, double hbar, int flags);

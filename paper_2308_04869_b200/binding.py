@@ -8,6 +8,7 @@ import numpy as np
 
 KIND_CONST, KIND_COULOMB_SCREENED, KIND_TCHAN_S2, KIND_ISO_DSIGMA = 0, 1, 2, 3
 RBG_FP64, RBG_FP32_KINEMATICS = 0, 1
+SAMPLER_UNIFORM, SAMPLER_TCHANNEL = 0, 1
 
 _PKG = Path(__file__).resolve().parent
 _LIB_PATH = _PKG / "librbg.so"
@@ -32,7 +33,7 @@ class _Species(C.Structure):
 
 class _Process(C.Structure):
     _fields_ = [("a", C.c_int), ("b", C.c_int), ("c", C.c_int), ("d", C.c_int), ("kind", C.c_int),
-                ("par", C.c_double * 4), ("sym", C.c_double)]
+                ("par", C.c_double * 4), ("sym", C.c_double), ("sampler", C.c_int)]
 
 
 # every symbol include/rbg.h declares
@@ -121,7 +122,7 @@ class Collision:
                                                       (C.c_double * 3)(*g["pmax"])) for g in gr])
         P = (_Process * max(len(pr), 1))(*[_Process(p["a"], p["b"], p["c"], p["d"], p["kind"],
                                                     (C.c_double * 4)(*(list(p["par"]) + [0.0] * 4)[:4]),
-                                                    p.get("sym", -1.0)) for p in pr])
+                                                    p.get("sym", -1.0), int(p.get("sampler", 0))) for p in pr])
         h = C.c_void_p()
         _check(lib.rbg_create(C.byref(h), C.byref(sg), len(sp), S, G, len(pr), P, float(problem.get("hbar", 1.0)),
                               RBG_FP32_KINEMATICS if fp32_kinematics else RBG_FP64))

@@ -24,6 +24,7 @@ struct Role {
     double par[4];
     double sym;
     int index;             // global role index
+    int sampler;           // RBG_SAMPLER_*
 };
 
 }  // namespace
@@ -104,6 +105,7 @@ rbg::RoleParams<R> make_role_params(const rbg_handle& H, const Role& r) {
     k.tk2 = k.tk4 = (R)tk2;
     k.par0 = (R)(r.kind == RBG_M2_ISO_DSIGMA ? 64.0 * M_PI * M_PI * r.par[0] : r.par[0]);
     k.mD2 = (R)(r.par[1] * r.par[1]);
+    k.twomD2 = (R)(2.0 * (r.par[1] * r.par[1]));
     const double g2c = r.par[0] * r.par[0];
     k.g4 = (R)(g2c * g2c);
     k.symV2 = r.sym * V2;
@@ -113,10 +115,10 @@ rbg::RoleParams<R> make_role_params(const rbg_handle& H, const Role& r) {
     return k;
 }
 
-template <typename R, int KIND, bool Q, bool SMEM, int MAXT, int SPL>
+template <typename R, int KIND, bool Q, bool SMEM, int MAXT, int SPL, bool TCH>
 cudaError_t launch_one(const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp, int grid, int threads, size_t smem,
                        cudaStream_t st) {
-    auto kern = rbg::collision_role_kernel<R, KIND, Q, SMEM, MAXT, SPL>;
+    auto kern = rbg::collision_role_kernel<R, KIND, Q, SMEM, MAXT, SPL, TCH>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kern<<<grid, threads, smem, st>>>(rp, lp);
@@ -125,21 +127,21 @@ cudaError_t launch_one(const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp
 
 // geometry variant: CTAs of up to 512 threads evaluate SPL = 1 or 2 samples per lane and iteration
 // (up to 128 registers per thread); CTAs of up to 1024 threads evaluate 1 (64 registers).
-template <typename R, int KIND, bool Q, bool SMEM>
+template <typename R, int KIND, bool Q, bool SMEM, bool TCH>
 cudaError_t launch_geo(int spl, const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp, int grid, int threads,
                        size_t smem, cudaStream_t st) {
-    if (threads > 512) return launch_one<R, KIND, Q, SMEM, 1024, 1>(rp, lp, grid, threads, smem, st);
-    if (spl == 2) return launch_one<R, KIND, Q, SMEM, 512, 2>(rp, lp, grid, threads, smem, st);
-    return launch_one<R, KIND, Q, SMEM, 512, 1>(rp, lp, grid, threads, smem, st);
+    if (threads > 512) return launch_one<R, KIND, Q, SMEM, 1024, 1, TCH>(rp, lp, grid, threads, smem, st);
+    if (spl == 2) return launch_one<R, KIND, Q, SMEM, 512, 2, TCH>(rp, lp, grid, threads, smem, st);
+    return launch_one<R, KIND, Q, SMEM, 512, 1, TCH>(rp, lp, grid, threads, smem, st);
 }
 
-template <typename R, int KIND>
+template <typename R, int KIND, bool TCH>
 cudaError_t launch_kq(bool q, bool smem_path, int spl, const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp, int grid,
                       int threads, size_t smem, cudaStream_t st) {
-    if (q) return smem_path ? launch_geo<R, KIND, true, true>(spl, rp, lp, grid, threads, smem, st)
-                            : launch_geo<R, KIND, true, false>(spl, rp, lp, grid, threads, smem, st);
-    return smem_path ? launch_geo<R, KIND, false, true>(spl, rp, lp, grid, threads, smem, st)
-                     : launch_geo<R, KIND, false, false>(spl, rp, lp, grid, threads, smem, st);
+    if (q) return smem_path ? launch_geo<R, KIND, true, true, TCH>(spl, rp, lp, grid, threads, smem, st)
+                            : launch_geo<R, KIND, true, false, TCH>(spl, rp, lp, grid, threads, smem, st);
+    return smem_path ? launch_geo<R, KIND, false, true, TCH>(spl, rp, lp, grid, threads, smem, st)
+                     : launch_geo<R, KIND, false, false, TCH>(spl, rp, lp, grid, threads, smem, st);
 }
 
 template <typename R>
@@ -198,11 +200,19 @@ int run_roles(rbg_handle* h, const double* f, double* out, bool update, double d
         if (grid > 0x7fffffffL) return fail(h, RBG_E_UNSUPPORTED, "grid too large; raise p1_per_cta");
         const bool q = h->species[r.s1].stat != 0 || h->species[r.s2].stat != 0;
         cudaError_t e;
+        const bool tch = r.sampler == RBG_SAMPLER_TCHANNEL;
+        const int th = warps * 32;
         switch (r.kind) {
-            case RBG_M2_CONST: e = launch_kq<R, rbg::KIND_CONST>(q, smem_path, spl, rp, lp, (int)grid, warps * 32, smem, st); break;
-            case RBG_M2_COULOMB_SCREENED: e = launch_kq<R, rbg::KIND_COULOMB>(q, smem_path, spl, rp, lp, (int)grid, warps * 32, smem, st); break;
-            case RBG_M2_TCHAN_S2: e = launch_kq<R, rbg::KIND_TCHAN_S2>(q, smem_path, spl, rp, lp, (int)grid, warps * 32, smem, st); break;
-            default: e = launch_kq<R, rbg::KIND_ISO_DSIGMA>(q, smem_path, spl, rp, lp, (int)grid, warps * 32, smem, st); break;
+            case RBG_M2_CONST: e = launch_kq<R, rbg::KIND_CONST, false>(q, smem_path, spl, rp, lp, (int)grid, th, smem, st); break;
+            case RBG_M2_COULOMB_SCREENED:
+                e = tch ? launch_kq<R, rbg::KIND_COULOMB, true>(q, smem_path, spl, rp, lp, (int)grid, th, smem, st)
+                        : launch_kq<R, rbg::KIND_COULOMB, false>(q, smem_path, spl, rp, lp, (int)grid, th, smem, st);
+                break;
+            case RBG_M2_TCHAN_S2:
+                e = tch ? launch_kq<R, rbg::KIND_TCHAN_S2, true>(q, smem_path, spl, rp, lp, (int)grid, th, smem, st)
+                        : launch_kq<R, rbg::KIND_TCHAN_S2, false>(q, smem_path, spl, rp, lp, (int)grid, th, smem, st);
+                break;
+            default: e = launch_kq<R, rbg::KIND_ISO_DSIGMA, false>(q, smem_path, spl, rp, lp, (int)grid, th, smem, st); break;
         }
         if (e != cudaSuccess) return fail(h, RBG_E_CUDA, std::string("kernel launch: ") + cudaGetErrorString(e));
         ++h->last_launches;
@@ -273,7 +283,13 @@ int rbg_create(rbg_handle** out, const rbg_spatial_grid* grid, int n_species, co
             if (idx[j] < 0 || idx[j] >= n_species) { delete h; return fail(nullptr, RBG_E_INVALID_ARG, "process " + std::to_string(i) + ": species index out of range"); }
         if (p.kind < RBG_M2_CONST || p.kind > RBG_M2_ISO_DSIGMA) { delete h; return fail(nullptr, RBG_E_INVALID_ARG, "process " + std::to_string(i) + ": unknown |M|^2 kind"); }
         if (p.c != p.a || p.d != p.b) { delete h; return fail(nullptr, RBG_E_UNSUPPORTED, "process " + std::to_string(i) + ": only elastic processes (c==a, d==b) are implemented"); }
+        if (p.sampler != RBG_SAMPLER_UNIFORM && p.sampler != RBG_SAMPLER_TCHANNEL) { delete h; return fail(nullptr, RBG_E_INVALID_ARG, "process " + std::to_string(i) + ": unknown sampler"); }
+        if (p.sampler == RBG_SAMPLER_TCHANNEL && !((p.kind == RBG_M2_COULOMB_SCREENED || p.kind == RBG_M2_TCHAN_S2) && p.par[1] != 0.0)) {
+            delete h;
+            return fail(nullptr, RBG_E_INVALID_ARG, "process " + std::to_string(i) + ": the t-channel sampler needs a t-channel |M|^2 kind with a non-zero regulator par[1]");
+        }
         Role r;
+        r.sampler = p.sampler;
         r.kind = p.kind; std::memcpy(r.par, p.par, sizeof r.par);
         r.sym = p.sym < 0 ? (p.a == p.b ? 0.5 : 1.0) : p.sym;
         r.s1 = p.a; r.s2 = p.b; r.index = (int)h->roles.size();

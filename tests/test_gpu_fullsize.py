@@ -88,3 +88,28 @@ def test_paper_collision_test_thermalises_species_b():
     C = col.collision(torch.from_numpy(f0).cuda(), 16, w["seed"])
     torch.cuda.synchronize()
     _check_cells(dict(w, n_samples=16), C.cpu().numpy(), (0,), False)
+
+
+def test_fullsize_config2_tchannel_sampler():
+    """Config 2 at full size with the t-channel importance sampler: sampled parity, and the per-cell scatter of
+    C across spatial cells (which differ only by their density factor and their random streams) is far below
+    the uniform sampler's."""
+    import paper_2308_04869_b200 as rbg
+    res = {}
+    for sampler in (1, 0):
+        w = workloads.make(2, sampler=sampler)
+        col = rbg.Collision(w["problem"])
+        C = col.collision(torch.from_numpy(w["f"]).cuda(), w["n_samples"], w["seed"])
+        torch.cuda.synchronize()
+        if sampler == 1:
+            _check_cells(w, C.cpu().numpy(), (3, 508), False)
+        res[sampler] = C
+    # H+ block: C(x, p) / n(x)^2 is the same function of p in every spatial cell up to Monte Carlo noise
+    offs, _ = workloads.f_layout(w["problem"])
+    nx, npc = w["problem"]["nx"], 8000
+    dens = torch.from_numpy(w["f"][offs[1]:offs[1] + nx * npc].reshape(nx, npc)[:, 0] / w["f"][offs[1]]).cuda()
+    noise = {}
+    for sampler, C in res.items():
+        blk = C[offs[1]:offs[1] + nx * npc].view(nx, npc) / (dens * dens)[:, None]
+        noise[sampler] = float(blk.std(0).mean())
+    assert noise[1] < 0.2 * noise[0], noise

@@ -256,3 +256,33 @@ def test_evolve_is_repeated_update():
         col.collision_evolve(f, dt, 1, 8, 1, scratch=f)
     with pytest.raises(rbg.RbgError):
         col.collision_evolve(f, dt, -1, 8, 1)
+
+
+@pytest.mark.parametrize("cfg,kw,fp32", [(2, dict(nx=3, np_side=20, n_samples=64), False), (2, dict(nx=2, np_side=7, n_samples=33), False),
+                                         (3, dict(nx=2, np_side=8, n_samples=96), False), (2, dict(nx=2, np_side=10, n_samples=64), True),
+                                         (3, dict(nx=1, np_side=8, n_samples=64), True)])
+def test_parity_tchannel_importance_sampler(cfg, kw, fp32):
+    """sampler = 1: same bar as the uniform sampler, both precisions, and a result that
+    differs from the uniform sampler's (the two draw different directions from the same words)."""
+    w = workloads.make(cfg, sampler=1, **kw)
+    assert all(p.get("sampler") == 1 for p in w["problem"]["processes"])
+    orc = oracle.Oracle(w["problem"], use_float=fp32)
+    C_ref, mag = oracle_C_and_scale(orc, w["f"], w["n_samples"], w["seed"])
+    C, col = gpu_C(w["problem"], w["f"], w["n_samples"], w["seed"], fp32=fp32)
+    assert_parity(C, C_ref, mag, TOL32 if fp32 else TOL64, f"tchannel cfg{cfg} {kw}")
+    w0 = workloads.make(cfg, **kw)
+    C0, _ = gpu_C(w0["problem"], w0["f"], w0["n_samples"], w0["seed"], fp32=fp32)
+    assert not np.array_equal(C, C0)
+    if not fp32:
+        other, _ = gpu_C(w["problem"], w["f"], w["n_samples"], w["seed"], options=[("gather", 2), ("warps_per_cta", 5)])
+        assert np.array_equal(C, other)
+
+
+def test_sampler_argument_errors():
+    rbg = _rbg()
+    P = workloads.make(1, np_side=4)["problem"]
+    for bad in (dict(P, processes=[dict(P["processes"][0], sampler=1)]),                     # CONST kind
+                dict(P, processes=[dict(P["processes"][0], kind=1, par=[1.0, 0.0], sampler=1)]),   # no regulator
+                dict(P, processes=[dict(P["processes"][0], kind=1, par=[1.0, 0.1], sampler=7)])):
+        with pytest.raises(rbg.RbgError):
+            rbg.Collision(bad)

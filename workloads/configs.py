@@ -49,10 +49,12 @@ def _elastic(a, b, kind, par):
     return dict(a=a, b=b, c=a, d=b, kind=kind, par=list(par), sym=-1.0)
 
 
-def make(cfg: int, nx: int | None = None, n_samples: int | None = None, np_side: int | None = None):
+def make(cfg: int, nx: int | None = None, n_samples: int | None = None, np_side: int | None = None,
+         sampler: int = 0):
     """Return dict(name, problem, f, n_samples, seed, dt, fp32).  ``nx``/``n_samples``/``np_side``
     override the config's spatial cell count / sample count / momentum cells per axis (tests use
-    reduced sizes; bench.py uses the defaults)."""
+    reduced sizes; bench.py uses the defaults).  ``sampler`` = 1 asks for the t-channel importance
+    sampler on every process whose |M|^2 kind has the t-channel shape (configs 2, 3, 5)."""
     rng = np.random.Generator(np.random.PCG64(INPUT_SEED_BASE + cfg))
     seed = MC_SEED_BASE + cfg
     dt, fp32 = 0.0, False
@@ -143,6 +145,11 @@ def make(cfg: int, nx: int | None = None, n_samples: int | None = None, np_side:
         name = "cfg6: paper's collision test (Eq. 46-48): 2 classical species m=0.3, const dsigma/dOmega 1/20/0.01"
     else:
         raise ValueError(f"unknown config {cfg}")
+    if sampler:
+        for p in procs:
+            if p["kind"] in (KIND_COULOMB_SCREENED, KIND_TCHAN_S2):
+                p["sampler"] = int(sampler)
+        name += " [t-channel importance sampler]"
     problem = dict(nx=int(nx), species=species, grids=grids, processes=procs, hbar=1.0)
     f = np.concatenate([np.ascontiguousarray(a, dtype=np.float64).reshape(-1) for a in fs])
     return dict(cfg=cfg, name=name, problem=problem, f=f, n_samples=int(N if n_samples is None else n_samples),
