@@ -37,8 +37,8 @@ QUANTUM_EXTRA_FLOPS = 10.0
 FLOPS_PER_SAMPLE_TCHANNEL = {1: 185.0, 2: 187.0}
 FP64_LANES_PER_SM = 64          # FMA/clk/SM; confirmed by the live probe
 # dram__bytes_read.sum + dram__bytes_write.sum of one role launch from the committed `ncu --set full`
-# capture (profiles/r1b_chain_v2_cfg2.md: 32.84 MB + 1.64 MB, config 2 at full size); null elsewhere.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {2: 34.48e6}
+# capture (profiles/r1c_chain_v2_cfg2.md: 32.87 MB + 2.15 MB, config 2 at full size); null elsewhere.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {2: 35.02e6}
 
 
 def flops_per_sweep(problem, n_samples):
@@ -250,7 +250,7 @@ def main():
         peak_nominal *= 2                       # 128 fp32 lanes per SM
     roof = {"bound": "alu", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s", "frac": achieved / peak_nominal,
             "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.config) if args.nx is None and not args.sampler else None,
-            "traffic_unit": "bytes per launch (ncu capture, profiles/r1b_chain_v2_cfg2.md)", "peak_source": f"{sms} SM x {FP64_LANES_PER_SM * (2 if w['fp32'] else 1)} FMA/clk x 2 x "
+            "traffic_unit": "bytes per launch (ncu capture, profiles/r1c_chain_v2_cfg2.md)", "peak_source": f"{sms} SM x {FP64_LANES_PER_SM * (2 if w['fp32'] else 1)} FMA/clk x 2 x "
                                             f"{max_mhz:.0f} MHz (DESIGN.md section 8)",
             "peak_probe_tflops": probe, "frac_of_probe": achieved / probe,
             "kernel": "rbg::collision_role_kernel", "launch_ms": t_launch * 1e3,

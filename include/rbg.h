@@ -148,6 +148,13 @@ void rbg_destroy(rbg_handle* h);
  * one FMA as one operation.  Used by bench.py for the live roofline denominator. */
 int rbg_probe_alu_peak(int what, int iters, double* ops_per_s, void* cuda_stream);
 
+/* Measurement helper for the instruction-issue bound: one CTA of warps_per_sm warps per SM
+ * loops over n_fp64 DFMA + n_imad IMAD + n_lop3 LOP3 on independent registers; *cycles_per_iter is the SM clock
+ * span of one loop iteration of the whole CTA (divide by warps_per_sm / 4 for cycles per warp-iteration per
+ * scheduler).  Supported mixes (n_fp64, n_imad, n_lop3): (8,0,0) (0,8,0) (0,0,8) (0,4,4) (0,8,8) (8,2,2) (8,4,4)
+ * (8,8,0) (8,0,8) (8,8,8).  Synchronous, default stream. */
+int rbg_probe_issue_mix(int n_fp64, int n_imad, int n_lop3, int warps_per_sm, int iters, double* cycles_per_iter);
+
 /* Diagnostic: compares the kernels' own fp64 and fp32 divide / reciprocal / square-root sequences
  * (the round-to-nearest fast paths without range checks) bit for bit with the
  * CUDA library operators on n_operands random operand sets (10 comparisons each); *mismatches must

@@ -8,6 +8,6 @@ CUDA device the calls raise.
 from __future__ import annotations
 
 from .binding import (  # noqa: F401
-    Collision, RbgError, KIND_CONST, KIND_COULOMB_SCREENED, KIND_TCHAN_S2, KIND_ISO_DSIGMA, load_library, probe_alu_peak,
+    Collision, RbgError, KIND_CONST, KIND_COULOMB_SCREENED, KIND_TCHAN_S2, KIND_ISO_DSIGMA, load_library, probe_alu_peak, probe_issue_mix,
     exported_symbols, selftest_math,
 )

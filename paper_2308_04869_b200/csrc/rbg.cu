@@ -426,4 +426,37 @@ int rbg_probe_alu_peak(int what, int iters, double* ops_per_s, void* cuda_stream
     return RBG_OK;
 }
 
+int rbg_probe_issue_mix(int n_fp64, int n_imad, int n_lop3, int warps_per_sm, int iters, double* cycles_per_iter) {
+    if (!cycles_per_iter || iters <= 0 || warps_per_sm < 1 || warps_per_sm > 32) return fail(nullptr, RBG_E_INVALID_ARG, "bad probe arguments");
+    int dev = 0, sms = 0;
+    RBG_CUDA(nullptr, cudaGetDevice(&dev));
+    RBG_CUDA(nullptr, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    void (*kern)(double*, int, long long*) = nullptr;
+    const int key = n_fp64 * 100 + n_imad * 10 + n_lop3;
+    switch (key) {
+        case 800: kern = rbg::issue_mix_kernel<8, 0, 0>; break;
+        case 80:  kern = rbg::issue_mix_kernel<0, 8, 0>; break;
+        case 8:   kern = rbg::issue_mix_kernel<0, 0, 8>; break;
+        case 44:  kern = rbg::issue_mix_kernel<0, 4, 4>; break;
+        case 88:  kern = rbg::issue_mix_kernel<0, 8, 8>; break;
+        case 822: kern = rbg::issue_mix_kernel<8, 2, 2>; break;
+        case 844: kern = rbg::issue_mix_kernel<8, 4, 4>; break;
+        case 880: kern = rbg::issue_mix_kernel<8, 8, 0>; break;
+        case 808: kern = rbg::issue_mix_kernel<8, 0, 8>; break;
+        case 888: kern = rbg::issue_mix_kernel<8, 8, 8>; break;
+        default: return fail(nullptr, RBG_E_INVALID_ARG, "unsupported mix (see include/rbg.h)");
+    }
+    double* out = nullptr; long long* cyc = nullptr;
+    RBG_CUDA(nullptr, cudaMalloc(&out, (size_t)sms * 1024 * sizeof(double)));
+    RBG_CUDA(nullptr, cudaMalloc(&cyc, sizeof(long long)));
+    for (int rep = 0; rep < 2; ++rep) kern<<<sms, warps_per_sm * 32>>>(out, iters, cyc);
+    cudaError_t e = cudaDeviceSynchronize();
+    long long h = 0;
+    if (e == cudaSuccess) e = cudaMemcpy(&h, cyc, sizeof h, cudaMemcpyDeviceToHost);
+    cudaFree(out); cudaFree(cyc);
+    if (e != cudaSuccess) return fail(nullptr, RBG_E_CUDA, cudaGetErrorString(e));
+    *cycles_per_iter = (double)h / iters;
+    return RBG_OK;
+}
+
 }  // extern "C"
