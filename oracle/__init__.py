@@ -87,6 +87,8 @@ def lib():
                                           dp, C.c_void_p, C.c_void_p, C.c_int]
         L.orc_trace.argtypes = [C.c_void_p, dp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_uint64, dp,
                                 C.POINTER(C.c_int), C.c_void_p, C.c_void_p, C.c_int]
+        L.orc_m2_qcd.restype = C.c_double
+        L.orc_m2_qcd.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_double]
         L.orc_update.restype = C.c_long
         L.orc_update.argtypes = [C.c_size_t, dp, dp, C.c_double, dp]
         L.orc_philox4x32_10.argtypes = [C.POINTER(C.c_uint32)] * 3
@@ -119,7 +121,7 @@ def _dp(a):
     return a.ctypes.data_as(C.POINTER(C.c_double)) if a is not None else None
 
 
-TRACE_FIELDS = ("E1", "E2", "E3", "s", "t", "pf", "w", "f1", "f2", "f3", "f4", "gain", "loss")
+TRACE_FIELDS = ("E1", "E2", "E3", "s", "t", "pf", "w", "f1", "f2", "f3", "f4", "gain", "loss", "u")
 
 
 class Oracle:
@@ -140,7 +142,7 @@ class Oracle:
                                             p.get("sym", -1.0), int(p.get("sampler", 0))) for p in pr])
         self._h = L.orc_create(self.nx, len(sp), S, G, len(pr), P, float(problem.get("hbar", 1.0)), int(use_float))
         if not self._h:
-            raise ValueError("oracle: unsupported problem (only elastic processes c==a, d==b; sampler 1 needs a t-channel kind)")
+            raise ValueError("oracle: unsupported problem (unknown kind or sampler; a+b->b+a must be written a+b->a+b; sampler 1 needs an elastic t-channel kind)")
         self.n_species = len(sp)
         self.np = [int(np.prod(g["n"])) for g in gr]
         self.f_elems = int(L.orc_f_elems(self._h))
@@ -204,9 +206,13 @@ class Oracle:
                                   int(box_cut))
         return out
 
+    def m2_qcd(self, role, s, t, u):
+        """|M|^2(s,t,u) of a Table III role as the sample loop evaluates it."""
+        return float(lib().orc_m2_qcd(self._h, int(role), float(s), float(t), float(u)))
+
     def trace(self, f, role, ix, ip1, n, seed, fcb=None, box_cut=True):
         f = np.ascontiguousarray(f, dtype=np.float64) if f is not None else np.zeros(self.f_elems)
-        dout = np.zeros(25)
+        dout = np.zeros(26)
         iout = (C.c_int * 5)()
         keep, ptr = self._cb(fcb)
         lib().orc_trace(self._h, _dp(f), role, ix, ip1, n, int(seed), _dp(dout), iout, *self._fp(ptr), int(box_cut))

@@ -28,7 +28,9 @@
 // massless closed form, a scipy quadrature of the loss rate, exact detailed balance for
 // MJ/FD/BE inputs, the paper's own 5-D form Eq. 37 (oracle/eq37.py), number/energy conservation,
 // deterministic brute-force quadrature of (R) (oracle/quadrature.py), H-theorem sign,
-// thread-count independence.  No function here is "parity unpinned".
+// thread-count independence; Table III kinds against textbook values, crossing symmetry and regulator limits;
+// inelastic roles against per-sample kinematics, detailed balance, the quadrature and cross-species bookkeeping
+// (tests/test_oracle_qcd.py).  No function here is "parity unpinned".
 #include <cmath>
 #include <cstdint>
 #include <cstdlib>
@@ -77,7 +79,22 @@ enum Kind { M2_CONST = 0, M2_COULOMB_SCREENED = 1, M2_TCHAN_S2 = 2,
             // |M|^2 = 64 pi^2 s par0: a constant differential cross section dsigma/dOmega = par0, isotropic in
             // the CM frame (the paper's collision test quotes its processes this way, Eq. 48 PAPER.md:493-500;
             // relation cross section <-> matrix element: Eq. 20-22, reading R17)
-            M2_ISO_DSIGMA = 3 };
+            M2_ISO_DSIGMA = 3,
+            // Table III: |M|^2 of the 2->2 parton processes of QCD, summed over the helicities and
+            // colours of all four particles, with the regulator m_g^2 = par1^2 subtracted from t and u in the
+            // denominators; g = par0; SU_c(3): d_F = C_A = 3, C_F = 4/3, d_A = 8.  t = (p1-p3)^2, u = (p1-p4)^2
+            // (role labels; the role permutations of orc_create keep t and u those of the process as written).
+            // Rows :677, :679, :683-684 and :687 of the table are garbled in PAPER.md: they are restated from the
+            // legible rows by crossing symmetry (reading R20) and all rows are pinned to the textbook
+            // 90-degree values (tests/golden/qcd_90deg.txt).
+            M2_QCD_Q1Q2 = 4,           // q1 q2 -> q1 q2 (also qbar1 q2, q1 qbar2, qbar1 qbar2)
+            M2_QCD_Q1Q1 = 5,           // q1 q1 -> q1 q1 (also qbar1 qbar1)
+            M2_QCD_Q1QB1 = 6,          // q1 qbar1 -> q1 qbar1
+            M2_QCD_Q1QB1_Q2QB2 = 7,    // q1 qbar1 -> q2 qbar2
+            M2_QCD_QQB_GG = 8,         // q1 qbar1 -> g g
+            M2_QCD_QG = 9,             // q1 g -> q1 g (also qbar1 g)
+            M2_QCD_GG = 10,            // g g -> g g
+            M2_KIND_LAST = 10 };
 
 // A role = one process seen from one grid species: particle 1 is the grid
 // particle, 2 its sampled partner, (3,4) the other pair.
@@ -85,7 +102,7 @@ enum Kind { M2_CONST = 0, M2_COULOMB_SCREENED = 1, M2_TCHAN_S2 = 2,
 // about the CM direction of particle 1 drawn from the t-channel shape 1/(t - mD^2)^2 by its inverse CDF
 // (steps S1..S7 below), azimuth uniform.  Both estimate the same integral (R).
 enum Sampler { SAMPLER_UNIFORM = 0, SAMPLER_TCHANNEL = 1 };
-struct Role { int s[4]; int kind; double par[4]; double sym; int process; int sampler; };
+struct Role { int s[4]; int kind; double par[4]; double sym; int process; int sampler; double gab; };
 
 typedef double (*FCallback)(int species, const double* p, void* user);
 
@@ -116,7 +133,7 @@ struct Handle {
 // Per-sample record for tests (oracle-only).
 struct Trace {
     double p1[3], p2[3], p3[3], p4[3];
-    double E1, E2, E3, s, t, pf, w, f1, f2, f3, f4, gain, loss;
+    double E1, E2, E3, s, t, pf, w, f1, f2, f3, f4, gain, loss, u;
     int j2, j3, j4;            // linear momentum cell, -1 = outside the box
     int status;                // 0 ok, 1 skipped at O4 (h<=0), 2 below threshold
     int draws;                 // Philox calls consumed (always 1)
@@ -210,6 +227,9 @@ template <typename R> struct RoleConst {
     int n[4][3];
     R theta_kappa[4];
     R par0, mD2, twomD2, g4, sig64;
+    R msqsum;                      // m1^2 + m2^2 + m3^2 + m4^2 (u = msqsum - s - t)
+    R qA, qB, qC, qD, qG;          // Table III group factors times g^4 (see Evaluator)
+    R cg, cl;                      // degrees-of-freedom factors of the gain and the loss direction (see Evaluator)
 };
 
 template <typename R> inline R dot3(const R* a, const R* b) {
@@ -257,6 +277,49 @@ struct Evaluator {
         const double g2 = role.par[0] * role.par[0];
         k.g4   = (R)(g2 * g2);
         k.sig64 = (R)(64.0 * M_PI * M_PI * role.par[0]);     // M2_ISO_DSIGMA: |M|^2 = sig64 * s
+        k.msqsum = (R)((m[0] * m[0] + m[1] * m[1]) + (m[2] * m[2] + m[3] * m[3]));
+        // Table III prefactors (d_F = C_A = 3, C_F = 4/3, d_A = 8), times g^4 = par0^4
+        const double dF = 3.0, CA = 3.0, CF = 4.0 / 3.0, dA = 8.0, g4d = g2 * g2;
+        k.qA = (R)(8.0 * g4d * dF * dF * CF * CF / dA);          // 8 g^4 dF^2 CF^2 / dA
+        k.qB = (R)(16.0 * g4d * dF * CF * (CF - CA / 2.0));      // 16 g^4 dF CF (CF - CA/2)
+        k.qC = (R)(8.0 * g4d * dF * CF * CF);                    // 8 g^4 dF CF^2
+        k.qD = (R)(8.0 * g4d * dF * CF * CA);                    // 8 g^4 dF CF CA
+        k.qG = (R)(16.0 * g4d * dA * CA * CA);                   // 16 g^4 dA CA^2
+        // Degrees of freedom ("an average over the DOF in the initial state and a sum over the DOF
+        // in the final state are implied in M_{ab<->cd}, and a sum over the DOF of the distribution function is
+        // also implied"; reading R21).  With |M|^2_sum the matrix element summed over the DOF of all
+        // four particles, the loss direction 1+2 -> 3+4 carries |M|^2_sum / (g1 g2) and the gain direction
+        // 3+4 -> 1+2 carries |M|^2_sum / (g3 g4).  Table III kinds ARE |M|^2_sum; kinds 0..3
+        // give |M|^2 of the process as written, a+b -> c+d, averaged over g_a g_b, i.e. |M|^2_sum = |M|^2 g_a g_b.
+        // For an elastic role of kinds 0..3 both factors are exactly 1.
+        {
+            const Process_dof d = dof_of(H, role);
+            k.cl = (R)(d.sum_norm / (d.g[0] * d.g[1]));
+            k.cg = (R)(d.sum_norm / (d.g[2] * d.g[3]));
+        }
+    }
+
+    struct Process_dof { double g[4]; double sum_norm; };
+    static Process_dof dof_of(const Handle& h, const Role& r) {
+        Process_dof d;
+        for (int i = 0; i < 4; ++i) d.g[i] = h.sp[r.s[i]].g;
+        d.sum_norm = r.kind >= M2_QCD_Q1Q2 ? 1.0 : r.gab;      // gab = g_a g_b of the process as written
+        return d;
+    }
+
+    // O9 for the Table III kinds: |M|^2(s,t,u) with T = t - m_g^2, U = u - m_g^2.
+    inline R m2_qcd(R s, R t, R u) const {
+        const R T = t - k.mD2, U = u - k.mD2;
+        const R s2 = s * s, t2 = t * t, u2 = u * u;
+        switch (role.kind) {
+            case M2_QCD_Q1Q2:        return k.qA * ((s2 + u2) / (T * T));
+            case M2_QCD_Q1Q1:        return k.qA * ((s2 + u2) / (T * T) + (s2 + t2) / (U * U)) + k.qB * (s2 / (T * U));
+            case M2_QCD_Q1QB1:       return k.qA * ((s2 + u2) / (T * T) + (u2 + t2) / s2) + k.qB * (u2 / (T * s));
+            case M2_QCD_Q1QB1_Q2QB2: return k.qA * ((t2 + u2) / s2);
+            case M2_QCD_QQB_GG:      return k.qC * (u / T + t / U) - k.qD * ((t2 + u2) / s2);
+            case M2_QCD_QG:          return k.qD * ((s2 + u2) / (T * T)) - k.qC * (u / s + s / U);
+            default:                 return k.qG * ((((R)3 - (s * u) / (T * T)) - (s * t) / (U * U)) - (t * u) / s2);
+        }
     }
 
     // O10.  Nearest-cell gather: tau_d = fma(p_d, invDelta_d, -pmin_d*invDelta_d); inside iff
@@ -320,7 +383,7 @@ struct Evaluator {
             // the low bytes of words 0..2 make the 24-bit azimuth index, word 3 gives cos(theta)
             const uint32_t k24 = ((r0.v[0] & 255u) << 16) | ((r0.v[1] & 255u) << 8) | (r0.v[2] & 255u);
             int status = 0, draws = 1;
-            R E2 = 0, s = 0, t = 0, pf = 0, w = 0, E3 = 0, f2 = 0, f3 = 0, f4 = 0, gain = 0, loss = 0;
+            R E2 = 0, s = 0, t = 0, u = 0, pf = 0, w = 0, E3 = 0, f2 = 0, f3 = 0, f4 = 0, gain = 0, loss = 0;
             R p3[3] = {0, 0, 0}, p4[3] = {0, 0, 0};
             int j3 = -1, j4 = -1;
             do {
@@ -415,10 +478,15 @@ struct Evaluator {
                     const R dl2 = dot3<R>(dl, dl);
                     const R dE = E1 - E3;
                     t = rfma<R>(dE, dE, -dl2);
-                    const R D = t - k.mD2;
-                    const R den = (D * D) * ers;
-                    if (role.kind == M2_COULOMB_SCREENED) w = (k.par0 * pf) / den;
-                    else                                  w = ((k.g4 * (s * s)) * pf) / den;
+                    if (role.kind >= M2_QCD_Q1Q2) {
+                        u = (k.msqsum - s) - t;                 // s + t + u = sum of the squared masses
+                        w = (m2_qcd(s, t, u) * pf) / ers;
+                    } else {
+                        const R D = t - k.mD2;
+                        const R den = (D * D) * ers;
+                        if (role.kind == M2_COULOMB_SCREENED) w = (k.par0 * pf) / den;
+                        else                                  w = ((k.g4 * (s * s)) * pf) / den;
+                    }
                 }
                 // ---- O10: gathers ------------------------------------------------------------
                 j3 = cell_of(2, p3); j4 = cell_of(3, p4);
@@ -427,8 +495,8 @@ struct Evaluator {
                 const R F2 = rfma<R>(k.theta_kappa[1], f2, (R)1);
                 const R F3 = rfma<R>(k.theta_kappa[2], f3, (R)1);
                 const R F4 = rfma<R>(k.theta_kappa[3], f4, (R)1);
-                gain = (f3 * f4) * (F1 * F2);
-                loss = (f1 * f2) * (F3 * F4);
+                gain = k.cg * ((f3 * f4) * (F1 * F2));
+                loss = k.cl * ((f1 * f2) * (F3 * F4));
                 // ---- O12: accumulate in double ---------------------------------------------
                 const double wg = (double)(w * gain), wl = (double)(w * loss);
                 acc.G += wg; acc.Ls += wl;
@@ -441,7 +509,7 @@ struct Evaluator {
             if (want) {
                 for (int d = 0; d < 3; ++d) { tr.p1[d] = p1[d]; tr.p2[d] = p2[d]; tr.p3[d] = p3[d]; tr.p4[d] = p4[d]; }
                 tr.E1 = E1; tr.E2 = E2; tr.E3 = E3; tr.s = s; tr.t = t; tr.pf = pf; tr.w = w;
-                tr.f1 = f1; tr.f2 = f2; tr.f3 = f3; tr.f4 = f4; tr.gain = gain; tr.loss = loss;
+                tr.f1 = f1; tr.f2 = f2; tr.f3 = f3; tr.f4 = f4; tr.gain = gain; tr.loss = loss; tr.u = u;
                 tr.j2 = j2; tr.j3 = j3; tr.j4 = j4; tr.status = status; tr.draws = draws;
                 *trace = tr;
             }
@@ -530,27 +598,40 @@ void* orc_create(int nx, int n_species, const Species* sp, const Grid* grid, int
         H->np.push_back(np);
         off += (size_t)nx * np;
     }
-    // Role expansion (Eq. 19): process a+b->c+d contributes to C of every
-    // distinct external species when that species is placed on the grid leg.  By the symmetry of
-    // |M|^2 under crossing the labels of a 2->2 process we treat:
-    //   grid particle = a : role (a,b,c,d)      grid particle = b : role (b,a,d,c)   (if b != a)
-    // For the elastic processes (c==a, d==b) these are the gain/loss pair of Eq. 16 with the
-    // forward and reverse reaction being the same process.  sym: <0 => paper rule (0.5 iff a==b).
+    // Role expansion (Eq. 16 and Eq. 19).  A role (1,2,3,4) is Eq. 16 with the grid
+    // particle d(p) = 1, its partner c(k3) = 2 and the incident pair a(k1), b(k2) = 3, 4: gain f3 f4 F1 F2 from
+    // 3+4 -> 1+2, loss f1 f2 F3 F4 from the reverse reaction, both with the same |M|^2 (M_{ab<->cd}).
+    // A process written a+b -> c+d therefore contributes
+    //   to C_a: role (a,b,c,d)      to C_b: role (b,a,d,c)   (if b != a)
+    // and, when it is inelastic ({c,d} != {a,b}), also
+    //   to C_c: role (c,d,a,b)      to C_d: role (d,c,b,a)   (if d != c);
+    // for an elastic process (c == a, d == b) the second pair would repeat the first.  These permutations keep
+    // t = (p1-p3)^2 and u = (p1-p4)^2 equal to the t and u of the process as written.
+    // Symmetry factor ("1/2 ... when all incident particles are of the same type"): the incident
+    // pair of a role is (3,4), so sym = 1/2 iff species 3 == species 4, else 1; sym >= 0 in the process
+    // overrides it for every role of that process.
     size_t roff = 0;
     for (int i = 0; i < n_process; ++i) {
         const Process& p = pr[i];
-        if (p.c != p.a || p.d != p.b) { delete H; return nullptr; }   // elastic roles only (R15)
-        if (p.kind < M2_CONST || p.kind > M2_ISO_DSIGMA) { delete H; return nullptr; }
+        const bool elastic = p.c == p.a && p.d == p.b;
+        const bool same_sets = (p.c == p.a && p.d == p.b) || (p.c == p.b && p.d == p.a);
+        if (!elastic && same_sets) { delete H; return nullptr; }      // write a+b -> b+a as a+b -> a+b
+        if (p.kind < M2_CONST || p.kind > M2_KIND_LAST) { delete H; return nullptr; }
         if (p.sampler != SAMPLER_UNIFORM && p.sampler != SAMPLER_TCHANNEL) { delete H; return nullptr; }
-        // the t-channel sampler needs a t-channel kind with a non-zero regulator
-        if (p.sampler == SAMPLER_TCHANNEL && !((p.kind == M2_COULOMB_SCREENED || p.kind == M2_TCHAN_S2) && p.par[1] != 0.0)) { delete H; return nullptr; }
-        const double sym = p.sym < 0 ? (p.a == p.b ? 0.5 : 1.0) : p.sym;
-        Role r; r.kind = p.kind; std::memcpy(r.par, p.par, sizeof r.par); r.sym = sym; r.process = i; r.sampler = p.sampler;
-        r.s[0] = p.a; r.s[1] = p.b; r.s[2] = p.c; r.s[3] = p.d;
-        H->roles.push_back(r); H->role_off.push_back(roff); roff += (size_t)nx * H->np[p.a];
-        if (p.b != p.a) {
-            r.s[0] = p.b; r.s[1] = p.a; r.s[2] = p.d; r.s[3] = p.c;
-            H->roles.push_back(r); H->role_off.push_back(roff); roff += (size_t)nx * H->np[p.b];
+        // the t-channel sampler needs an elastic process of a t-channel kind with a non-zero regulator
+        if (p.sampler == SAMPLER_TCHANNEL && !(elastic && (p.kind == M2_COULOMB_SCREENED || p.kind == M2_TCHAN_S2) && p.par[1] != 0.0)) { delete H; return nullptr; }
+        Role r; r.kind = p.kind; std::memcpy(r.par, p.par, sizeof r.par); r.process = i; r.sampler = p.sampler;
+        r.gab = sp[p.a].g * sp[p.b].g;
+        auto add = [&](int s1, int s2, int s3, int s4) {
+            r.s[0] = s1; r.s[1] = s2; r.s[2] = s3; r.s[3] = s4;
+            r.sym = p.sym < 0 ? (s3 == s4 ? 0.5 : 1.0) : p.sym;
+            H->roles.push_back(r); H->role_off.push_back(roff); roff += (size_t)nx * H->np[s1];
+        };
+        add(p.a, p.b, p.c, p.d);
+        if (p.b != p.a) add(p.b, p.a, p.d, p.c);
+        if (!elastic) {
+            add(p.c, p.d, p.a, p.b);
+            if (p.d != p.c) add(p.d, p.c, p.b, p.a);
         }
     }
     H->role_off.push_back(roff);
@@ -603,16 +684,24 @@ int orc_collision_point(void* h, const double* f, int role, int ix, int ip1, int
     return 0;
 }
 
-// Kinematics of sample n of (role, ix, ip1): 27 doubles + 5 ints, see struct Trace.
+// Kinematics of sample n of (role, ix, ip1): 26 doubles + 5 ints, see struct Trace.
 int orc_trace(void* h, const double* f, int role, int ix, int ip1, int n, uint64_t seed, double* dout, int* iout,
               FCallback fcb, void* user, int box_cut) {
     Handle* H = (Handle*)h;
     Trace tr; Accum acc;
     if (H->use_float) { Evaluator<float> ev(*H, role, fcb, user, box_cut); ev.eval_p1(f, ix, ip1, n + 1, seed, acc, &tr, n); }
     else { Evaluator<double> ev(*H, role, fcb, user, box_cut); ev.eval_p1(f, ix, ip1, n + 1, seed, acc, &tr, n); }
-    std::memcpy(dout, &tr, 25 * sizeof(double));
+    std::memcpy(dout, &tr, 26 * sizeof(double));
     iout[0] = tr.j2; iout[1] = tr.j3; iout[2] = tr.j4; iout[3] = tr.status; iout[4] = tr.draws;
     return 0;
+}
+
+// |M|^2(s,t,u) of a Table III role exactly as the sample loop evaluates it (pins: tests/test_oracle_qcd.py).
+double orc_m2_qcd(void* h, int role, double s, double t, double u) {
+    Handle* H = (Handle*)h;
+    if (role < 0 || role >= (int)H->roles.size() || H->roles[role].kind < M2_QCD_Q1Q2) return std::numeric_limits<double>::quiet_NaN();
+    Evaluator<double> ev(*H, role, nullptr, nullptr, 1);
+    return ev.m2_qcd(s, t, u);
 }
 
 // O-update (Eq. 27; positivity PAPER.md:263): f_out = f + dt*C, count f_out < 0.

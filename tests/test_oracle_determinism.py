@@ -58,7 +58,9 @@ def test_roles_and_symmetry_factor():
     # a+b and b+a views of one process are consecutive, "a-side" first
     assert [r["s"][:2] for r in o.roles[4:6]] == [(0, 1), (1, 0)]
     with pytest.raises(ValueError):
-        bad = dict(w["problem"], processes=[dict(a=0, b=1, c=1, d=2, kind=0, par=[1.0], sym=-1.0)])
+        # a + b -> b + a must be written a + b -> a + b (inelastic processes are accepted since NEXT-2(ii):
+        # Eq. 16 is general, tests/test_oracle_qcd.py)
+        bad = dict(w["problem"], processes=[dict(a=0, b=1, c=1, d=0, kind=0, par=[1.0], sym=-1.0)])
         oracle.Oracle(bad)
 
 
