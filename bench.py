@@ -31,7 +31,10 @@ METRIC, UNIT = "collision_samples_per_s", "samples/s"
 
 # Algorithmic FP64 work per sample of chain O1-O12 (FMA = 2 flops, every other
 # add/mul/compare/sqrt/divide = 1), by |M|^2 kind, classical statistics (+12 with quantum factors).
-FLOPS_PER_SAMPLE = {0: 141.0, 1: 155.0, 2: 157.0, 3: 142.0}
+FLOPS_PER_SAMPLE = {0: 141.0, 1: 155.0, 2: 157.0, 3: 142.0,
+                    # Table III kinds: 138 (O2-O7, O10-O12) + t 11 + u 2 + T, U 2 + squares 3 + weight 3 + the row's
+                    # rational function (5 / 14 / 14 / 5 / 12 / 12 / 16; a reciprocal = 1)
+                    4: 164.0, 5: 173.0, 6: 173.0, 7: 164.0, 8: 171.0, 9: 171.0, 10: 175.0}
 QUANTUM_EXTRA_FLOPS = 10.0
 # the same count for the t-channel importance sampler (steps S1-S7), kinds 1 and 2
 FLOPS_PER_SAMPLE_TCHANNEL = {1: 185.0, 2: 187.0}
@@ -43,12 +46,11 @@ NCU_TRAFFIC_BYTES_PER_LAUNCH = {2: 35.02e6}
 
 def flops_per_sweep(problem, n_samples):
     tot = 0.0
-    for p in problem["processes"]:
-        q = any(problem["species"][s]["stat"] != 0 for s in (p["a"], p["b"]))
+    for r, p in zip(wl.roles(problem), wl.role_processes(problem)):
+        q = any(problem["species"][s]["stat"] != 0 for s in r)
         table = FLOPS_PER_SAMPLE_TCHANNEL if p.get("sampler", 0) == 1 else FLOPS_PER_SAMPLE
         per = table[p["kind"]] + (QUANTUM_EXTRA_FLOPS if q else 0.0)
-        for s in ([p["a"]] if p["a"] == p["b"] else [p["a"], p["b"]]):
-            tot += per * problem["nx"] * int(np.prod(problem["grids"][s]["n"])) * n_samples
+        tot += per * problem["nx"] * int(np.prod(problem["grids"][r[0]]["n"])) * n_samples
     return tot
 
 
@@ -144,7 +146,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5); 2 = configs[1]")
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5); 2 = configs[1]; 6, 7 = the paper's own workloads")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-cells", type=int, default=6, help="spatial cells per step of the reference arm")
     ap.add_argument("--cpu-cells", type=int, default=48, help="spatial cells of the cpu_baseline leg")

@@ -71,11 +71,23 @@ typedef enum {
     RBG_M2_COULOMB_SCREENED = 1,  /* |M|^2 = par[0] / (t - par[1]^2)^2                */
     RBG_M2_TCHAN_S2         = 2,  /* |M|^2 = par[0]^4 s^2 / (t - par[1]^2)^2   (Table III t-channel
                                      form with regulator)          */
-    RBG_M2_ISO_DSIGMA       = 3   /* |M|^2 = 64 pi^2 s par[0]: a constant differential cross section
+    RBG_M2_ISO_DSIGMA       = 3,  /* |M|^2 = 64 pi^2 s par[0]: a constant differential cross section
                                      dsigma/dOmega = par[0], isotropic in the CM frame -- how the paper's
                                      collision test quotes its processes (Eq. 48, PAPER.md:493-500;
                                      cross section <-> matrix element Eq. 20-22, PAPER.md:214-230;
                                      DESIGN.md reading R17)                           */
+    /* Table III of the paper: |M|^2 of the 2->2 parton processes of QCD, summed over the helicities
+     * and colours of all four particles; par[0] = g, par[1] = m_g (the regulator m_g^2 is subtracted from t and u in
+     * the denominators); SU_c(3): d_F = C_A = 3, C_F = 4/3, d_A = 8.  t = (k1 - k3)^2, u = (k1 - p)^2 of the process as
+     * written a(k1) + b(k2) -> c(k3) + d(p).  With A = 8 g^4 d_F^2 C_F^2 / d_A, B = 16 g^4 d_F C_F (C_F - C_A/2),
+     * C = 8 g^4 d_F C_F^2, D = 8 g^4 d_F C_F C_A, T = t - m_g^2, U = u - m_g^2:                                        */
+    RBG_M2_QCD_Q1Q2         = 4,  /* q1 q2 -> q1 q2 (any mix of q, qbar of two flavours): A (s^2+u^2)/T^2                */
+    RBG_M2_QCD_Q1Q1         = 5,  /* q1 q1 -> q1 q1: A [(s^2+u^2)/T^2 + (s^2+t^2)/U^2] + B s^2/(T U)                      */
+    RBG_M2_QCD_Q1QB1        = 6,  /* q1 qbar1 -> q1 qbar1: A [(s^2+u^2)/T^2 + (u^2+t^2)/s^2] + B u^2/(T s)                */
+    RBG_M2_QCD_Q1QB1_Q2QB2  = 7,  /* q1 qbar1 -> q2 qbar2: A (t^2+u^2)/s^2                                               */
+    RBG_M2_QCD_QQB_GG       = 8,  /* q1 qbar1 -> g g: C (u/T + t/U) - D (t^2+u^2)/s^2                                     */
+    RBG_M2_QCD_QG           = 9,  /* q1 g -> q1 g: D (s^2+u^2)/T^2 - C (u/s + s/U)                                        */
+    RBG_M2_QCD_GG           = 10  /* g g -> g g: 16 g^4 d_A C_A^2 (3 - s u/T^2 - s t/U^2 - t u/s^2)                       */
 } rbg_m2_kind;
 
 /* How the CM scattering direction of a process is drawn (both estimate the same integral):
@@ -83,20 +95,29 @@ typedef enum {
  *   RBG_SAMPLER_TCHANNEL  polar angle about the CM direction of the grid particle drawn from the shape
  *                         1/(t - par[1]^2)^2 of the screened t-channel kinds by its inverse CDF, azimuth
  *                         uniform; the angular factor of |M|^2 then cancels in the weight (DESIGN.md
- *                         section 4b).  Only with RBG_M2_COULOMB_SCREENED / RBG_M2_TCHAN_S2 and par[1] != 0;
+ *                         section 4b).  Only for elastic processes of RBG_M2_COULOMB_SCREENED / RBG_M2_TCHAN_S2 with par[1] != 0;
  *                         removes the (p* / par[1])^2-sized variance of sampling a forward peak uniformly. */
 #define RBG_SAMPLER_UNIFORM  0
 #define RBG_SAMPLER_TCHANNEL 1
 
-/* Process a + b -> c + d (species indices).  Only elastic processes (c == a, d == b) are
- * implemented; anything else is RBG_E_UNSUPPORTED.  sym < 0 selects the paper's rule
- * (PAPER.md:208): 1/2 if a == b, else 1. */
+/* Process a + b -> c + d (species indices), Eq. 16.  It contributes to the collision term of every
+ * external species ("roles"): seen from a and from b, and, when it is inelastic ({c,d} != {a,b}),
+ * through the reverse reaction (same |M|^2, "M_{ab<->cd}") also from c and from d.  An elastic process is written
+ * c == a, d == b (a + b -> b + a is refused: t and u would be ambiguous).
+ * sym < 0 selects the paper's rule ("1/2 ... when all incident particles are of the same type"): per
+ * role, 1/2 if the two particles of the pair opposite the grid particle's pair are of one species, else 1; for an
+ * elastic process that is 1/2 iff a == b.  sym >= 0 is used for every role of the process.
+ * Degrees of freedom (reading R21): f is summed over the g internal states of its species.
+ * Kinds 0..3 give |M|^2 of a + b -> c + d averaged over the states of a and b and summed over those of c and d; the
+ * reverse direction is rescaled by g_a g_b / (g_c g_d).  The Table III kinds are summed over all four.  For elastic
+ * processes of kinds 0..3 no factor appears. */
 typedef struct { int a, b, c, d; int kind; double par[4]; double sym; int sampler; } rbg_process;
 
 /* Create a handle.  Returns RBG_OK and stores the handle in *out, or a negative code (then *out
  * is NULL and rbg_last_error(NULL) has the text).  Rejects: non-positive grid counts,
  * pmax <= pmin, negative mass, stat not in {0,+1,-1}, g <= 0, species index out of range,
- * unknown kind, sampler or flags, a sampler that does not fit the kind, inelastic processes, no CUDA device. */
+ * unknown kind, sampler or flags, a sampler that does not fit the kind or an inelastic process, a process
+ * written a + b -> b + a, no CUDA device. */
 int rbg_create(rbg_handle** out, const rbg_spatial_grid* grid, int n_species, const rbg_species* species,
                const rbg_momentum_grid* momentum_grids /* [n_species] */, int n_process,
                const rbg_process* processes, double hbar, int flags);

@@ -7,6 +7,9 @@ from pathlib import Path
 import numpy as np
 
 KIND_CONST, KIND_COULOMB_SCREENED, KIND_TCHAN_S2, KIND_ISO_DSIGMA = 0, 1, 2, 3
+# Table III
+(KIND_QCD_Q1Q2, KIND_QCD_Q1Q1, KIND_QCD_Q1QB1, KIND_QCD_Q1QB1_Q2QB2, KIND_QCD_QQB_GG, KIND_QCD_QG,
+ KIND_QCD_GG) = 4, 5, 6, 7, 8, 9, 10
 RBG_FP64, RBG_FP32_KINEMATICS = 0, 1
 SAMPLER_UNIFORM, SAMPLER_TCHANNEL = 0, 1
 

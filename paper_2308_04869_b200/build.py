@@ -18,7 +18,7 @@ SOURCES = [PKG / "csrc" / "rbg.cu"]
 DEPS = SOURCES + [PKG / "csrc" / "rbg_kernels.cuh", ROOT / "include" / "rbg.h"]
 LIB = PKG / "librbg.so"
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-fmad=false",
-              "-Xcompiler", "-fPIC,-ffp-contract=off,-O2", "-shared", "--ptxas-options=-v"]
+              "-Xcompiler", "-fPIC,-ffp-contract=off,-O2", "-shared", "--ptxas-options=-v", "-split-compile=0"]
 
 
 def _digest() -> str:

@@ -19,12 +19,14 @@ namespace {
 thread_local std::string g_create_error;
 
 struct Role {
-    int s1, s2;            // grid species, partner species (elastic: s3 = s1, s4 = s2)
+    int s[4];              // species of the grid particle 1, its partner 2 and the incident pair 3, 4
     int kind;
     double par[4];
     double sym;
     int index;             // global role index
     int sampler;           // RBG_SAMPLER_*
+    double cl, cg;         // degrees-of-freedom factors of the loss and the gain direction (reading R21)
+    bool elastic;          // s3 == s1 && s4 == s2
 };
 
 }  // namespace
@@ -71,9 +73,8 @@ template <typename R>
 rbg::RoleParams<R> make_role_params(const rbg_handle& H, const Role& r) {
     rbg::RoleParams<R> k;
     std::memset(&k, 0, sizeof k);
-    const int sl[4] = {r.s1, r.s2, r.s1, r.s2};
     double m[4];
-    for (int i = 0; i < 4; ++i) m[i] = H.species[sl[i]].mass;
+    for (int i = 0; i < 4; ++i) m[i] = H.species[r.s[i]].mass;
     const double msum = m[0] + m[1], m34 = m[2] + m[3], md = m[2] - m[3];
     k.m1 = (R)m[0]; k.m2 = (R)m[1];
     k.msq1 = (R)(m[0] * m[0]); k.msq2 = (R)(m[1] * m[1]);
@@ -82,43 +83,50 @@ rbg::RoleParams<R> make_role_params(const rbg_handle& H, const Role& r) {
     k.Mth = (R)(msum * msum - m34 * m34);
     k.Mdf = (R)(md * md);
     k.dm34 = (R)(m[2] * m[2] - m[3] * m[3]);
-    const rbg_momentum_grid& g1 = H.grids[r.s1];
-    const rbg_momentum_grid& g2 = H.grids[r.s2];
-    double V2 = 1.0;
+    k.msqsum = (R)((m[0] * m[0] + m[1] * m[1]) + (m[2] * m[2] + m[3] * m[3]));
+    const rbg_momentum_grid& g1 = H.grids[r.s[0]];
+    const rbg_momentum_grid& g2 = H.grids[r.s[1]];
+    const rbg_momentum_grid& g3 = H.grids[r.s[2]];
+    const rbg_momentum_grid& g4 = H.grids[r.s[3]];
     for (int d = 0; d < 3; ++d) {
         const double L1 = g1.pmax[d] - g1.pmin[d], L2 = g2.pmax[d] - g2.pmin[d];
-        const double invD1 = (double)g1.n[d] / L1, invD2 = (double)g2.n[d] / L2;
+        const double invD3 = (double)g3.n[d] / (g3.pmax[d] - g3.pmin[d]), invD4 = (double)g4.n[d] / (g4.pmax[d] - g4.pmin[d]);
         k.pmin1[d] = (R)g1.pmin[d];
         k.delta1[d] = (R)(L1 / (double)g1.n[d]);
         k.pmin2[d] = (R)g2.pmin[d];
         k.L2[d] = (R)L2;
-        k.invD3[d] = (R)invD1; k.off3[d] = (R)(-g1.pmin[d] * invD1);
-        k.invD4[d] = (R)invD2; k.off4[d] = (R)(-g2.pmin[d] * invD2);
-        k.n1[d] = k.n3[d] = g1.n[d];
-        k.n2[d] = k.n4[d] = g2.n[d];
+        k.invD3[d] = (R)invD3; k.off3[d] = (R)(-g3.pmin[d] * invD3);
+        k.invD4[d] = (R)invD4; k.off4[d] = (R)(-g4.pmin[d] * invD4);
+        k.n1[d] = g1.n[d]; k.n2[d] = g2.n[d]; k.n3[d] = g3.n[d]; k.n4[d] = g4.n[d];
     }
-    V2 = (g2.pmax[0] - g2.pmin[0]) * (g2.pmax[1] - g2.pmin[1]) * (g2.pmax[2] - g2.pmin[2]);
+    const double V2 = (g2.pmax[0] - g2.pmin[0]) * (g2.pmax[1] - g2.pmin[1]) * (g2.pmax[2] - g2.pmin[2]);
     const double tph = 2.0 * M_PI * H.hbar;
-    const double tk1 = (double)H.species[r.s1].stat * (tph * tph * tph) / H.species[r.s1].g;
-    const double tk2 = (double)H.species[r.s2].stat * (tph * tph * tph) / H.species[r.s2].g;
-    k.tk1 = k.tk3 = (R)tk1;
-    k.tk2 = k.tk4 = (R)tk2;
+    R* tk[4] = {&k.tk1, &k.tk2, &k.tk3, &k.tk4};
+    for (int i = 0; i < 4; ++i) *tk[i] = (R)((double)H.species[r.s[i]].stat * (tph * tph * tph) / H.species[r.s[i]].g);
     k.par0 = (R)(r.kind == RBG_M2_ISO_DSIGMA ? 64.0 * M_PI * M_PI * r.par[0] : r.par[0]);
     k.mD2 = (R)(r.par[1] * r.par[1]);
     k.twomD2 = (R)(2.0 * (r.par[1] * r.par[1]));
     const double g2c = r.par[0] * r.par[0];
     k.g4 = (R)(g2c * g2c);
-    k.symV2 = r.sym * V2;
-    k.np1 = (int)H.np[r.s1]; k.np2 = (int)H.np[r.s2]; k.np3 = k.np1;
+    // Table III prefactors (d_F = C_A = 3, C_F = 4/3, d_A = 8), times g^4 = par0^4
+    const double dF = 3.0, CA = 3.0, CF = 4.0 / 3.0, dA = 8.0, g4d = g2c * g2c;
+    k.qA = (R)(8.0 * g4d * dF * dF * CF * CF / dA);
+    k.qB = (R)(16.0 * g4d * dF * CF * (CF - CA / 2.0));
+    k.qC = (R)(8.0 * g4d * dF * CF * CF);
+    k.qD = (R)(8.0 * g4d * dF * CF * CA);
+    k.qG = (R)(16.0 * g4d * dA * CA * CA);
+    k.qcd = r.kind >= RBG_M2_QCD_Q1Q2 ? r.kind - RBG_M2_QCD_Q1Q2 : 0;
+    k.rho = (R)(r.cg / r.cl);
+    k.symV2 = r.sym * V2 * r.cl;
+    for (int i = 0; i < 4; ++i) k.np[i] = (int)H.np[r.s[i]];
     k.role = r.index;
-    k.same_species = r.s1 == r.s2;
     return k;
 }
 
-template <typename R, int KIND, bool Q, bool SMEM, int MAXT, int SPL, bool TCH>
+template <typename R, int KIND, bool Q, bool SMEM, int MAXT, int SPL, bool TCH, bool INEL>
 cudaError_t launch_one(const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp, int grid, int threads, size_t smem,
                        cudaStream_t st) {
-    auto kern = rbg::collision_role_kernel<R, KIND, Q, SMEM, MAXT, SPL, TCH>;
+    auto kern = rbg::collision_role_kernel<R, KIND, Q, SMEM, MAXT, SPL, TCH, INEL>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kern<<<grid, threads, smem, st>>>(rp, lp);
@@ -130,14 +138,21 @@ cudaError_t launch_one(const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp
 template <typename R, int KIND, bool Q, bool SMEM, bool TCH>
 cudaError_t launch_geo(int spl, const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp, int grid, int threads,
                        size_t smem, cudaStream_t st) {
-    if (threads > 512) return launch_one<R, KIND, Q, SMEM, 1024, 1, TCH>(rp, lp, grid, threads, smem, st);
-    if (spl == 2) return launch_one<R, KIND, Q, SMEM, 512, 2, TCH>(rp, lp, grid, threads, smem, st);
-    return launch_one<R, KIND, Q, SMEM, 512, 1, TCH>(rp, lp, grid, threads, smem, st);
+    if (threads > 512) return launch_one<R, KIND, Q, SMEM, 1024, 1, TCH, false>(rp, lp, grid, threads, smem, st);
+    if (spl == 2) return launch_one<R, KIND, Q, SMEM, 512, 2, TCH, false>(rp, lp, grid, threads, smem, st);
+    return launch_one<R, KIND, Q, SMEM, 512, 1, TCH, false>(rp, lp, grid, threads, smem, st);
 }
 
+// inel: general roles (species 3,4 differ from 1,2) run one geometry (up to 16 warps, 2 samples per lane), uniform sampler
 template <typename R, int KIND, bool TCH>
-cudaError_t launch_kq(bool q, bool smem_path, int spl, const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp, int grid,
-                      int threads, size_t smem, cudaStream_t st) {
+cudaError_t launch_kq(bool q, bool smem_path, bool inel, int spl, const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp,
+                      int grid, int threads, size_t smem, cudaStream_t st) {
+    if (inel) {
+        if (q) return smem_path ? launch_one<R, KIND, true, true, 512, 2, false, true>(rp, lp, grid, threads, smem, st)
+                                : launch_one<R, KIND, true, false, 512, 2, false, true>(rp, lp, grid, threads, smem, st);
+        return smem_path ? launch_one<R, KIND, false, true, 512, 2, false, true>(rp, lp, grid, threads, smem, st)
+                         : launch_one<R, KIND, false, false, 512, 2, false, true>(rp, lp, grid, threads, smem, st);
+    }
     if (q) return smem_path ? launch_geo<R, KIND, true, true, TCH>(spl, rp, lp, grid, threads, smem, st)
                             : launch_geo<R, KIND, true, false, TCH>(spl, rp, lp, grid, threads, smem, st);
     return smem_path ? launch_geo<R, KIND, false, true, TCH>(spl, rp, lp, grid, threads, smem, st)
@@ -151,8 +166,8 @@ int run_roles(rbg_handle* h, const double* f, double* out, bool update, double d
     // last role per species (update mode counts negatives there); species with no role: C = 0 / f_out = f
     std::vector<int> first_role(h->n_species, -1), last_role(h->n_species, -1);
     for (size_t i = 0; i < h->roles.size(); ++i) {
-        if (first_role[h->roles[i].s1] < 0) first_role[h->roles[i].s1] = (int)i;
-        last_role[h->roles[i].s1] = (int)i;
+        if (first_role[h->roles[i].s[0]] < 0) first_role[h->roles[i].s[0]] = (int)i;
+        last_role[h->roles[i].s[0]] = (int)i;
     }
     for (int s = 0; s < h->n_species; ++s) {
         if (first_role[s] >= 0) continue;
@@ -165,54 +180,67 @@ int run_roles(rbg_handle* h, const double* f, double* out, bool update, double d
             RBG_CUDA(h, cudaMemsetAsync(out + h->sp_off[s], 0, n * sizeof(double), st));
         }
     }
-    for (size_t i = 0; i < h->roles.size(); ++i) {
-        const Role& r = h->roles[i];
+    for (size_t ir = 0; ir < h->roles.size(); ++ir) {
+        const Role& r = h->roles[ir];
         const rbg::RoleParams<R> rp = make_role_params<R>(*h, r);
-        const int warps = h->opt_warps > 0 ? h->opt_warps : 16;
+        const bool inel = !r.elastic;
+        int warps = h->opt_warps > 0 ? h->opt_warps : 16;
+        if (inel && warps > 16) warps = 16;
         const int spl = h->opt_spl > 0 ? h->opt_spl : 2;
-        long work = (long)h->nx * rp.np1;
+        const int np1 = rp.np[0];
+        long work = (long)h->nx * np1;
         int T = h->opt_p1_per_cta > 0 ? h->opt_p1_per_cta : (int)std::min<long>(512, std::max<long>(warps, work / ((long)h->sm_count * 8)));
-        T = std::min(T, rp.np1);
-        // shared memory: [16 B mbarrier][T doubles][table2][table1 if species differ]
-        const size_t tab2 = (((size_t)rp.np2 + 3) & ~(size_t)3) * sizeof(R);
-        const size_t tab1 = rp.same_species ? 0 : (size_t)rp.np1 * sizeof(R);
-        const size_t head = 16 + (((size_t)T * 8 + 15) & ~(size_t)15);
-        bool smem_path = head + tab2 + tab1 <= (size_t)h->max_smem_optin;
-        if (h->opt_gather == 1 && !smem_path) return fail(h, RBG_E_UNSUPPORTED, "gather=1 (shared memory) requested but the f tables do not fit");
-        if (h->opt_gather == 2) smem_path = false;
-        const size_t smem = head + (smem_path ? tab2 + tab1 : 0);
+        T = std::min(T, np1);
+        // shared memory: [16 B mbarrier][T doubles][one f table per distinct species among slots 2, 3, 4, 16-B aligned]
         rbg::LaunchParams lp;
         std::memset(&lp, 0, sizeof lp);
-        lp.f1_base = f + h->sp_off[r.s1];
-        lp.f2_base = f + h->sp_off[r.s2];
-        lp.out_base = out + h->sp_off[r.s1];
+        const size_t head = 16 + (((size_t)T * 8 + 15) & ~(size_t)15);
+        size_t tabs = 0;
+        for (int i = 1; i < 4; ++i) {
+            int owner = i;
+            for (int j = 1; j < i; ++j) if (r.s[j] == r.s[i]) { owner = j; break; }
+            if (owner == i) {
+                lp.tab_own[i] = 1; lp.tab_off[i] = (int)tabs;
+                tabs += ((size_t)rp.np[i] * sizeof(R) + 15) & ~(size_t)15;
+            } else {
+                lp.tab_own[i] = 0; lp.tab_off[i] = lp.tab_off[owner];
+            }
+        }
+        bool smem_path = head + tabs <= (size_t)h->max_smem_optin;
+        if (h->opt_gather == 1 && !smem_path) return fail(h, RBG_E_UNSUPPORTED, "gather=1 (shared memory) requested but the f tables do not fit");
+        if (h->opt_gather == 2) smem_path = false;
+        const size_t smem = head + (smem_path ? tabs : 0);
+        for (int i = 0; i < 4; ++i) lp.fb[i] = f + h->sp_off[r.s[i]];
+        lp.out_base = out + h->sp_off[r.s[0]];
         lp.nx_local = h->nx; lp.ix_offset = h->ix_offset; lp.n_samples = n_samples;
         lp.key0 = (uint32_t)seed; lp.key1 = (uint32_t)(seed >> 32);
         for (int rr = 0; rr < 10; ++rr) {
             lp.rk[2 * rr] = lp.key0 + (uint32_t)rr * 0x9E3779B9u;
             lp.rk[2 * rr + 1] = lp.key1 + (uint32_t)rr * 0xBB67AE85u;
         }
-        lp.p1_per_cta = T; lp.tiles = (rp.np1 + T - 1) / T;
-        lp.accumulate = first_role[r.s1] != (int)i;
+        lp.p1_per_cta = T; lp.tiles = (np1 + T - 1) / T;
+        lp.accumulate = first_role[r.s[0]] != (int)ir;
         lp.update = update; lp.dt = dt; lp.neg_flag = neg_flag;
-        lp.count_negative = update && last_role[r.s1] == (int)i;
+        lp.count_negative = update && last_role[r.s[0]] == (int)ir;
         const long grid = (long)lp.tiles * h->nx;
         if (grid > 0x7fffffffL) return fail(h, RBG_E_UNSUPPORTED, "grid too large; raise p1_per_cta");
-        const bool q = h->species[r.s1].stat != 0 || h->species[r.s2].stat != 0;
+        bool q = false;
+        for (int i = 0; i < 4; ++i) q = q || h->species[r.s[i]].stat != 0;
         cudaError_t e;
         const bool tch = r.sampler == RBG_SAMPLER_TCHANNEL;
         const int th = warps * 32;
         switch (r.kind) {
-            case RBG_M2_CONST: e = launch_kq<R, rbg::KIND_CONST, false>(q, smem_path, spl, rp, lp, (int)grid, th, smem, st); break;
+            case RBG_M2_CONST: e = launch_kq<R, rbg::KIND_CONST, false>(q, smem_path, inel, spl, rp, lp, (int)grid, th, smem, st); break;
             case RBG_M2_COULOMB_SCREENED:
-                e = tch ? launch_kq<R, rbg::KIND_COULOMB, true>(q, smem_path, spl, rp, lp, (int)grid, th, smem, st)
-                        : launch_kq<R, rbg::KIND_COULOMB, false>(q, smem_path, spl, rp, lp, (int)grid, th, smem, st);
+                e = tch ? launch_kq<R, rbg::KIND_COULOMB, true>(q, smem_path, inel, spl, rp, lp, (int)grid, th, smem, st)
+                        : launch_kq<R, rbg::KIND_COULOMB, false>(q, smem_path, inel, spl, rp, lp, (int)grid, th, smem, st);
                 break;
             case RBG_M2_TCHAN_S2:
-                e = tch ? launch_kq<R, rbg::KIND_TCHAN_S2, true>(q, smem_path, spl, rp, lp, (int)grid, th, smem, st)
-                        : launch_kq<R, rbg::KIND_TCHAN_S2, false>(q, smem_path, spl, rp, lp, (int)grid, th, smem, st);
+                e = tch ? launch_kq<R, rbg::KIND_TCHAN_S2, true>(q, smem_path, inel, spl, rp, lp, (int)grid, th, smem, st)
+                        : launch_kq<R, rbg::KIND_TCHAN_S2, false>(q, smem_path, inel, spl, rp, lp, (int)grid, th, smem, st);
                 break;
-            default: e = launch_kq<R, rbg::KIND_ISO_DSIGMA, false>(q, smem_path, spl, rp, lp, (int)grid, th, smem, st); break;
+            case RBG_M2_ISO_DSIGMA: e = launch_kq<R, rbg::KIND_ISO_DSIGMA, false>(q, smem_path, inel, spl, rp, lp, (int)grid, th, smem, st); break;
+            default: e = launch_kq<R, rbg::KIND_QCD, false>(q, smem_path, inel, spl, rp, lp, (int)grid, th, smem, st); break;
         }
         if (e != cudaSuccess) return fail(h, RBG_E_CUDA, std::string("kernel launch: ") + cudaGetErrorString(e));
         ++h->last_launches;
@@ -281,20 +309,36 @@ int rbg_create(rbg_handle** out, const rbg_spatial_grid* grid, int n_species, co
         const int idx[4] = {p.a, p.b, p.c, p.d};
         for (int j = 0; j < 4; ++j)
             if (idx[j] < 0 || idx[j] >= n_species) { delete h; return fail(nullptr, RBG_E_INVALID_ARG, "process " + std::to_string(i) + ": species index out of range"); }
-        if (p.kind < RBG_M2_CONST || p.kind > RBG_M2_ISO_DSIGMA) { delete h; return fail(nullptr, RBG_E_INVALID_ARG, "process " + std::to_string(i) + ": unknown |M|^2 kind"); }
-        if (p.c != p.a || p.d != p.b) { delete h; return fail(nullptr, RBG_E_UNSUPPORTED, "process " + std::to_string(i) + ": only elastic processes (c==a, d==b) are implemented"); }
+        if (p.kind < RBG_M2_CONST || p.kind > RBG_M2_QCD_GG) { delete h; return fail(nullptr, RBG_E_INVALID_ARG, "process " + std::to_string(i) + ": unknown |M|^2 kind"); }
+        const bool elastic = p.c == p.a && p.d == p.b;
+        if (!elastic && p.c == p.b && p.d == p.a) { delete h; return fail(nullptr, RBG_E_INVALID_ARG, "process " + std::to_string(i) + ": write a+b -> b+a as a+b -> a+b (t and u would be ambiguous)"); }
         if (p.sampler != RBG_SAMPLER_UNIFORM && p.sampler != RBG_SAMPLER_TCHANNEL) { delete h; return fail(nullptr, RBG_E_INVALID_ARG, "process " + std::to_string(i) + ": unknown sampler"); }
-        if (p.sampler == RBG_SAMPLER_TCHANNEL && !((p.kind == RBG_M2_COULOMB_SCREENED || p.kind == RBG_M2_TCHAN_S2) && p.par[1] != 0.0)) {
+        if (p.sampler == RBG_SAMPLER_TCHANNEL && !(elastic && (p.kind == RBG_M2_COULOMB_SCREENED || p.kind == RBG_M2_TCHAN_S2) && p.par[1] != 0.0)) {
             delete h;
-            return fail(nullptr, RBG_E_INVALID_ARG, "process " + std::to_string(i) + ": the t-channel sampler needs a t-channel |M|^2 kind with a non-zero regulator par[1]");
+            return fail(nullptr, RBG_E_INVALID_ARG, "process " + std::to_string(i) + ": the t-channel sampler needs an elastic process of a t-channel |M|^2 kind with a non-zero regulator par[1]");
         }
+        // Role expansion: a+b -> c+d seen from a, from b, and, if inelastic, from c and from d.
+        // DOF factors (reading R21): Table III kinds are summed over the DOF of all four particles; kinds 0..3 are
+        // averaged over those of a and b.
+        const double sum_norm = p.kind >= RBG_M2_QCD_Q1Q2 ? 1.0 : species[p.a].g * species[p.b].g;
         Role r;
         r.sampler = p.sampler;
         r.kind = p.kind; std::memcpy(r.par, p.par, sizeof r.par);
-        r.sym = p.sym < 0 ? (p.a == p.b ? 0.5 : 1.0) : p.sym;
-        r.s1 = p.a; r.s2 = p.b; r.index = (int)h->roles.size();
-        h->roles.push_back(r);
-        if (p.b != p.a) { r.s1 = p.b; r.s2 = p.a; r.index = (int)h->roles.size(); h->roles.push_back(r); }
+        r.elastic = elastic;
+        auto add = [&](int s1, int s2, int s3, int s4) {
+            r.s[0] = s1; r.s[1] = s2; r.s[2] = s3; r.s[3] = s4;
+            r.sym = p.sym < 0 ? (s3 == s4 ? 0.5 : 1.0) : p.sym;
+            r.cl = sum_norm / (species[s1].g * species[s2].g);
+            r.cg = sum_norm / (species[s3].g * species[s4].g);
+            r.index = (int)h->roles.size();
+            h->roles.push_back(r);
+        };
+        add(p.a, p.b, p.c, p.d);
+        if (p.b != p.a) add(p.b, p.a, p.d, p.c);
+        if (!elastic) {
+            add(p.c, p.d, p.a, p.b);
+            if (p.d != p.c) add(p.d, p.c, p.b, p.a);
+        }
     }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { delete h; return fail(nullptr, RBG_E_CUDA, "no CUDA device (there is no CPU fallback)"); }
@@ -357,7 +401,7 @@ int rbg_n_roles(const rbg_handle* h) { return h ? (int)h->roles.size() : 0; }
 uint64_t rbg_sample_evals(const rbg_handle* h, int n_samples) {
     if (!h) return 0;
     uint64_t t = 0;
-    for (const Role& r : h->roles) t += (uint64_t)h->nx * h->np[r.s1] * (uint64_t)n_samples;
+    for (const Role& r : h->roles) t += (uint64_t)h->nx * h->np[r.s[0]] * (uint64_t)n_samples;
     return t;
 }
 int rbg_last_launch_count(const rbg_handle* h) { return h ? h->last_launches : 0; }

@@ -26,7 +26,7 @@ def oracle_C_and_scale(orc, f, n_samples, seed, **kw):
     for r in range(orc.n_roles):
         s1 = orc.roles[r]["s"][0]
         n = orc.nx * orc.np[s1]
-        mag[orc.sp_off[s1]:orc.sp_off[s1] + n] += (d["G"] + d["L"])[orc.role_off[r]:orc.role_off[r] + n]
+        mag[orc.sp_off[s1]:orc.sp_off[s1] + n] += (np.abs(d["G"]) + np.abs(d["L"]))[orc.role_off[r]:orc.role_off[r] + n]
     return C_ref, mag
 
 
@@ -203,14 +203,16 @@ def test_argument_errors():
             dict(P, grids=[dict(n=[4, 0, 4], pmin=[-1.0] * 3, pmax=[1.0] * 3)]),
             dict(P, grids=[dict(n=[4, 4, 4], pmin=[1.0] * 3, pmax=[1.0] * 3)]),
             dict(P, processes=[dict(a=0, b=1, c=0, d=1, kind=0, par=[1.0], sym=-1.0)]),
-            dict(P, processes=[dict(a=0, b=0, c=0, d=0, kind=9, par=[1.0], sym=-1.0)])]
+            dict(P, processes=[dict(a=0, b=0, c=0, d=0, kind=11, par=[1.0], sym=-1.0)])]
     for bad in bads:
         with pytest.raises(rbg.RbgError):
             rbg.Collision(bad)
-    with pytest.raises(rbg.RbgError, match="elastic"):
-        two = dict(P, species=P["species"] * 2, grids=P["grids"] * 2,
-                   processes=[dict(a=0, b=0, c=1, d=1, kind=0, par=[1.0], sym=-1.0)])
-        rbg.Collision(two)
+    two = dict(P, species=P["species"] * 2, grids=P["grids"] * 2)
+    with pytest.raises(rbg.RbgError, match="ambiguous"):          # a + b -> b + a must be written a + b -> a + b
+        rbg.Collision(dict(two, processes=[dict(a=0, b=1, c=1, d=0, kind=0, par=[1.0], sym=-1.0)]))
+    with pytest.raises(rbg.RbgError, match="elastic"):            # the t-channel sampler is for elastic processes
+        rbg.Collision(dict(two, processes=[dict(a=0, b=0, c=1, d=1, kind=1, par=[1.0, 0.1], sym=-1.0, sampler=1)]))
+    assert rbg.Collision(dict(two, processes=[dict(a=0, b=0, c=1, d=1, kind=0, par=[1.0], sym=-1.0)])).n_roles == 2
     col = rbg.Collision(P)
     f = torch.from_numpy(w["f"]).cuda()
     with pytest.raises(rbg.RbgError):
@@ -286,3 +288,59 @@ def test_sampler_argument_errors():
                 dict(P, processes=[dict(P["processes"][0], kind=1, par=[1.0, 0.1], sampler=7)])):
         with pytest.raises(rbg.RbgError):
             rbg.Collision(bad)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# NEXT-2(ii): Table III kinds and inelastic roles (workload 7 = the paper's quark-gluon plasma scenario, 70 roles)
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kw", [dict(nx=2, np_side=6, n_samples=48),       # 216-cell tables: TMA staging
+                                dict(nx=3, np_side=5, n_samples=33),       # 125 cells: odd size, cooperative staging
+                                dict(nx=1, np_side=11, n_samples=16)])     # the paper's 11^3 momentum grid
+def test_parity_fp64_qgp_all_table3_processes(kw):
+    w = workloads.make(7, **kw)
+    orc = oracle.Oracle(w["problem"])
+    assert orc.n_roles == 70
+    C_ref, mag = oracle_C_and_scale(orc, w["f"], w["n_samples"], w["seed"])
+    C, col = gpu_C(w["problem"], w["f"], w["n_samples"], w["seed"])
+    assert_parity(C, C_ref, mag, TOL64, f"cfg7 {kw}")
+    assert col.last_launch_count() == 70
+    assert col.sample_evals(w["n_samples"]) == workloads.configs.sample_evals(w["problem"], w["n_samples"])
+    # the global-memory gather path gives the same numbers
+    C2, _ = gpu_C(w["problem"], w["f"], w["n_samples"], w["seed"], options=(("gather", 2),))
+    assert np.array_equal(C, C2)
+
+
+def test_parity_fp32_qgp():
+    w = workloads.make(7, nx=2, np_side=6, n_samples=48)
+    orc = oracle.Oracle(w["problem"], use_float=True)
+    C_ref, mag = oracle_C_and_scale(orc, w["f"], w["n_samples"], w["seed"])
+    C, _ = gpu_C(w["problem"], w["f"], w["n_samples"], w["seed"], fp32=True)
+    assert_parity(C, C_ref, mag, TOL32, "fp32 cfg7")
+
+
+def test_parity_inelastic_role_with_four_species_four_grids_and_a_threshold():
+    """a + b -> c + d with four masses, four different momentum grids (three tables in shared memory) and unequal
+    degrees of freedom: the heavy pair is below threshold for part of the samples."""
+    species = [dict(mass=m, charge=0.0, stat=st, g=g) for m, st, g in
+               ((0.2, -1, 2.0), (0.35, 1, 3.0), (0.9, 0, 1.0), (1.4, -1, 4.0))]
+    grids = [dict(n=[6, 5, 7], pmin=[-2.0, -2.5, -2.0], pmax=[2.0, 2.5, 2.2]),
+             dict(n=[4, 8, 6], pmin=[-3.0] * 3, pmax=[3.0] * 3),
+             dict(n=[7, 7, 7], pmin=[-2.5] * 3, pmax=[2.5] * 3),
+             dict(n=[8, 4, 6], pmin=[-3.5] * 3, pmax=[3.5] * 3)]
+    procs = [dict(a=0, b=1, c=2, d=3, kind=0, par=[1.5], sym=-1.0),
+             dict(a=2, b=2, c=0, d=3, kind=2, par=[1.3, 0.7], sym=-1.0)]
+    prob = dict(nx=3, species=species, grids=grids, processes=procs, hbar=0.2)      # occupation numbers below 1
+    rng = np.random.default_rng(77)
+    orc = oracle.Oracle(prob)
+    assert orc.n_roles == 7
+    f = rng.random(orc.f_elems) * 0.2
+    C_ref, mag = oracle_C_and_scale(orc, f, 80, 4321)
+    C, col = gpu_C(prob, f, 80, 4321)
+    assert_parity(C, C_ref, mag, TOL64, "four-species inelastic")
+    # fused update over inelastic roles: several roles accumulate into one species block
+    out_ref, neg_ref = oracle.update(f, C_ref, 0.05)
+    ft = torch.from_numpy(f).cuda()
+    out, flag = col.collision_update(ft, 0.05, 80, 4321)
+    torch.cuda.synchronize()
+    assert np.all(np.abs(out.cpu().numpy() - out_ref) <= 0.05 * TOL64 * mag + 1e-15)
+    assert int(flag.item()) == neg_ref

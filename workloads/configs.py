@@ -12,6 +12,9 @@ KIND_CONST = 0              # |M|^2 = par[0]
 KIND_COULOMB_SCREENED = 1   # |M|^2 = par[0] / (t - par[1]^2)^2
 KIND_TCHAN_S2 = 2           # |M|^2 = par[0]^4 s^2 / (t - par[1]^2)^2
 KIND_ISO_DSIGMA = 3         # |M|^2 = 64 pi^2 s par[0]  (constant CM-frame dsigma/dOmega = par[0])
+# Table III of the paper, par = [g, m_g]
+(KIND_QCD_Q1Q2, KIND_QCD_Q1Q1, KIND_QCD_Q1QB1, KIND_QCD_Q1QB1_Q2QB2, KIND_QCD_QQB_GG, KIND_QCD_QG,
+ KIND_QCD_GG) = 4, 5, 6, 7, 8, 9, 10
 
 INPUT_SEED_BASE = 0x5EED0000
 MC_SEED_BASE = 20230810
@@ -47,6 +50,40 @@ def equilibrium_nbar(E, T, stat, mu=0.0):
 
 def _elastic(a, b, kind, par):
     return dict(a=a, b=b, c=a, d=b, kind=kind, par=list(par), sym=-1.0)
+
+
+def _process(a, b, c, d, kind, par):
+    return dict(a=a, b=b, c=c, d=d, kind=kind, par=list(par), sym=-1.0)
+
+
+def qgp_processes(par, n_flavours=3):
+    """Every row of Table III among n_flavours quarks (species 0..nf-1), their antiquarks
+    (nf..2nf-1) and the gluon (2nf): "seven particle species ... u, d, and s quarks, their anti-quarks, and gluons"
+    (PAPER.md:510).  With 3 flavours: 34 processes, 70 roles."""
+    nf = n_flavours
+    q, qb, G = list(range(nf)), list(range(nf, 2 * nf)), 2 * nf
+    procs = []
+    for i in range(nf):
+        for j in range(i + 1, nf):
+            procs.append(_elastic(q[i], q[j], KIND_QCD_Q1Q2, par))
+            procs.append(_elastic(qb[i], qb[j], KIND_QCD_Q1Q2, par))
+        for j in range(nf):
+            if j != i:
+                procs.append(_elastic(q[i], qb[j], KIND_QCD_Q1Q2, par))
+    for i in range(nf):
+        procs.append(_elastic(q[i], q[i], KIND_QCD_Q1Q1, par))
+        procs.append(_elastic(qb[i], qb[i], KIND_QCD_Q1Q1, par))
+        procs.append(_elastic(q[i], qb[i], KIND_QCD_Q1QB1, par))
+    for i in range(nf):
+        for j in range(i + 1, nf):
+            procs.append(_process(q[i], qb[i], q[j], qb[j], KIND_QCD_Q1QB1_Q2QB2, par))
+    for i in range(nf):
+        procs.append(_process(q[i], qb[i], G, G, KIND_QCD_QQB_GG, par))
+    for i in range(nf):
+        procs.append(_elastic(q[i], G, KIND_QCD_QG, par))
+        procs.append(_elastic(qb[i], G, KIND_QCD_QG, par))
+    procs.append(_elastic(G, G, KIND_QCD_GG, par))
+    return procs
 
 
 def make(cfg: int, nx: int | None = None, n_samples: int | None = None, np_side: int | None = None,
@@ -143,6 +180,32 @@ def make(cfg: int, nx: int | None = None, n_samples: int | None = None, np_side:
         fs = [np.tile(f0 * inside, (nx, 1)) for f0 in (0.2, 0.4)]
         dt = 0.0002 / 0.197
         name = "cfg6: paper's collision test (Eq. 46-48): 2 classical species m=0.3, const dsigma/dOmega 1/20/0.01"
+    elif cfg == 7:
+        # The paper's multi-GPU performance scenario (Table II :484-491): quark-gluon plasma, seven
+        # species (u, d, s, their antiquarks, gluons), every process of Table III, the recommended per-run grid
+        # 21^3 spatial x 11^3 momentum cells.  Not in BASELINE.json (NEXT-2(ii)).  The paper gives no masses, coupling,
+        # regulator, box or initial state for that run (reading R22): quarks m = 0.3, 0.3, 0.45 with g = 6
+        # (Fermi-Dirac), gluon m = 0.5 with g = 16 (Bose-Einstein), coupling 2, regulator m_g = 0.8,
+        # box [-2,2]^3, hbar = 1, f = nbar/kappa at T = 0.4 with a seeded anisotropy and the gluons under-populated
+        # by a factor 1/2 (so that q qbar <-> g g has a net rate); 256 samples per cell and role.
+        nxd, N, side = 21 ** 3, 256, 11
+        nx = nxd if nx is None else nx
+        side = side if np_side is None else np_side
+        masses = [0.3, 0.3, 0.45, 0.3, 0.3, 0.45, 0.5]
+        stats = [-1] * 6 + [1]
+        gs = [6.0] * 6 + [16.0]
+        species = [dict(mass=m, charge=0.0, stat=st, g=g) for m, st, g in zip(masses, stats, gs)]
+        grids = [_grid(side, -2.0, 2.0) for _ in masses]
+        procs = qgp_processes([2.0, 0.8])
+        fs = []
+        for s, g in zip(species, grids):
+            P = cell_centres(g)
+            E = np.sqrt((P * P).sum(1) + s["mass"] ** 2)
+            kappa = (2.0 * np.pi) ** 3 / s["g"]
+            nbar = equilibrium_nbar(E, 0.4, s["stat"]) * (0.5 if s["stat"] == 1 else 1.0)
+            aniso = 1.0 + 0.2 * (P[:, 2] / E)[None, :] * (2.0 * rng.random((nx, P.shape[0])) - 1.0)
+            fs.append(nbar[None, :] / kappa * aniso)
+        name = "cfg7: quark-gluon plasma, 7 species, all Table III processes (34 processes, 70 roles)"
     else:
         raise ValueError(f"unknown config {cfg}")
     if sampler:
@@ -156,14 +219,35 @@ def make(cfg: int, nx: int | None = None, n_samples: int | None = None, np_side:
                 seed=int(seed), dt=float(dt), fp32=bool(fp32))
 
 
+def roles(problem):
+    """(s1, s2, s3, s4) of every role, in role order: a + b -> c + d is seen from a, from b (if
+    b != a) and, if it is inelastic, from c and from d (if d != c)."""
+    out = []
+    for p in problem["processes"]:
+        a, b, c, d = p["a"], p["b"], p["c"], p["d"]
+        out.append((a, b, c, d))
+        if b != a:
+            out.append((b, a, d, c))
+        if not (c == a and d == b):
+            out.append((c, d, a, b))
+            if d != c:
+                out.append((d, c, b, a))
+    return out
+
+
+def role_processes(problem):
+    """The process each role comes from, in role order."""
+    out = []
+    for p in problem["processes"]:
+        a, b, c, d = p["a"], p["b"], p["c"], p["d"]
+        out += [p] * ((1 if b == a else 2) + (0 if (c == a and d == b) else (1 if d == c else 2)))
+    return out
+
+
 def n_roles(problem) -> int:
-    return sum(1 if p["a"] == p["b"] else 2 for p in problem["processes"])
+    return len(roles(problem))
 
 
 def sample_evals(problem, n_samples) -> int:
     """roles * Nx * Np * N: the 'collision samples' one sweep evaluates (BASELINE.json metric)."""
-    tot = 0
-    for p in problem["processes"]:
-        for s in ([p["a"]] if p["a"] == p["b"] else [p["a"], p["b"]]):
-            tot += problem["nx"] * int(np.prod(problem["grids"][s]["n"])) * n_samples
-    return tot
+    return sum(problem["nx"] * int(np.prod(problem["grids"][r[0]]["n"])) * n_samples for r in roles(problem))
