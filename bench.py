@@ -141,8 +141,104 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def run_be_steps(args):
+    """--path be: the NEXT-4 kernels (rbg_moments, rbg_drift_step, rbg_vlasov_step) on the chosen config, one JSON line.
+    A step = moments + one drift step + one Vlasov step over every phase-space cell.  HBM roofline: algorithmic bytes
+    are 8 B per cell for the moments (f read once) and 16 B per cell for each stencil (f read once, f_out written once);
+    peak = MEASURED_PEAKS.json hbm_gbs (sustained copy bandwidth), else the profiling guide's fallback 6500 GB/s."""
+    import torch
+    import paper_2308_04869_b200 as rbg
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    torch.cuda.set_device(0)
+    w = workloads.make(args.config, nx=args.nx)
+    prob = w["problem"]
+    nx = prob["nx"]
+    side = round(nx ** (1.0 / 3.0))
+    nxyz = (side, side, side) if side ** 3 == nx else (nx, 1, 1)
+    charges = (-1.0, 1.0, 2.0, 0.5, -0.5, 0.0, 1.5)
+    for sp, q in zip(prob["species"], charges):
+        if sp.get("charge", 0.0) == 0.0:
+            sp["charge"] = q                       # the Vlasov step needs charged species
+    col = rbg.Collision(dict(prob, nx=nxyz))
+    f = torch.from_numpy(w["f"]).cuda()
+    out = torch.empty_like(f)
+    rng = np.random.default_rng(5)
+    E = torch.from_numpy(rng.normal(size=(nx, 3))).cuda()
+    B = torch.from_numpy(rng.normal(size=(nx, 3))).cuda()
+    cells = int(f.numel())
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+    dx = (0.5, 0.5, 0.5)
+    kernels = {"moments": (lambda: col.moments(f, stream=stream), 8.0),
+               "drift": (lambda: col.drift_step(f, 0.01, dx, out=out, stream=stream), 16.0),
+               "vlasov": (lambda: col.vlasov_step(f, 0.01, E, B, out=out, stream=stream), 16.0)}
+    try:
+        peaks = json.loads((ROOT / "MEASURED_PEAKS.json").read_text())
+        peak, peak_src = float(peaks["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+    except (OSError, ValueError, KeyError):
+        peak, peak_src = 6500.0, "B200_PROFILING.md fallback"
+    res, launches = {}, 0
+    with ClockSampler(0) as cs:
+        for name, (fn, bytes_per_cell) in kernels.items():
+            for _ in range(max(args.warmup, 3)):
+                fn()
+            torch.cuda.synchronize()
+            ts = []
+            for _ in range(args.steps):
+                flush.fill_(1)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream); fn(); e1.record(stream)
+                torch.cuda.synchronize()
+                ts.append(e0.elapsed_time(e1))
+            launches += col.last_launch_count() * args.steps
+            ms = sum(ts) / len(ts)
+            gbs = bytes_per_cell * cells / (ms * 1e-3) / 1e9
+            res[name] = {"ms": ms, "algorithmic_bytes_per_cell": bytes_per_cell, "achieved_gbs": gbs, "frac": gbs / peak}
+    clocks = cs.summary()
+    t_step = sum(r["ms"] for r in res.values()) * 1e-3
+    # e2e: host buffers in, host buffers out, for the three calls of one step
+    f_host = torch.from_numpy(w["f"]).pin_memory()
+    o_host = torch.empty_like(f_host).pin_memory()
+    t0 = time.perf_counter()
+    fd = f_host.cuda(non_blocking=True)
+    M, tot, em = col.moments(fd)
+    o1 = col.drift_step(fd, 0.01, dx)
+    o2 = col.vlasov_step(o1, 0.01, E, B)
+    o_host.copy_(o2, non_blocking=True); em_h = em.cpu()
+    torch.cuda.synchronize()
+    t_e2e = time.perf_counter() - t0
+    dom = max(("drift", "vlasov"), key=lambda k: res[k]["ms"])
+    line = {"metric": "be_step_phase_space_cells_per_s", "value": cells / t_step, "unit": "cells/s", "n_gpus": 1, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": t_step * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w["name"] + " [moments + UPFD drift + UPFD Vlasov, NEXT-4]", "cfg": args.config, "nxyz": list(nxyz),
+                       "cells": cells, "f_bytes": int(w["f"].nbytes), "l2": "L2 flushed (256 MB write) between timed iterations"},
+            "clocks": clocks, "gpu_launches": launches,
+            "e2e": {"value": cells / t_e2e, "unit": "cells/s", "h2d_bytes_per_step": int(w["f"].nbytes),
+                    "d2h_bytes_per_step": int(w["f"].nbytes) + int(em.numel() * 8), "ms_per_step": t_e2e * 1e3},
+            "roofline": {"bound": "hbm", "achieved": res[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s", "frac": res[dom]["frac"],
+                         "traffic": None, "kernel": f"rbg::{dom}_upfd_kernel", "peak_source": peak_src},
+            "kernels": res}
+    if not args.no_cpu_baseline:
+        from oracle import be_steps as bs
+        ncell = max(1, min(nx, 8))
+        sub = dict(prob, nx=ncell)
+        fsub = np.concatenate([w["f"][o:o + ncell * int(np.prod(g["n"]))] for o, g in zip(wl.f_layout(prob)[0], prob["grids"])])
+        t0 = time.perf_counter()
+        bs.moments(sub, fsub)
+        g1 = bs.drift_upfd(sub, fsub, (ncell, 1, 1), 0.01, dx)
+        bs.vlasov_upfd(sub, g1, 0.01, E.cpu().numpy()[:ncell], B.cpu().numpy()[:ncell])
+        dt = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": fsub.size / dt, "unit": "cells/s", "cores": 1, "kind": "oracle",
+                                "sample": f"{ncell} of {nx} spatial cells as an {ncell}x1x1 periodic box, every species and momentum cell"}
+    print(json.dumps(line))
+
+
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--path", default="collision", choices=["collision", "be"], help="collision: the hot path "
+                    "(default); be: the NEXT-4 kernels (moments, UPFD drift, UPFD Vlasov)")
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
@@ -159,6 +255,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.path == "be":
+        return run_be_steps(args)
 
     import torch
     import torch.distributed as dist

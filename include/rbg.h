@@ -147,6 +147,34 @@ int rbg_collision_evolve(rbg_handle* h, double* f_dev, double* scratch_dev, doub
  * is not required. */
 int rbg_collision_host(rbg_handle* h, const double* f_host, double* C_host, int n_samples, uint64_t seed);
 
+/* ---- The steps either side of the collision term ---------------------------------
+ * Moments of f per species and spatial cell (midpoint sums over the momentum grid, Int d3p -> Sum dp^3, c = 1):
+ *   n = Int f, j^k = Int v^k f (Eq. 5-6), T^{mu nu} = Int d3p/p0 p^mu p^nu f (Eq. 9).
+ * M_dev: [n_species][Nx][RBG_N_MOMENTS] doubles in the order n, jx, jy, jz, T00, T01, T02, T03, T11, T12, T13, T22,
+ * T23, T33.  total_dev (may be NULL): [Nx][RBG_N_MOMENTS] = the sum over species (Eq. 7, 9).  em_dev (may be NULL):
+ * [Nx][4] = (rho, Jx, Jy, Jz) = Sum_a Q_a (n_a, j_a) (Eq. 15).  All device pointers, caller-owned,
+ * overwritten.  Asynchronous on cuda_stream. */
+#define RBG_N_MOMENTS 14
+int rbg_moments(rbg_handle* h, const double* f_dev, double* M_dev, double* total_dev, double* em_dev, void* cuda_stream);
+
+/* One first-order UPFD (unconditionally positivity-preserving finite difference) step of the drift term, Eq. 25 with
+ * Eq. 28-30, all three directions at once (reading R23):
+ *   f_out(x) = [ f/3 + dt Sum_d |v_d| f(x - sign(v_d) dx_d e_d) / dx_d ] / [ 1/3 + dt Sum_d |v_d| / dx_d ],  v = p/E_p.
+ * The spatial grid is the (nx, ny, nz) of rbg_create, ix = (i_x ny + i_y) nz + i_z.  bc[d]: 1 periodic, 0 wall; a wall
+ * reflects with probability zeta in [0,1]: the value beyond it is zeta * f(wall cell, p_d -> -p_d),
+ * which needs momentum grids symmetric about 0 when zeta != 0 (else RBG_E_UNSUPPORTED); zeta = 0 absorbs.
+ * f_out_dev must not alias f_dev.  Needs the whole spatial domain in this handle (ix_offset == 0): across GPUs the
+ * stencil would need the paper's ghost-layer exchange, which is out of scope. */
+typedef struct { double dt; double dx[3]; int bc[3]; double zeta; } rbg_drift_params;
+int rbg_drift_step(rbg_handle* h, const double* f_dev, double* f_out_dev, const rbg_drift_params* p, void* cuda_stream);
+
+/* One first-order UPFD step of the Vlasov term, Eq. 26 with Eq. 34, all three directions at once:
+ *   f_out(p) = [ f/3 + dt Sum_d |F_d| f(p - sign(F_d) dp_d e_d) / dp_d ] / [ 1/3 + dt Sum_d |F_d| / dp_d ],
+ * F = Q (E + v x B) with the species' charge and the fields of the spatial cell, E_dev and B_dev being
+ * [Nx][3] doubles; periodic in every momentum direction.  f_out_dev must not alias f_dev. */
+int rbg_vlasov_step(rbg_handle* h, const double* f_dev, double* f_out_dev, double dt, const double* E_dev,
+                    const double* B_dev, void* cuda_stream);
+
 /* Number of doubles in f / C / f_out. */
 size_t rbg_f_elems(const rbg_handle* h);
 /* Number of roles (a process seen from one grid species; a+b with a != b gives two). */

@@ -34,6 +34,13 @@ class _Species(C.Structure):
     _fields_ = [("mass", C.c_double), ("charge", C.c_double), ("stat", C.c_int), ("g", C.c_double)]
 
 
+class _DriftParams(C.Structure):
+    _fields_ = [("dt", C.c_double), ("dx", C.c_double * 3), ("bc", C.c_int * 3), ("zeta", C.c_double)]
+
+
+N_MOMENTS = 14
+
+
 class _Process(C.Structure):
     _fields_ = [("a", C.c_int), ("b", C.c_int), ("c", C.c_int), ("d", C.c_int), ("kind", C.c_int),
                 ("par", C.c_double * 4), ("sym", C.c_double), ("sampler", C.c_int)]
@@ -49,6 +56,9 @@ _SIGNATURES = {
     "rbg_collision_evolve": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int, C.c_void_p, C.c_int,
                                        C.c_uint64, C.c_void_p]),
     "rbg_collision_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_uint64]),
+    "rbg_moments": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "rbg_drift_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "rbg_vlasov_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]),
     "rbg_f_elems": (C.c_size_t, [C.c_void_p]),
     "rbg_n_roles": (C.c_int, [C.c_void_p]),
     "rbg_sample_evals": (C.c_uint64, [C.c_void_p, C.c_int]),
@@ -140,6 +150,8 @@ class Collision:
         self._h = h
         self.f_elems = int(lib.rbg_f_elems(h))
         self.n_roles = int(lib.rbg_n_roles(h))
+        self.n_species = len(sp)
+        self.n_cells = int(np.prod(nxyz))
 
     def __del__(self):
         h = getattr(self, "_h", None)
@@ -198,6 +210,41 @@ class Collision:
                                                    int(n_steps), C.c_void_p(neg_flag.data_ptr()), int(n_samples),
                                                    int(seed), _stream_ptr(stream)), self._h)
         return f, neg_flag
+
+    # -- the steps either side of the collision term (NEXT-4) --------------------------------------
+    def moments(self, f, stream=None):
+        """rbg_moments: (M[n_species, Nx, 14], total[Nx, 14], em[Nx, 4]) as CUDA tensors."""
+        import torch
+        M = torch.empty((self.n_species, self.n_cells, N_MOMENTS), dtype=torch.float64, device=f.device)
+        tot = torch.empty((self.n_cells, N_MOMENTS), dtype=torch.float64, device=f.device)
+        em = torch.empty((self.n_cells, 4), dtype=torch.float64, device=f.device)
+        _check(load_library().rbg_moments(self._h, self._dev(f, "f"), C.c_void_p(M.data_ptr()), C.c_void_p(tot.data_ptr()),
+                                          C.c_void_p(em.data_ptr()), _stream_ptr(stream)), self._h)
+        return M, tot, em
+
+    def drift_step(self, f, dt: float, dx, bc=(1, 1, 1), zeta: float = 0.0, out=None, stream=None):
+        """rbg_drift_step: one UPFD step of the drift term (Eq. 30)."""
+        import torch
+        if out is None:
+            out = torch.empty_like(f)
+        p = _DriftParams(float(dt), (C.c_double * 3)(*[float(v) for v in dx]), (C.c_int * 3)(*[int(v) for v in bc]), float(zeta))
+        _check(load_library().rbg_drift_step(self._h, self._dev(f, "f"), self._dev(out, "out"), C.byref(p),
+                                             _stream_ptr(stream)), self._h)
+        return out
+
+    def vlasov_step(self, f, dt: float, E, B, out=None, stream=None):
+        """rbg_vlasov_step: one UPFD step of the Vlasov term (Eq. 34); E, B are [Nx, 3] float64 CUDA tensors."""
+        import torch
+        if out is None:
+            out = torch.empty_like(f)
+        for name, t in (("E", E), ("B", B)):
+            if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+                    and t.numel() == 3 * self.n_cells):
+                raise RbgError(f"{name} must be a contiguous float64 CUDA tensor with {3 * self.n_cells} elements")
+        _check(load_library().rbg_vlasov_step(self._h, self._dev(f, "f"), self._dev(out, "out"), float(dt),
+                                              C.c_void_p(E.data_ptr()), C.c_void_p(B.data_ptr()), _stream_ptr(stream)),
+               self._h)
+        return out
 
     def collision_host(self, f_host, n_samples: int, seed: int, out=None):
         """rbg_collision_host: host buffers in, host buffers out (numpy float64 or pinned CPU tensors)."""

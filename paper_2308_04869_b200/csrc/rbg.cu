@@ -13,6 +13,7 @@
 #include <vector>
 
 #include "rbg_kernels.cuh"
+#include "rbg_be_kernels.cuh"
 
 namespace {
 
@@ -33,6 +34,7 @@ struct Role {
 
 struct rbg_handle {
     int nx = 0, ix_offset = 0;
+    int nxyz[3] = {0, 0, 0};
     int n_species = 0;
     std::vector<rbg_species> species;
     std::vector<rbg_momentum_grid> grids;
@@ -47,6 +49,9 @@ struct rbg_handle {
     // options
     int opt_warps = 0, opt_p1_per_cta = 0, opt_gather = 0, opt_spl = 0;
     int last_launches = 0;
+    // per-species device tables for the moment / drift / Vlasov kernels: 1/E_p and v = p/E_p per momentum cell
+    std::vector<double*> tab_iE, tab_v;
+    double* charges_dev = nullptr;
     // scratch for the host entry point
     double *scratch_f = nullptr, *scratch_c = nullptr;
     size_t scratch_elems = 0;
@@ -282,6 +287,7 @@ int rbg_create(rbg_handle** out, const rbg_spatial_grid* grid, int n_species, co
     if (flags != RBG_FP64 && flags != RBG_FP32_KINEMATICS) return fail(nullptr, RBG_E_INVALID_ARG, "unknown flags");
     rbg_handle* h = new rbg_handle;
     h->nx = grid->nx * grid->ny * grid->nz;
+    h->nxyz[0] = grid->nx; h->nxyz[1] = grid->ny; h->nxyz[2] = grid->nz;
     h->ix_offset = grid->ix_offset;
     h->n_species = n_species; h->hbar = hbar; h->flags = flags;
     size_t off = 0;
@@ -345,6 +351,39 @@ int rbg_create(rbg_handle** out, const rbg_spatial_grid* grid, int n_species, co
     cudaGetDevice(&h->device);
     cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, h->device);
     cudaDeviceGetAttribute(&h->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device);
+    // momentum-cell tables (E_p = sqrt(|p|^2 + m^2); v = p / E_p, Eq. 6): inputs of the NEXT-4 kernels
+    std::vector<double> charges(n_species);
+    for (int s = 0; s < n_species; ++s) {
+        const rbg_momentum_grid& G = h->grids[s];
+        const size_t np = h->np[s];
+        std::vector<double> iE(np), v(3 * np);
+        const double m = h->species[s].mass;
+        charges[s] = h->species[s].charge;
+        size_t j = 0;
+        for (int i0 = 0; i0 < G.n[0]; ++i0)
+            for (int i1 = 0; i1 < G.n[1]; ++i1)
+                for (int i2 = 0; i2 < G.n[2]; ++i2, ++j) {
+                    const int id[3] = {i0, i1, i2};
+                    double pc[3];
+                    for (int d = 0; d < 3; ++d) pc[d] = G.pmin[d] + ((double)id[d] + 0.5) * ((G.pmax[d] - G.pmin[d]) / (double)G.n[d]);
+                    const double E = std::sqrt(((pc[0] * pc[0] + pc[1] * pc[1]) + pc[2] * pc[2]) + m * m);
+                    iE[j] = E > 0.0 ? 1.0 / E : 0.0;
+                    for (int d = 0; d < 3; ++d) v[(size_t)d * np + j] = E > 0.0 ? pc[d] / E : 0.0;
+                }
+        double *d_iE = nullptr, *d_v = nullptr;
+        if (cudaMalloc(&d_iE, np * sizeof(double)) != cudaSuccess || cudaMalloc(&d_v, 3 * np * sizeof(double)) != cudaSuccess ||
+            cudaMemcpy(d_iE, iE.data(), np * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(d_v, v.data(), 3 * np * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess) {
+            cudaFree(d_iE); cudaFree(d_v); rbg_destroy(h);
+            return fail(nullptr, RBG_E_CUDA, "allocating the momentum-cell tables failed");
+        }
+        h->tab_iE.push_back(d_iE); h->tab_v.push_back(d_v);
+    }
+    if (cudaMalloc(&h->charges_dev, n_species * sizeof(double)) != cudaSuccess ||
+        cudaMemcpy(h->charges_dev, charges.data(), n_species * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess) {
+        rbg_destroy(h);
+        return fail(nullptr, RBG_E_CUDA, "allocating the charge table failed");
+    }
     *out = h;
     return RBG_OK;
 }
@@ -422,7 +461,106 @@ const char* rbg_last_error(const rbg_handle* h) { return h ? h->err.c_str() : g_
 void rbg_destroy(rbg_handle* h) {
     if (!h) return;
     cudaFree(h->scratch_f); cudaFree(h->scratch_c);
+    for (double* p : h->tab_iE) cudaFree(p);
+    for (double* p : h->tab_v) cudaFree(p);
+    cudaFree(h->charges_dev);
     delete h;
+}
+
+// ---- NEXT-4: the steps either side of the collision term -------------------------------------------------------
+namespace {
+rbg::SpeciesTables species_tables(const rbg_handle* h, int s) {
+    rbg::SpeciesTables t;
+    t.iE = h->tab_iE[s]; t.v = h->tab_v[s];
+    for (int d = 0; d < 3; ++d) {
+        t.pmin[d] = h->grids[s].pmin[d];
+        t.delta[d] = (h->grids[s].pmax[d] - h->grids[s].pmin[d]) / (double)h->grids[s].n[d];
+        t.n[d] = h->grids[s].n[d];
+    }
+    t.np = (int)h->np[s];
+    t.mass = h->species[s].mass; t.charge = h->species[s].charge;
+    return t;
+}
+struct DeviceGuard {
+    int prev = -1; int want;
+    explicit DeviceGuard(int w) : want(w) { cudaGetDevice(&prev); if (prev != want) cudaSetDevice(want); }
+    ~DeviceGuard() { if (prev >= 0 && prev != want) cudaSetDevice(prev); }
+};
+}  // namespace
+
+int rbg_moments(rbg_handle* h, const double* f_dev, double* M_dev, double* total_dev, double* em_dev, void* cuda_stream) {
+    if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
+    if (!f_dev || !M_dev) return fail(h, RBG_E_INVALID_ARG, "null buffer");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    DeviceGuard guard(h->device);
+    h->last_launches = 0;
+    for (int s = 0; s < h->n_species; ++s) {
+        rbg::moments_kernel<<<h->nx, 128, 0, st>>>(f_dev + h->sp_off[s], species_tables(h, s), h->nx,
+                                                   M_dev + (size_t)s * h->nx * rbg::N_MOMENTS);
+        RBG_CUDA(h, cudaGetLastError());
+        ++h->last_launches;
+    }
+    if (total_dev || em_dev) {
+        const size_t n = (size_t)h->nx * rbg::N_MOMENTS;
+        rbg::totals_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(M_dev, h->charges_dev, h->n_species, h->nx, total_dev, em_dev);
+        RBG_CUDA(h, cudaGetLastError());
+        ++h->last_launches;
+    }
+    return RBG_OK;
+}
+
+int rbg_drift_step(rbg_handle* h, const double* f_dev, double* f_out_dev, const rbg_drift_params* p, void* cuda_stream) {
+    if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
+    if (!f_dev || !f_out_dev || !p) return fail(h, RBG_E_INVALID_ARG, "null argument");
+    if (f_dev == f_out_dev) return fail(h, RBG_E_INVALID_ARG, "output must not alias f (the stencil reads neighbours)");
+    if (!(p->dt >= 0.0)) return fail(h, RBG_E_INVALID_ARG, "dt must be >= 0");
+    if (h->ix_offset != 0) return fail(h, RBG_E_UNSUPPORTED, "the drift stencil needs the whole spatial domain on one GPU (no ghost-layer exchange)");
+    rbg::DriftParams dp;
+    dp.dt = p->dt; dp.zeta = p->zeta;
+    for (int d = 0; d < 3; ++d) {
+        if (!(p->dx[d] > 0.0)) return fail(h, RBG_E_INVALID_ARG, "dx must be positive");
+        if (p->bc[d] != 0 && p->bc[d] != 1) return fail(h, RBG_E_INVALID_ARG, "bc must be 0 (wall) or 1 (periodic)");
+        dp.inv_dx[d] = 1.0 / p->dx[d]; dp.nxyz[d] = h->nxyz[d]; dp.bc[d] = p->bc[d];
+    }
+    if (!(p->zeta >= 0.0 && p->zeta <= 1.0)) return fail(h, RBG_E_INVALID_ARG, "zeta must be in [0, 1]");
+    if (p->zeta != 0.0)
+        for (int s = 0; s < h->n_species; ++s)
+            for (int d = 0; d < 3; ++d)
+                if (p->bc[d] == 0 && std::fabs(h->grids[s].pmin[d] + h->grids[s].pmax[d]) > 1e-12 * (h->grids[s].pmax[d] - h->grids[s].pmin[d]))
+                    return fail(h, RBG_E_UNSUPPORTED, "reflecting walls need momentum grids symmetric about 0 (the mirrored momentum must be a grid cell)");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    DeviceGuard guard(h->device);
+    h->last_launches = 0;
+    dp.slab = 16;
+    for (int s = 0; s < h->n_species; ++s) {
+        const int nchunks = ((int)h->np[s] + 255) / 256;
+        const long grid = (long)nchunks * ((h->nx + dp.slab - 1) / dp.slab);
+        rbg::drift_upfd_kernel<<<(unsigned)grid, 256, 0, st>>>(f_dev + h->sp_off[s], f_out_dev + h->sp_off[s], species_tables(h, s), dp);
+        RBG_CUDA(h, cudaGetLastError());
+        ++h->last_launches;
+    }
+    return RBG_OK;
+}
+
+int rbg_vlasov_step(rbg_handle* h, const double* f_dev, double* f_out_dev, double dt, const double* E_dev, const double* B_dev,
+                    void* cuda_stream) {
+    if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
+    if (!f_dev || !f_out_dev || !E_dev || !B_dev) return fail(h, RBG_E_INVALID_ARG, "null buffer");
+    if (f_dev == f_out_dev) return fail(h, RBG_E_INVALID_ARG, "output must not alias f (the stencil reads neighbours)");
+    if (!(dt >= 0.0)) return fail(h, RBG_E_INVALID_ARG, "dt must be >= 0");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    DeviceGuard guard(h->device);
+    h->last_launches = 0;
+    rbg::VlasovParams vp;
+    vp.dt = dt; vp.nx_cells = h->nx; vp.slab = 16; vp.E = E_dev; vp.B = B_dev;
+    for (int s = 0; s < h->n_species; ++s) {
+        const int nchunks = ((int)h->np[s] + 255) / 256;
+        const long grid = (long)nchunks * ((h->nx + vp.slab - 1) / vp.slab);
+        rbg::vlasov_upfd_kernel<<<(unsigned)grid, 256, 0, st>>>(f_dev + h->sp_off[s], f_out_dev + h->sp_off[s], species_tables(h, s), vp);
+        RBG_CUDA(h, cudaGetLastError());
+        ++h->last_launches;
+    }
+    return RBG_OK;
 }
 
 int rbg_selftest_math(uint64_t n_operands, uint32_t seed, uint64_t* mismatches) {

@@ -1,0 +1,120 @@
+"""Parity of the NEXT-4 kernels (rbg_moments, rbg_drift_step, rbg_vlasov_step) against oracle/be_steps.py through
+the C ABI, element by element on the same seeded inputs.
+
+Tolerances (fp64, derived from the arithmetic): a moment is a sum of Np products, compared within
+1e-12 of the sum of the absolute values of its terms (summation order differs); a stencil output is a ratio of two
+short sums of non-negative terms, compared within 1e-14 relative (a few roundings)."""
+import numpy as np
+import pytest
+import torch
+
+import workloads
+from oracle import be_steps as bs
+
+pytestmark = pytest.mark.gpu
+
+
+def _rbg():
+    import paper_2308_04869_b200 as rbg
+    return rbg
+
+
+def _with_grid(problem, nxyz):
+    return dict(problem, nx=tuple(nxyz))
+
+
+CASES = [(2, dict(np_side=20), (3, 2, 2)),          # two species, 8000-cell grids
+         (7, dict(np_side=11), (2, 3, 2)),          # seven species, the paper's 11^3 grid (odd: a cell at p = 0)
+         (3, dict(np_side=8), (1, 1, 5)),           # includes an almost massless species
+         (1, dict(np_side=16), (1, 1, 1))]
+
+
+@pytest.mark.parametrize("cfg,kw,nxyz", CASES)
+def test_moments_parity(cfg, kw, nxyz):
+    rbg = _rbg()
+    w = workloads.make(cfg, nx=int(np.prod(nxyz)), **kw)
+    prob = w["problem"]
+    for s, q in zip(prob["species"], (-1.0, 1.0, 2.0, 0.5, -0.5, 0.0, 1.5)):
+        s["charge"] = q
+    M_ref, tot_ref, em_ref = bs.moments(prob, w["f"])
+    Mabs, totabs, _ = bs.moments(prob, np.abs(w["f"]))
+    # scale of a term sum: moments of |f| with |weights| are bounded by E-weighted ones; use n and T00 of |f|
+    col = rbg.Collision(_with_grid(prob, nxyz))
+    M, tot, em = col.moments(torch.from_numpy(w["f"]).cuda())
+    torch.cuda.synchronize()
+    M, tot, em = M.cpu().numpy(), tot.cpu().numpy(), em.cpu().numpy()
+    assert M.shape == M_ref.shape
+    pmax = max(max(abs(v) for v in g["pmin"] + g["pmax"]) for g in prob["grids"])
+    scale = np.maximum(Mabs[..., 0:1], Mabs[..., 4:5]) * max(1.0, pmax) ** 2
+    assert np.all(np.abs(M - M_ref) <= 1e-12 * scale), np.max(np.abs(M - M_ref) / scale)
+    assert np.all(np.abs(tot - tot_ref) <= 1e-12 * scale.sum(0))
+    assert np.all(np.abs(em - em_ref) <= 3e-12 * scale.sum(0)[:, :1])
+    assert np.any(M_ref[..., 1:4] != 0) and np.all(M_ref[..., 0] > 0)
+    assert col.last_launch_count() == len(prob["species"]) + 1
+
+
+@pytest.mark.parametrize("cfg,kw,nxyz,bc,zeta", [
+    (2, dict(np_side=8), (5, 4, 3), (1, 1, 1), 0.0),
+    (2, dict(np_side=8), (5, 4, 3), (0, 1, 0), 0.0),          # absorbing walls in x and z
+    (7, dict(np_side=5), (3, 6, 4), (0, 0, 0), 0.6),          # partially reflecting walls, odd momentum grid
+    (4, dict(np_side=20), (2, 2, 19), (1, 0, 1), 1.0),        # slab boundary inside the z rows (19 cells per row, slabs of 16)
+    (1, dict(np_side=16), (1, 1, 1), (1, 1, 1), 0.0)])        # one cell: every neighbour is the cell itself
+def test_drift_step_parity(cfg, kw, nxyz, bc, zeta):
+    rbg = _rbg()
+    w = workloads.make(cfg, nx=int(np.prod(nxyz)), **kw)
+    prob = w["problem"]
+    dt, dx = 0.07, (0.5, 0.8, 0.3)
+    ref = bs.drift_upfd(prob, w["f"], nxyz, dt, dx, bc=bc, zeta=zeta)
+    col = rbg.Collision(_with_grid(prob, nxyz))
+    out = col.drift_step(torch.from_numpy(w["f"]).cuda(), dt, dx, bc=bc, zeta=zeta)
+    torch.cuda.synchronize()
+    out = out.cpu().numpy()
+    assert np.all(np.abs(out - ref) <= 1e-14 * np.abs(ref)), np.max(np.abs(out - ref) / np.abs(ref))
+    assert np.all(out >= 0)
+    # a single periodic cell is its own neighbour: the step leaves it unchanged; everything else moves
+    assert np.allclose(out, w["f"], rtol=1e-13) == (int(np.prod(nxyz)) == 1)
+
+
+@pytest.mark.parametrize("cfg,kw,nx", [(2, dict(np_side=8), 7), (7, dict(np_side=5), 20), (2, dict(np_side=20), 3),
+                                       (3, dict(np_side=6), 17)])
+def test_vlasov_step_parity(cfg, kw, nx):
+    rbg = _rbg()
+    w = workloads.make(cfg, nx=nx, **kw)
+    prob = w["problem"]
+    for s, q in zip(prob["species"], (-1.0, 1.0, 2.0, 0.5, -0.5, 0.0, 1.5)):
+        s["charge"] = q
+    rng = np.random.default_rng(11)
+    E = rng.normal(size=(nx, 3)); B = rng.normal(size=(nx, 3))
+    E[0] = 0.0; B[0] = 0.0                                   # a field-free cell: f unchanged
+    B[1] = 0.0
+    dt = 0.02
+    ref = bs.vlasov_upfd(prob, w["f"], dt, E, B)
+    col = rbg.Collision(prob)
+    out = col.vlasov_step(torch.from_numpy(w["f"]).cuda(), dt, torch.from_numpy(E).cuda(), torch.from_numpy(B).cuda())
+    torch.cuda.synchronize()
+    out = out.cpu().numpy()
+    assert np.all(np.abs(out - ref) <= 1e-14 * np.abs(ref)), np.max(np.abs(out - ref) / np.abs(ref))
+    assert np.all(out >= 0) and not np.allclose(out, w["f"])
+
+
+def test_be_step_argument_errors():
+    rbg = _rbg()
+    w = workloads.make(1, np_side=4)
+    col = rbg.Collision(w["problem"])
+    f = torch.from_numpy(w["f"]).cuda()
+    with pytest.raises(rbg.RbgError):
+        col.drift_step(f, 0.1, (1.0, 1.0, 1.0), out=f)               # aliasing
+    with pytest.raises(rbg.RbgError):
+        col.drift_step(f, 0.1, (0.0, 1.0, 1.0))                      # dx = 0
+    with pytest.raises(rbg.RbgError):
+        col.drift_step(f, 0.1, (1.0, 1.0, 1.0), bc=(2, 1, 1))
+    with pytest.raises(rbg.RbgError):
+        col.drift_step(f, 0.1, (1.0, 1.0, 1.0), bc=(0, 1, 1), zeta=1.5)
+    off = rbg.Collision(w["problem"], ix_offset=3)
+    with pytest.raises(rbg.RbgError, match="ghost"):
+        off.drift_step(f, 0.1, (1.0, 1.0, 1.0))
+    skew = dict(w["problem"], grids=[dict(n=[4, 4, 4], pmin=[-1.0, -1.0, -1.0], pmax=[2.0, 1.0, 1.0])])
+    with pytest.raises(rbg.RbgError, match="symmetric"):
+        rbg.Collision(skew).drift_step(f, 0.1, (1.0, 1.0, 1.0), bc=(0, 1, 1), zeta=0.5)
+    with pytest.raises(rbg.RbgError):
+        col.vlasov_step(f, 0.1, torch.zeros(2, dtype=torch.float64, device="cuda"), torch.zeros(3, dtype=torch.float64, device="cuda"))
