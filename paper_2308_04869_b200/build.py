@@ -15,7 +15,7 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 SOURCES = [PKG / "csrc" / "rbg.cu"]
-DEPS = SOURCES + [PKG / "csrc" / "rbg_kernels.cuh", ROOT / "include" / "rbg.h"]
+DEPS = SOURCES + [PKG / "csrc" / "rbg_kernels.cuh", PKG / "csrc" / "rbg_be_kernels.cuh", ROOT / "include" / "rbg.h"]
 LIB = PKG / "librbg.so"
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-fmad=false",
               "-Xcompiler", "-fPIC,-ffp-contract=off,-O2", "-shared", "--ptxas-options=-v", "-split-compile=0"]

@@ -488,6 +488,36 @@ struct DeviceGuard {
 };
 }  // namespace
 
+namespace {
+// Geometry of the persistent staged kernels (moments, Vlasov): shared memory is [head][1/E table][ring of stages].  A
+// stage is `group` consecutive spatial cells: at least one per team, an even number when np is odd (so that its byte
+// count is a multiple of 16), and 32 KB or more per copy where the domain allows it.
+struct StagedGeometry { int team, group, n_stages, lead, ctas; size_t smem; bool ok; };
+StagedGeometry staged_geometry(const rbg_handle* h, int s, const double* fs, size_t head) {
+    StagedGeometry g{};
+    const size_t np = h->np[s];
+    const int nyz = h->grids[s].n[1] * h->grids[s].n[2];
+    const size_t tab_bytes = (np * 8 + 127) & ~(size_t)127;
+    const size_t avail = (size_t)h->max_smem_optin > head + tab_bytes ? (size_t)h->max_smem_optin - head - tab_bytes : 0;
+    g.team = 32;
+    while (g.team < rbg::MOM_THREADS && g.team < nyz) g.team *= 2;
+    g.group = rbg::MOM_THREADS / g.team;
+    if ((np % 2) && (g.group % 2)) g.group *= 2;
+    while ((size_t)g.group * np * 8 < 32768 && (size_t)(2 * g.group) * np * 8 * 3 <= avail) g.group *= 2;
+    while (g.group > 1 && (size_t)g.group * np * 8 * 2 > avail) g.group /= 2;
+    if (g.group < rbg::MOM_THREADS / g.team) g.team = rbg::MOM_THREADS / g.group;          // fewer, larger teams
+    const size_t stage_bytes = ((size_t)g.group * np * 8 + 127) & ~(size_t)127;
+    g.n_stages = (int)std::min<size_t>(rbg::MOM_MAX_STAGES, avail / stage_bytes);
+    g.ok = g.n_stages >= 2;
+    // an odd leading cell puts the groups on 16-byte boundaries when the species block starts 8 bytes off one
+    g.lead = (reinterpret_cast<uintptr_t>(fs) % 16 != 0 && (np % 2)) ? 1 : 0;
+    g.smem = head + tab_bytes + (size_t)g.n_stages * stage_bytes;
+    const int n_units = (g.lead ? 1 : 0) + (h->nx - g.lead + g.group - 1) / g.group;
+    g.ctas = std::max(1, std::min(h->sm_count, n_units));
+    return g;
+}
+}  // namespace
+
 int rbg_moments(rbg_handle* h, const double* f_dev, double* M_dev, double* total_dev, double* em_dev, void* cuda_stream) {
     if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
     if (!f_dev || !M_dev) return fail(h, RBG_E_INVALID_ARG, "null buffer");
@@ -495,8 +525,20 @@ int rbg_moments(rbg_handle* h, const double* f_dev, double* M_dev, double* total
     DeviceGuard guard(h->device);
     h->last_launches = 0;
     for (int s = 0; s < h->n_species; ++s) {
-        rbg::moments_kernel<<<h->nx, 128, 0, st>>>(f_dev + h->sp_off[s], species_tables(h, s), h->nx,
-                                                   M_dev + (size_t)s * h->nx * rbg::N_MOMENTS);
+        const rbg::SpeciesTables tb = species_tables(h, s);
+        const double* fs = f_dev + h->sp_off[s];
+        double* Ms = M_dev + (size_t)s * h->nx * rbg::N_MOMENTS;
+        const int nyz = tb.n[1] * tb.n[2];
+        const size_t head = (64 + (2 * (rbg::MOM_THREADS / 32) * 16 + (size_t)tb.n[0]) * 8 + 127) & ~(size_t)127;
+        const StagedGeometry g = staged_geometry(h, s, fs, head);
+        if (!g.ok) return fail(h, RBG_E_UNSUPPORTED, "rbg_moments: two spatial cells of one species plus its 1/E table must fit in shared memory");
+        if (g.team >= nyz) {
+            RBG_CUDA(h, cudaFuncSetAttribute(rbg::moments_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
+            rbg::moments_kernel<1><<<g.ctas, rbg::MOM_THREADS, g.smem, st>>>(fs, tb, h->nx, Ms, g.group, g.n_stages, g.team, g.lead);
+        } else {
+            RBG_CUDA(h, cudaFuncSetAttribute(rbg::moments_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
+            rbg::moments_kernel<4><<<g.ctas, rbg::MOM_THREADS, g.smem, st>>>(fs, tb, h->nx, Ms, g.group, g.n_stages, g.team, g.lead);
+        }
         RBG_CUDA(h, cudaGetLastError());
         ++h->last_launches;
     }
@@ -531,10 +573,13 @@ int rbg_drift_step(rbg_handle* h, const double* f_dev, double* f_out_dev, const 
     cudaStream_t st = (cudaStream_t)cuda_stream;
     DeviceGuard guard(h->device);
     h->last_launches = 0;
-    dp.slab = 16;
+    dp.zseg = std::min(16, h->nxyz[2]);
+    dp.tile_y = std::min(8, h->nxyz[1]);
+    const long nzseg = (h->nxyz[2] + dp.zseg - 1) / dp.zseg, nyt = (h->nxyz[1] + dp.tile_y - 1) / dp.tile_y;
     for (int s = 0; s < h->n_species; ++s) {
-        const int nchunks = ((int)h->np[s] + 255) / 256;
-        const long grid = (long)nchunks * ((h->nx + dp.slab - 1) / dp.slab);
+        const long nchunks = ((long)h->np[s] + 255) / 256;
+        const long grid = nchunks * nzseg * dp.tile_y * h->nxyz[0] * nyt;
+        if (grid > 0x7fffffffL) return fail(h, RBG_E_UNSUPPORTED, "rbg_drift_step: grid too large");
         rbg::drift_upfd_kernel<<<(unsigned)grid, 256, 0, st>>>(f_dev + h->sp_off[s], f_out_dev + h->sp_off[s], species_tables(h, s), dp);
         RBG_CUDA(h, cudaGetLastError());
         ++h->last_launches;
@@ -552,11 +597,22 @@ int rbg_vlasov_step(rbg_handle* h, const double* f_dev, double* f_out_dev, doubl
     DeviceGuard guard(h->device);
     h->last_launches = 0;
     rbg::VlasovParams vp;
-    vp.dt = dt; vp.nx_cells = h->nx; vp.slab = 16; vp.E = E_dev; vp.B = B_dev;
+    vp.dt = dt; vp.nx_cells = h->nx; vp.E = E_dev; vp.B = B_dev;
     for (int s = 0; s < h->n_species; ++s) {
-        const int nchunks = ((int)h->np[s] + 255) / 256;
-        const long grid = (long)nchunks * ((h->nx + vp.slab - 1) / vp.slab);
-        rbg::vlasov_upfd_kernel<<<(unsigned)grid, 256, 0, st>>>(f_dev + h->sp_off[s], f_out_dev + h->sp_off[s], species_tables(h, s), vp);
+        const rbg::SpeciesTables tb = species_tables(h, s);
+        const double* fs = f_dev + h->sp_off[s];
+        double* os = f_out_dev + h->sp_off[s];
+        const int nyz = tb.n[1] * tb.n[2];
+        const size_t head = (64 + (size_t)tb.n[0] * 8 + 127) & ~(size_t)127;
+        const StagedGeometry g = staged_geometry(h, s, fs, head);
+        if (!g.ok) return fail(h, RBG_E_UNSUPPORTED, "rbg_vlasov_step: two spatial cells of one species plus its 1/E table must fit in shared memory");
+        if (g.team >= nyz) {
+            RBG_CUDA(h, cudaFuncSetAttribute(rbg::vlasov_upfd_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
+            rbg::vlasov_upfd_kernel<1><<<g.ctas, rbg::MOM_THREADS, g.smem, st>>>(fs, os, tb, vp, g.group, g.n_stages, g.team, g.lead);
+        } else {
+            RBG_CUDA(h, cudaFuncSetAttribute(rbg::vlasov_upfd_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
+            rbg::vlasov_upfd_kernel<4><<<g.ctas, rbg::MOM_THREADS, g.smem, st>>>(fs, os, tb, vp, g.group, g.n_stages, g.team, g.lead);
+        }
         RBG_CUDA(h, cudaGetLastError());
         ++h->last_launches;
     }

@@ -25,66 +25,165 @@ struct SpeciesTables {
 };
 
 // ---------------------------------------------------------------------------------------------------------------
-// Moments.  One CTA per (species, spatial cell).  Momentum integrals are midpoint sums, Int d3p -> Sum dp^3.
+// Moments.  Momentum integrals are midpoint sums, Int d3p -> Sum dp^3.
 // With g = f / E and q = |p|^2 + m^2 (so E f = q g):
 //   n = S f, T^{0k} = S p_k f, j^k = S p_k g, T^{ik} = S p_i p_k g, T^{00} = S q g.
 // A lane owns columns of fixed (ipy, ipz) and walks along ipx, so that only five running sums need the per-cell
 // arithmetic (X0 = S_x f, X1 = S_x px f, G0 = S_x g, G1 = S_x px g, G2 = S_x px^2 g); the p_y, p_z factors are applied
 // once per column.  Loads are coalesced across the lanes of a warp (consecutive (ipy, ipz)).
 // ---------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128)
-moments_kernel(const double* __restrict__ f_species, SpeciesTables tb, int nx_cells, double* __restrict__ M_species) {
-    __shared__ double red[4][N_MOMENTS];
-    const int ix = blockIdx.x;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-    const double* __restrict__ f = f_species + (size_t)ix * tb.np;
-    const double* __restrict__ iE = tb.iE;
-    const int nyz = tb.n[1] * tb.n[2];
-    const double msq = tb.mass * tb.mass;
-    double acc[N_MOMENTS];
+// Persistent kernel, one CTA of 512 threads per SM.  Shared memory holds the species' 1/E table (read for every spatial
+// cell) and a ring of stages; a stage is a group of consecutive spatial cells of f (contiguous in memory), filled by one
+// TMA bulk copy that completes on the stage's mbarrier while earlier stages are being reduced, so the bytes in flight
+// are set by the ring (64 KB and more per SM), not by registers or occupancy.  A group whose byte count or address is
+// not a multiple of 16 (an odd leading cell, the tail of the domain) is copied cooperatively with plain loads instead.
+// The cells of a stage are shared out among teams of `team` threads (a power of two, 32..512: about one thread per
+// (ipy, ipz) column), so small momentum grids keep every warp busy.
+enum { MOM_MAX_STAGES = 8, MOM_THREADS = 512 };
+
+// Sum of v[m] over the 32 lanes for 16 values at once: each step halves the number of values a lane carries, so the
+// whole reduction takes 8 + 4 + 2 + 1 + 1 shuffles instead of 16 x 5.  On return lane l (l < 16) holds the total of
+// value index rev4(l) (bit-reversed), see mom_slot().
+__device__ __forceinline__ double warp_reduce16(double (&v)[16], int lane) {
 #pragma unroll
-    for (int m = 0; m < N_MOMENTS; ++m) acc[m] = 0.0;
-    for (int c = warp * 32 + lane; c < nyz; c += nwarps * 32) {
-        const int iy = c / tb.n[2], iz = c - iy * tb.n[2];
-        const double py = fma((double)iy + 0.5, tb.delta[1], tb.pmin[1]);
-        const double pz = fma((double)iz + 0.5, tb.delta[2], tb.pmin[2]);
-        double X0 = 0.0, X1 = 0.0, G0 = 0.0, G1 = 0.0, G2 = 0.0;
-#pragma unroll 4
-        for (int i = 0; i < tb.n[0]; ++i) {
-            const double px = fma((double)i + 0.5, tb.delta[0], tb.pmin[0]);
-            const size_t j = (size_t)i * nyz + c;
-            const double a = __ldcs(f + j);              // streamed once
-            const double g = a * __ldg(iE + j);          // table shared by every spatial cell: L2-resident
-            const double pg = px * g;
-            X0 += a;
-            X1 = fma(px, a, X1);
-            G0 += g;
-            G1 += pg;
-            G2 = fma(px, pg, G2);
+    for (int half = 8, bit = 1; half >= 1; half >>= 1, bit <<= 1) {
+        const bool up = (lane & bit) != 0;
+#pragma unroll
+        for (int k = 0; k < half; ++k) {
+            const double send = up ? v[k] : v[k + half];
+            const double keep = up ? v[k + half] : v[k];
+            v[k] = keep + __shfl_xor_sync(0xffffffffu, send, bit);
         }
-        const double r = fma(py, py, fma(pz, pz, msq));                   // q - px^2
-        const double yG0 = py * G0, zG0 = pz * G0;
-        acc[0] += X0;                                                     // n
-        acc[1] += G1; acc[2] += yG0; acc[3] += zG0;                       // j
-        acc[4] += fma(r, G0, G2);                                         // T00 = S (px^2 + r) g
-        acc[5] += X1; acc[6] = fma(py, X0, acc[6]); acc[7] = fma(pz, X0, acc[7]);   // T0k
-        acc[8] += G2; acc[9] = fma(py, G1, acc[9]); acc[10] = fma(pz, G1, acc[10]); // Txx Txy Txz
-        acc[11] = fma(py, yG0, acc[11]); acc[12] = fma(py, zG0, acc[12]); acc[13] = fma(pz, zG0, acc[13]);
     }
-#pragma unroll
-    for (int m = 0; m < N_MOMENTS; ++m) {
-        double v = acc[m];
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-        if (lane == 0) red[warp][m] = v;
+    return v[0] + __shfl_xor_sync(0xffffffffu, v[0], 16);
+}
+// value index held by lane l after warp_reduce16: bit j of l selects the upper half at step j
+__device__ __forceinline__ int mom_slot(int l) { return ((l & 1) << 3) | ((l & 2) << 1) | ((l & 4) >> 1) | ((l & 8) >> 3); }
+
+// MOM_MAXC = columns a thread owns at a time (1 when the team covers the (ipy, ipz) plane)
+template <int MOM_MAXC>
+__global__ void __launch_bounds__(MOM_THREADS, 1)
+moments_kernel(const double* __restrict__ f_species, SpeciesTables tb, int nx_cells, double* __restrict__ M_species,
+               int group, int n_stages, int team, int lead) {
+    extern __shared__ __align__(128) unsigned char mom_smem[];
+    uint64_t* bars = reinterpret_cast<uint64_t*>(mom_smem);                             // MOM_MAX_STAGES mbarriers
+    double* red = reinterpret_cast<double*>(mom_smem + 64);                             // [2][16 warps][16]
+    double* px_tab = red + 2 * (MOM_THREADS / 32) * 16;                                 // p_x of the n[0] cell centres
+    const size_t head = (64 + (2 * (MOM_THREADS / 32) * 16 + (size_t)tb.n[0]) * 8 + 127) & ~(size_t)127;
+    double* iEs = reinterpret_cast<double*>(mom_smem + head);
+    const size_t np = (size_t)tb.np;
+    const size_t tab_bytes = (np * 8 + 127) & ~(size_t)127;
+    const size_t stage_bytes = ((size_t)group * np * 8 + 127) & ~(size_t)127;
+    unsigned char* ring = mom_smem + head + tab_bytes;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int nyz = tb.n[1] * tb.n[2];
+    // units: [0, lead) (if lead > 0), then groups of `group` cells
+    const int n_units = (lead ? 1 : 0) + (nx_cells - lead + group - 1) / group;
+    auto unit_first = [&](int u) { return lead ? (u == 0 ? 0 : lead + (u - 1) * group) : u * group; };
+    auto unit_cells = [&](int u) { return (lead && u == 0) ? lead : min(group, nx_cells - unit_first(u)); };
+    auto unit_tma = [&](int u) {
+        return ((size_t)unit_cells(u) * np * 8) % 16 == 0 && reinterpret_cast<uintptr_t>(f_species + (size_t)unit_first(u) * np) % 16 == 0;
+    };
+    auto arm = [&](int slot, int u) {
+        if (u < n_units && unit_tma(u)) {
+            const uint32_t bytes = (uint32_t)((size_t)unit_cells(u) * np * 8);
+            mbar_expect_tx(&bars[slot], bytes);
+            tma_bulk_g2s(ring + (size_t)slot * stage_bytes, f_species + (size_t)unit_first(u) * np, bytes, &bars[slot]);
+        }
+    };
+    if (threadIdx.x == 0) {
+        for (int k = 0; k < n_stages; ++k) mbar_init(&bars[k], 1);
+        fence_mbar_init();
+        for (int k = 0; k < n_stages; ++k) arm(k, blockIdx.x + k * gridDim.x);          // prologue: fill the ring
     }
+    for (int i = threadIdx.x; i < tb.n[0]; i += MOM_THREADS) px_tab[i] = fma((double)i + 0.5, tb.delta[0], tb.pmin[0]);
+    for (size_t j = threadIdx.x; j < np; j += MOM_THREADS) iEs[j] = __ldg(tb.iE + j);
     __syncthreads();
-    if (threadIdx.x < N_MOMENTS) {
-        double v = 0.0;
-        for (int w = 0; w < nwarps; ++w) v += red[w][threadIdx.x];
-        const double dp3 = tb.delta[0] * tb.delta[1] * tb.delta[2];
-        M_species[(size_t)ix * N_MOMENTS + threadIdx.x] = v * dp3;
+    const double msq = tb.mass * tb.mass;
+    const double dp3 = tb.delta[0] * tb.delta[1] * tb.delta[2];
+    const int n_teams = MOM_THREADS / team, my_team = threadIdx.x / team, t_in_team = threadIdx.x - my_team * team;
+    const int warps_per_team = team >> 5, warp_in_team = t_in_team >> 5;
+    int it = 0, flip = 0;
+    uint32_t phases = 0;                                       // bit k: parity of the next completion of stage k
+    for (int u = blockIdx.x; u < n_units; u += gridDim.x, ++it) {
+        const int slot = it % n_stages;
+        double* fs = reinterpret_cast<double*>(ring + (size_t)slot * stage_bytes);
+        const int cells = unit_cells(u), first = unit_first(u);
+        if (unit_tma(u)) {
+            mbar_wait(&bars[slot], (phases >> slot) & 1u);
+            phases ^= 1u << slot;
+        } else {
+            const double* src = f_species + (size_t)first * np;
+            for (size_t j = threadIdx.x; j < (size_t)cells * np; j += MOM_THREADS) fs[j] = __ldcs(src + j);
+            __syncthreads();
+        }
+        for (int cell0 = 0; cell0 < cells; cell0 += n_teams) {           // one round: every team reduces one cell
+            const int cell = cell0 + my_team;
+            const bool active = cell < cells;
+            const double* __restrict__ fc = fs + (size_t)(active ? cell : 0) * np;
+            double acc[16];
+#pragma unroll
+            for (int m = 0; m < 16; ++m) acc[m] = 0.0;
+            // a thread owns columns c = t_in_team + q * team of fixed (ipy, ipz) and walks along ipx
+            for (int c0 = t_in_team; active && c0 - lane < nyz; c0 += team * MOM_MAXC) {
+                double X0[MOM_MAXC], X1[MOM_MAXC], G0[MOM_MAXC], G1[MOM_MAXC], G2[MOM_MAXC];
+#pragma unroll
+                for (int q = 0; q < MOM_MAXC; ++q) { X0[q] = X1[q] = G0[q] = G1[q] = G2[q] = 0.0; }
+#pragma unroll
+                for (int q = 0; q < MOM_MAXC; ++q) {
+                    const int c = c0 + q * team;
+                    if (c < nyz) {
+                        const double* __restrict__ pf = fc + c;
+                        const double* __restrict__ pe = iEs + c;
+                        double x0 = 0.0, x1 = 0.0, g0 = 0.0, g1 = 0.0, g2 = 0.0;
+#pragma unroll 4
+                        for (int i = 0; i < tb.n[0]; ++i) {
+                            const double px = px_tab[i];
+                            const double a = pf[(size_t)i * nyz];
+                            const double g = a * pe[(size_t)i * nyz];
+                            const double pg = px * g;
+                            x0 += a;
+                            x1 = fma(px, a, x1);
+                            g0 += g;
+                            g1 += pg;
+                            g2 = fma(px, pg, g2);
+                        }
+                        X0[q] = x0; X1[q] = x1; G0[q] = g0; G1[q] = g1; G2[q] = g2;
+                    }
+                }
+#pragma unroll
+                for (int q = 0; q < MOM_MAXC; ++q) {
+                    const int c = c0 + q * team;
+                    if (c < nyz) {
+                        const int iy = c / tb.n[2], iz = c - iy * tb.n[2];
+                        const double py = fma((double)iy + 0.5, tb.delta[1], tb.pmin[1]);
+                        const double pz = fma((double)iz + 0.5, tb.delta[2], tb.pmin[2]);
+                        const double r = fma(py, py, fma(pz, pz, msq));                   // q - px^2
+                        const double yG0 = py * G0[q], zG0 = pz * G0[q];
+                        acc[0] += X0[q];                                                  // n
+                        acc[1] += G1[q]; acc[2] += yG0; acc[3] += zG0;                    // j
+                        acc[4] += fma(r, G0[q], G2[q]);                                   // T00 = S (px^2 + r) g
+                        acc[5] += X1[q]; acc[6] = fma(py, X0[q], acc[6]); acc[7] = fma(pz, X0[q], acc[7]);      // T0k
+                        acc[8] += G2[q]; acc[9] = fma(py, G1[q], acc[9]); acc[10] = fma(pz, G1[q], acc[10]);    // Txx Txy Txz
+                        acc[11] = fma(py, yG0, acc[11]); acc[12] = fma(py, zG0, acc[12]); acc[13] = fma(pz, zG0, acc[13]);
+                    }
+                }
+            }
+            const double tot = warp_reduce16(acc, lane);
+            double* rb = red + (size_t)flip * (MOM_THREADS / 32) * 16;
+            if (lane < 16) rb[warp * 16 + mom_slot(lane)] = tot;
+            __syncthreads();
+            if (active && t_in_team < N_MOMENTS) {
+                double v = 0.0;
+                for (int w = 0; w < warps_per_team; ++w) v += rb[(my_team * warps_per_team + w) * 16 + t_in_team];
+                M_species[((size_t)first + cell) * N_MOMENTS + t_in_team] = v * dp3;
+            }
+            flip ^= 1;                                         // the next round writes the other buffer: one barrier per round
+        }
+        __syncthreads();                                       // every team has finished reading the stage
+        if (threadIdx.x == 0) arm(slot, u + n_stages * gridDim.x);       // refill with the unit n_stages iterations ahead
     }
+    (void)warp_in_team;
 }
 
 // total[ix][m] = Sum_a M[a][ix][m] (Eq. 7, 9); em[ix][0..3] = Sum_a Q_a (n_a, j_a) (Eq. 15).  Either may be null.
@@ -118,17 +217,29 @@ struct DriftParams {
     int nxyz[3];
     int bc[3];               // 1 periodic, 0 wall with reflection probability zeta
     double zeta;
-    int slab;                // spatial cells per CTA
+    int zseg;                // cells of a z row per CTA
+    int tile_y;              // rows per y tile (CTA order: y tile, i_x, row in tile, z segment, momentum chunk)
 };
 
-__global__ void __launch_bounds__(256)
+enum { STENCIL_BATCH = 4 };  // spatial cells whose loads are issued together
+
+// CTA = (momentum chunk of 256 cells) x (segment of a z row).  CTAs are ordered so that consecutive CTAs walk along x
+// inside a tile of tile_y rows: the x neighbour of a cell was read tile_y * nz spatial cells earlier and is still in
+// L2 (for a 32^3 x 20^3 grid a whole x plane is 65 MB away in memory order, which L2 does not hold next to the output).
+__global__ void __launch_bounds__(256, 4)
 drift_upfd_kernel(const double* __restrict__ f_species, double* __restrict__ out_species, SpeciesTables tb, DriftParams dp) {
     const int nchunks = (tb.np + blockDim.x - 1) / blockDim.x;
-    const int chunk = blockIdx.x % nchunks, slab = blockIdx.x / nchunks;
+    const int nzseg = (dp.nxyz[2] + dp.zseg - 1) / dp.zseg;
+    int b = blockIdx.x;
+    const int chunk = b % nchunks; b /= nchunks;
+    const int zs = b % nzseg; b /= nzseg;
+    const int iy_in = b % dp.tile_y; b /= dp.tile_y;
+    const int ixx = b % dp.nxyz[0];
+    const int iy = (b / dp.nxyz[0]) * dp.tile_y + iy_in;
     const int ip = chunk * blockDim.x + threadIdx.x;
-    if (ip >= tb.np) return;
-    const int nx_cells = dp.nxyz[0] * dp.nxyz[1] * dp.nxyz[2];
-    const int ix_begin = slab * dp.slab, ix_end = min(ix_begin + dp.slab, nx_cells);
+    if (ip >= tb.np || iy >= dp.nxyz[1]) return;
+    const int z0 = zs * dp.zseg, z1 = min(z0 + dp.zseg, dp.nxyz[2]);
+    const ptrdiff_t np = tb.np;
     // per-momentum-cell constants
     double c[3];
     int sgn[3], mir[3];
@@ -148,80 +259,153 @@ drift_upfd_kernel(const double* __restrict__ f_species, double* __restrict__ out
         den += c[d];
     }
     const double rden = 1.0 / den;
+    // upwind neighbour along d of the spatial cell with index i along d: an interior or periodic neighbour (offset in
+    // spatial cells, weight c_d) or the wall ghost zeta * f(same cell, mirrored momentum)
     const int stride[3] = {dp.nxyz[1] * dp.nxyz[2], dp.nxyz[2], 1};
-    int i[3];
-    i[0] = ix_begin / stride[0]; i[1] = (ix_begin - i[0] * stride[0]) / stride[1]; i[2] = ix_begin - i[0] * stride[0] - i[1] * stride[1];
-    for (int ix = ix_begin; ix < ix_end; ++ix) {
-        const double* __restrict__ row = f_species + (size_t)ix * tb.np;
-        const double self = __ldg(row + ip);
-        double num = self * (1.0 / 3.0);
+    auto upwind = [&](int d, int i, ptrdiff_t& off, double& cs) {
+        const int j = i - sgn[d];
+        const bool inside = (unsigned)j < (unsigned)dp.nxyz[d];
+        const bool real = inside || dp.bc[d] == 1;
+        const int jn = inside ? j : (j < 0 ? dp.nxyz[d] - 1 : 0);
+        off = real ? (ptrdiff_t)((jn - i) * stride[d]) * np + ip : (ptrdiff_t)mir[d];
+        cs = real ? c[d] : c[d] * dp.zeta;
+    };
+    ptrdiff_t offx, offy;
+    double csx, csy;
+    upwind(0, ixx, offx, csx);
+    upwind(1, iy, offy, csy);
+    const size_t row0 = ((size_t)ixx * dp.nxyz[1] + iy) * dp.nxyz[2];
+    for (int zb = z0; zb < z1; zb += STENCIL_BATCH) {
+        double self[STENCIL_BATCH], ux[STENCIL_BATCH], uy[STENCIL_BATCH], uz[STENCIL_BATCH], csz[STENCIL_BATCH];
 #pragma unroll
-        for (int d = 0; d < 3; ++d) {
-            int j = i[d] - sgn[d];                           // upwind neighbour along d
-            double up;
-            if ((unsigned)j < (unsigned)dp.nxyz[d]) {
-                up = __ldg(row + (ptrdiff_t)(-sgn[d] * stride[d]) * tb.np + ip);
-            } else if (dp.bc[d] == 1) {
-                j = j < 0 ? dp.nxyz[d] - 1 : 0;
-                up = __ldg(row + (ptrdiff_t)((j - i[d]) * stride[d]) * tb.np + ip);
-            } else {
-                up = dp.zeta != 0.0 ? dp.zeta * __ldg(row + mir[d]) : 0.0;
-            }
-            num = fma(c[d], up, num);
+        for (int k = 0; k < STENCIL_BATCH; ++k) {
+            const int z = min(zb + k, z1 - 1);                       // the tail repeats the last cell (not stored)
+            const double* __restrict__ row = f_species + (row0 + z) * np;
+            ptrdiff_t offz;
+            upwind(2, z, offz, csz[k]);
+            self[k] = __ldg(row + ip);
+            ux[k] = __ldg(row + offx);
+            uy[k] = __ldg(row + offy);
+            uz[k] = __ldg(row + offz);
         }
-        out_species[(size_t)ix * tb.np + ip] = num * rden;
-        if (++i[2] == dp.nxyz[2]) { i[2] = 0; if (++i[1] == dp.nxyz[1]) { i[1] = 0; ++i[0]; } }
+#pragma unroll
+        for (int k = 0; k < STENCIL_BATCH; ++k) {
+            if (zb + k < z1) {
+                const double num = fma(csz[k], uz[k], fma(csy, uy[k], fma(csx, ux[k], self[k] * (1.0 / 3.0))));
+                __stcs(out_species + (row0 + zb + k) * np + ip, num * rden);
+            }
+        }
     }
 }
 
 struct VlasovParams {
     double dt;
     int nx_cells;
-    int slab;
     const double* E;         // [nx_cells][3]
     const double* B;         // [nx_cells][3]
 };
 
-__global__ void __launch_bounds__(256)
-vlasov_upfd_kernel(const double* __restrict__ f_species, double* __restrict__ out_species, SpeciesTables tb, VlasovParams vp) {
-    const int nchunks = (tb.np + blockDim.x - 1) / blockDim.x;
-    const int chunk = blockIdx.x % nchunks, slab = blockIdx.x / nchunks;
-    const int ip = chunk * blockDim.x + threadIdx.x;
-    if (ip >= tb.np) return;
-    const int ix_begin = slab * vp.slab, ix_end = min(ix_begin + vp.slab, vp.nx_cells);
-    // momentum neighbours of this cell, periodic: [d][0] at p_d - dp_d, [d][1] at p_d + dp_d
-    int nb[3][2];        // indexed with compile-time constants only (registers)
-    {
-        const int nyz = tb.n[1] * tb.n[2];
-        const int i0 = ip / nyz, i1 = (ip - i0 * nyz) / tb.n[2], i2 = ip - i0 * nyz - i1 * tb.n[2];
-        nb[0][0] = ip + (i0 > 0 ? -nyz : (tb.n[0] - 1) * nyz);
-        nb[0][1] = ip + (i0 < tb.n[0] - 1 ? nyz : -(tb.n[0] - 1) * nyz);
-        nb[1][0] = ip + (i1 > 0 ? -tb.n[2] : (tb.n[1] - 1) * tb.n[2]);
-        nb[1][1] = ip + (i1 < tb.n[1] - 1 ? tb.n[2] : -(tb.n[1] - 1) * tb.n[2]);
-        nb[2][0] = ip + (i2 > 0 ? -1 : tb.n[2] - 1);
-        nb[2][1] = ip + (i2 < tb.n[2] - 1 ? 1 : -(tb.n[2] - 1));
+// Vlasov step: the stencil lives inside the momentum block of one (species, spatial cell), so the block is staged in
+// shared memory exactly like in moments_kernel (persistent CTA, ring of TMA stages, 1/E table resident) and every
+// neighbour comes from shared memory: HBM sees f once in and f_out once out.  A thread owns (ipy, ipz) columns and walks
+// along ipx; v = p / E_p is rebuilt from the cell centre and the 1/E table; stores are coalesced across the lanes.
+template <int VL_MAXC>
+__global__ void __launch_bounds__(MOM_THREADS, 1)
+vlasov_upfd_kernel(const double* __restrict__ f_species, double* __restrict__ out_species, SpeciesTables tb, VlasovParams vp,
+                   int group, int n_stages, int team, int lead) {
+    extern __shared__ __align__(128) unsigned char mom_smem[];
+    uint64_t* bars = reinterpret_cast<uint64_t*>(mom_smem);
+    double* px_tab = reinterpret_cast<double*>(mom_smem + 64);
+    const size_t head = (64 + (size_t)tb.n[0] * 8 + 127) & ~(size_t)127;
+    double* iEs = reinterpret_cast<double*>(mom_smem + head);
+    const size_t np = (size_t)tb.np;
+    const size_t tab_bytes = (np * 8 + 127) & ~(size_t)127;
+    const size_t stage_bytes = ((size_t)group * np * 8 + 127) & ~(size_t)127;
+    unsigned char* ring = mom_smem + head + tab_bytes;
+    const int lane = threadIdx.x & 31;
+    const int nx_cells = vp.nx_cells;
+    const int nyz = tb.n[1] * tb.n[2], n0 = tb.n[0], n1 = tb.n[1], n2 = tb.n[2];
+    const int n_units = (lead ? 1 : 0) + (nx_cells - lead + group - 1) / group;
+    auto unit_first = [&](int u) { return lead ? (u == 0 ? 0 : lead + (u - 1) * group) : u * group; };
+    auto unit_cells = [&](int u) { return (lead && u == 0) ? lead : min(group, nx_cells - unit_first(u)); };
+    auto unit_tma = [&](int u) {
+        return ((size_t)unit_cells(u) * np * 8) % 16 == 0 && reinterpret_cast<uintptr_t>(f_species + (size_t)unit_first(u) * np) % 16 == 0;
+    };
+    auto arm = [&](int slot, int u) {
+        if (u < n_units && unit_tma(u)) {
+            const uint32_t bytes = (uint32_t)((size_t)unit_cells(u) * np * 8);
+            mbar_expect_tx(&bars[slot], bytes);
+            tma_bulk_g2s(ring + (size_t)slot * stage_bytes, f_species + (size_t)unit_first(u) * np, bytes, &bars[slot]);
+        }
+    };
+    if (threadIdx.x == 0) {
+        for (int k = 0; k < n_stages; ++k) mbar_init(&bars[k], 1);
+        fence_mbar_init();
+        for (int k = 0; k < n_stages; ++k) arm(k, blockIdx.x + k * gridDim.x);
     }
-    const double vx = __ldg(tb.v + ip), vy = __ldg(tb.v + (size_t)tb.np + ip), vz = __ldg(tb.v + 2 * (size_t)tb.np + ip);
+    for (int i = threadIdx.x; i < n0; i += MOM_THREADS) px_tab[i] = fma((double)i + 0.5, tb.delta[0], tb.pmin[0]);
+    for (size_t j = threadIdx.x; j < np; j += MOM_THREADS) iEs[j] = __ldg(tb.iE + j);
+    __syncthreads();
     const double k0 = vp.dt / tb.delta[0], k1 = vp.dt / tb.delta[1], k2 = vp.dt / tb.delta[2];
     const double Q = tb.charge;
-    for (int ix = ix_begin; ix < ix_end; ++ix) {
-        const double* __restrict__ row = f_species + (size_t)ix * tb.np;
-        const double* __restrict__ Ev = vp.E + (size_t)ix * 3;
-        const double* __restrict__ Bv = vp.B + (size_t)ix * 3;
-        const double Ex = __ldg(Ev), Ey = __ldg(Ev + 1), Ez = __ldg(Ev + 2);
-        const double Bx = __ldg(Bv), By = __ldg(Bv + 1), Bz = __ldg(Bv + 2);
-        // F = Q (E + v x B)
-        const double Fx = Q * (Ex + (vy * Bz - vz * By));
-        const double Fy = Q * (Ey + (vz * Bx - vx * Bz));
-        const double Fz = Q * (Ez + (vx * By - vy * Bx));
-        const double c0 = fabs(Fx) * k0, c1 = fabs(Fy) * k1, c2 = fabs(Fz) * k2;
-        const double self = __ldg(row + ip);
-        const double u0 = __ldg(row + (Fx > 0.0 ? nb[0][0] : nb[0][1]));
-        const double u1 = __ldg(row + (Fy > 0.0 ? nb[1][0] : nb[1][1]));
-        const double u2 = __ldg(row + (Fz > 0.0 ? nb[2][0] : nb[2][1]));
-        const double num = fma(c2, u2, fma(c1, u1, fma(c0, u0, self * (1.0 / 3.0))));
-        const double den = ((1.0 / 3.0 + c0) + c1) + c2;
-        out_species[(size_t)ix * tb.np + ip] = num / den;
+    const int n_teams = MOM_THREADS / team, my_team = threadIdx.x / team, t_in_team = threadIdx.x - my_team * team;
+    int it = 0;
+    uint32_t phases = 0;
+    for (int u = blockIdx.x; u < n_units; u += gridDim.x, ++it) {
+        const int slot = it % n_stages;
+        double* fs = reinterpret_cast<double*>(ring + (size_t)slot * stage_bytes);
+        const int cells = unit_cells(u), first = unit_first(u);
+        if (unit_tma(u)) {
+            mbar_wait(&bars[slot], (phases >> slot) & 1u);
+            phases ^= 1u << slot;
+        } else {
+            const double* src = f_species + (size_t)first * np;
+            for (size_t j = threadIdx.x; j < (size_t)cells * np; j += MOM_THREADS) fs[j] = __ldcs(src + j);
+            __syncthreads();
+        }
+        for (int cell = my_team; cell < cells; cell += n_teams) {
+            const double* __restrict__ fc = fs + (size_t)cell * np;
+            double* __restrict__ oc = out_species + ((size_t)first + cell) * np;
+            const double* __restrict__ Ev = vp.E + ((size_t)first + cell) * 3;
+            const double* __restrict__ Bv = vp.B + ((size_t)first + cell) * 3;
+            // F = Q (E + v x B) with Q folded into the fields of this spatial cell
+            const double QEx = Q * __ldg(Ev), QEy = Q * __ldg(Ev + 1), QEz = Q * __ldg(Ev + 2);
+            const double QBx = Q * __ldg(Bv), QBy = Q * __ldg(Bv + 1), QBz = Q * __ldg(Bv + 2);
+            for (int c0 = t_in_team; c0 - lane < nyz; c0 += team * VL_MAXC) {
+#pragma unroll
+                for (int q = 0; q < VL_MAXC; ++q) {
+                    const int c = c0 + q * team;
+                    if (c < nyz) {
+                        const int iy = c / n2, iz = c - iy * n2;
+                        const double py = fma((double)iy + 0.5, tb.delta[1], tb.pmin[1]);
+                        const double pz = fma((double)iz + 0.5, tb.delta[2], tb.pmin[2]);
+                        // periodic momentum neighbours of the column
+                        const int cym = iy > 0 ? c - n2 : c + (n1 - 1) * n2, cyp = iy < n1 - 1 ? c + n2 : c - (n1 - 1) * n2;
+                        const int czm = iz > 0 ? c - 1 : c + n2 - 1, czp = iz < n2 - 1 ? c + 1 : c - (n2 - 1);
+#pragma unroll 2
+                        for (int i = 0; i < n0; ++i) {
+                            const int base = i * nyz, j = base + c;
+                            const double iE = iEs[j];
+                            const double vx = px_tab[i] * iE, vy = py * iE, vz = pz * iE;
+                            const double Fx = fma(vy, QBz, fma(-vz, QBy, QEx));
+                            const double Fy = fma(vz, QBx, fma(-vx, QBz, QEy));
+                            const double Fz = fma(vx, QBy, fma(-vy, QBx, QEz));
+                            const double c0d = fabs(Fx) * k0, c1d = fabs(Fy) * k1, c2d = fabs(Fz) * k2;
+                            const int jxm = i > 0 ? j - nyz : j + (n0 - 1) * nyz, jxp = i < n0 - 1 ? j + nyz : j - (n0 - 1) * nyz;
+                            const double self = fc[j];
+                            const double u0 = fc[Fx > 0.0 ? jxm : jxp];
+                            const double u1 = fc[base + (Fy > 0.0 ? cym : cyp)];
+                            const double u2 = fc[base + (Fz > 0.0 ? czm : czp)];
+                            const double num = fma(c2d, u2, fma(c1d, u1, fma(c0d, u0, self * (1.0 / 3.0))));
+                            const double den = ((1.0 / 3.0 + c0d) + c1d) + c2d;
+                            __stcs(oc + j, num * rcp_fast(den));          // den >= 1/3: no range checks; ~1 ulp
+                        }
+                    }
+                }
+            }
+        }
+        __syncthreads();                                       // every team has finished reading the stage
+        if (threadIdx.x == 0) arm(slot, u + n_stages * gridDim.x);
     }
 }
 
