@@ -113,3 +113,79 @@ def test_fullsize_config2_tchannel_sampler():
         blk = C[offs[1]:offs[1] + nx * npc].view(nx, npc) / (dens * dens)[:, None]
         noise[sampler] = float(blk.std(0).mean())
     assert noise[1] < 0.2 * noise[0], noise
+
+
+def test_fullsize_config7_qgp_sampled_parity():
+    """Workload 7 (the paper's quark-gluon-plasma scenario, 21^3 x 11^3, 70 roles) at full size: the oracle recomputes
+    two spatial cells; every cell is finite and written."""
+    import paper_2308_04869_b200 as rbg
+    w = workloads.make(7)
+    col = rbg.Collision(w["problem"])
+    C = col.collision(torch.from_numpy(w["f"]).cuda(), w["n_samples"], w["seed"])
+    torch.cuda.synchronize()
+    assert col.last_launch_count() == 70
+    _check_cells(w, C.cpu().numpy(), (0, 9260), False)
+    assert bool(torch.isfinite(C).all())
+
+
+def test_fullsize_be_steps_config4_and_config7():
+    """NEXT-4 kernels at the sizes bench.py --path be times: sampled spatial cells against oracle/be_steps.py, plus
+    properties that hold at any size (positivity, particle number of a periodic drift / uniform-force Vlasov step,
+    totals = sum over species)."""
+    import paper_2308_04869_b200 as rbg
+    from oracle import be_steps as bs
+    for cfg, nxyz in ((4, (32, 32, 32)), (7, (21, 21, 21))):
+        w = workloads.make(cfg)
+        prob = w["problem"]
+        nx = prob["nx"]
+        for sp, q in zip(prob["species"], (-1.0, 1.0, 2.0, 0.5, -0.5, 0.3, 1.5)):
+            sp["charge"] = q
+        col = rbg.Collision(dict(prob, nx=nxyz))
+        f = torch.from_numpy(w["f"]).cuda()
+        offs, _ = workloads.f_layout(prob)
+        npcs = [int(np.prod(g["n"])) for g in prob["grids"]]
+        # ---- moments: three sampled cells per species against the oracle (moments are local in x)
+        M, tot, em = col.moments(f)
+        torch.cuda.synchronize()
+        Mh = M.cpu().numpy()
+        cells = [0, nx // 2 + 1, nx - 1]
+        sub = dict(prob, nx=len(cells))
+        fsub = np.concatenate([w["f"][o:o + nx * n].reshape(nx, n)[cells].reshape(-1) for o, n in zip(offs, npcs)])
+        M_ref, tot_ref, em_ref = bs.moments(sub, fsub)
+        scale = np.maximum(np.abs(M_ref[..., 0:1]), np.abs(M_ref[..., 4:5])) * 25.0
+        assert np.all(np.abs(Mh[:, cells] - M_ref) <= 1e-12 * scale)
+        assert torch.allclose(tot, M.sum(0), rtol=1e-13, atol=0)
+        # ---- Vlasov: same sampled cells (the stencil is local in x); uniform E only: particle number conserved
+        rng = np.random.default_rng(3)
+        E = rng.normal(size=(nx, 3)); B = rng.normal(size=(nx, 3))
+        out = col.vlasov_step(f, 0.01, torch.from_numpy(E).cuda(), torch.from_numpy(B).cuda())
+        torch.cuda.synchronize()
+        ref = bs.vlasov_upfd(sub, fsub, 0.01, E[cells], B[cells])
+        got = np.concatenate([out[o:o + nx * n].view(nx, n)[cells].reshape(-1).cpu().numpy() for o, n in zip(offs, npcs)])
+        assert np.all(np.abs(got - ref) <= 1e-14 * np.abs(ref))
+        assert bool((out > 0).all())
+        outE = col.vlasov_step(f, 0.01, torch.from_numpy(E).cuda(), torch.zeros_like(torch.from_numpy(B)).cuda())
+        for o, n in zip(offs, npcs):
+            a, b = f[o:o + nx * n].view(nx, n).sum(1), outE[o:o + nx * n].view(nx, n).sum(1)
+            assert torch.allclose(a, b, rtol=1e-12, atol=0)
+        # ---- drift, periodic: per momentum cell the particle number is conserved.  Oracle check: the 3 x 3 x nz block
+        # of rows (0..2, 0..2, :) run as its own periodic domain has the same x, y, z neighbours for its centre row
+        # (1, 1, :) as the full domain
+        dx = (0.5, 0.4, 0.3)
+        out = col.drift_step(f, 0.02, dx)
+        torch.cuda.synchronize()
+        assert bool((out > 0).all())
+        for o, n in zip(offs, npcs):
+            a, b = f[o:o + nx * n].view(nx, n).sum(0), out[o:o + nx * n].view(nx, n).sum(0)
+            assert torch.allclose(a, b, rtol=1e-12, atol=0)
+        nz = nxyz[2]
+        fsub = np.concatenate([w["f"][o:o + nx * n].reshape(*nxyz, n)[0:3, 0:3].reshape(-1) for o, n in zip(offs, npcs)])
+        ref = bs.drift_upfd(dict(prob, nx=9 * nz), fsub, (3, 3, nz), 0.02, dx)
+        o_sub = 0
+        for o, n in zip(offs, npcs):
+            r = ref[o_sub:o_sub + 9 * nz * n].reshape(3, 3, nz, n)[1, 1]
+            g = out[o:o + nx * n].view(*nxyz, n)[1, 1].cpu().numpy()
+            assert np.all(np.abs(g - r) <= 1e-14 * np.abs(r))
+            o_sub += 9 * nz * n
+        del f, out, outE, M, tot, em
+        torch.cuda.empty_cache()
