@@ -493,11 +493,11 @@ namespace {
 // stage is `group` consecutive spatial cells: at least one per team, an even number when np is odd (so that its byte
 // count is a multiple of 16), and 32 KB or more per copy where the domain allows it.
 struct StagedGeometry { int team, group, n_stages, lead, ctas; size_t smem; bool ok; };
-StagedGeometry staged_geometry(const rbg_handle* h, int s, const double* fs, size_t head) {
+StagedGeometry staged_geometry(const rbg_handle* h, int s, const double* fs, size_t head, bool table_in_smem) {
     StagedGeometry g{};
     const size_t np = h->np[s];
     const int nyz = h->grids[s].n[1] * h->grids[s].n[2];
-    const size_t tab_bytes = (np * 8 + 127) & ~(size_t)127;
+    const size_t tab_bytes = table_in_smem ? (np * 8 + 127) & ~(size_t)127 : 0;
     const size_t avail = (size_t)h->max_smem_optin > head + tab_bytes ? (size_t)h->max_smem_optin - head - tab_bytes : 0;
     g.team = 32;
     while (g.team < rbg::MOM_THREADS && g.team < nyz) g.team *= 2;
@@ -530,15 +530,21 @@ int rbg_moments(rbg_handle* h, const double* f_dev, double* M_dev, double* total
         double* Ms = M_dev + (size_t)s * h->nx * rbg::N_MOMENTS;
         const int nyz = tb.n[1] * tb.n[2];
         const size_t head = (64 + (2 * (rbg::MOM_THREADS / 32) * 16 + (size_t)tb.n[0]) * 8 + 127) & ~(size_t)127;
-        const StagedGeometry g = staged_geometry(h, s, fs, head);
-        if (!g.ok) return fail(h, RBG_E_UNSUPPORTED, "rbg_moments: two spatial cells of one species plus its 1/E table must fit in shared memory");
-        if (g.team >= nyz) {
-            RBG_CUDA(h, cudaFuncSetAttribute(rbg::moments_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
-            rbg::moments_kernel<1><<<g.ctas, rbg::MOM_THREADS, g.smem, st>>>(fs, tb, h->nx, Ms, g.group, g.n_stages, g.team, g.lead);
-        } else {
-            RBG_CUDA(h, cudaFuncSetAttribute(rbg::moments_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
-            rbg::moments_kernel<4><<<g.ctas, rbg::MOM_THREADS, g.smem, st>>>(fs, tb, h->nx, Ms, g.group, g.n_stages, g.team, g.lead);
-        }
+        // the 1/E table lives in shared memory when it fits next to two stages (measured: reading it through L1 and
+        // spending its shared memory on a third stage is slower, 0.73 vs 0.58 ms on config 4: the kernel is bound by the
+        // CTA's own instruction latency, the two-stage ring alone streams at 6.2 TB/s); otherwise it is read through L1
+        bool ie_smem = true;
+        StagedGeometry g = staged_geometry(h, s, fs, head, true);
+        if (!g.ok) { ie_smem = false; g = staged_geometry(h, s, fs, head, false); }
+        if (!g.ok) return fail(h, RBG_E_UNSUPPORTED, "rbg_moments: two spatial cells of one species must fit in shared memory");
+        auto launch = [&](auto kern) -> cudaError_t {
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem);
+            if (e != cudaSuccess) return e;
+            kern<<<g.ctas, rbg::MOM_THREADS, g.smem, st>>>(fs, tb, h->nx, Ms, g.group, g.n_stages, g.team, g.lead);
+            return cudaSuccess;
+        };
+        if (g.team >= nyz) RBG_CUDA(h, ie_smem ? launch(rbg::moments_kernel<1, true>) : launch(rbg::moments_kernel<1, false>));
+        else               RBG_CUDA(h, ie_smem ? launch(rbg::moments_kernel<4, true>) : launch(rbg::moments_kernel<4, false>));
         RBG_CUDA(h, cudaGetLastError());
         ++h->last_launches;
     }
@@ -604,7 +610,7 @@ int rbg_vlasov_step(rbg_handle* h, const double* f_dev, double* f_out_dev, doubl
         double* os = f_out_dev + h->sp_off[s];
         const int nyz = tb.n[1] * tb.n[2];
         const size_t head = (64 + (size_t)tb.n[0] * 8 + 127) & ~(size_t)127;
-        const StagedGeometry g = staged_geometry(h, s, fs, head);
+        const StagedGeometry g = staged_geometry(h, s, fs, head, true);
         if (!g.ok) return fail(h, RBG_E_UNSUPPORTED, "rbg_vlasov_step: two spatial cells of one species plus its 1/E table must fit in shared memory");
         if (g.team >= nyz) {
             RBG_CUDA(h, cudaFuncSetAttribute(rbg::vlasov_upfd_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));

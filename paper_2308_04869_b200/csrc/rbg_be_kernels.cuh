@@ -61,7 +61,8 @@ __device__ __forceinline__ double warp_reduce16(double (&v)[16], int lane) {
 __device__ __forceinline__ int mom_slot(int l) { return ((l & 1) << 3) | ((l & 2) << 1) | ((l & 4) >> 1) | ((l & 8) >> 3); }
 
 // MOM_MAXC = columns a thread owns at a time (1 when the team covers the (ipy, ipz) plane)
-template <int MOM_MAXC>
+// IE_SMEM: the 1/E table is copied to shared memory; when it does not fit next to two stages it is read through L1.
+template <int MOM_MAXC, bool IE_SMEM>
 __global__ void __launch_bounds__(MOM_THREADS, 1)
 moments_kernel(const double* __restrict__ f_species, SpeciesTables tb, int nx_cells, double* __restrict__ M_species,
                int group, int n_stages, int team, int lead) {
@@ -70,9 +71,9 @@ moments_kernel(const double* __restrict__ f_species, SpeciesTables tb, int nx_ce
     double* red = reinterpret_cast<double*>(mom_smem + 64);                             // [2][16 warps][16]
     double* px_tab = red + 2 * (MOM_THREADS / 32) * 16;                                 // p_x of the n[0] cell centres
     const size_t head = (64 + (2 * (MOM_THREADS / 32) * 16 + (size_t)tb.n[0]) * 8 + 127) & ~(size_t)127;
-    double* iEs = reinterpret_cast<double*>(mom_smem + head);
     const size_t np = (size_t)tb.np;
-    const size_t tab_bytes = (np * 8 + 127) & ~(size_t)127;
+    const size_t tab_bytes = IE_SMEM ? (np * 8 + 127) & ~(size_t)127 : 0;
+    const double* __restrict__ iEs = IE_SMEM ? reinterpret_cast<const double*>(mom_smem + head) : tb.iE;
     const size_t stage_bytes = ((size_t)group * np * 8 + 127) & ~(size_t)127;
     unsigned char* ring = mom_smem + head + tab_bytes;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -97,7 +98,10 @@ moments_kernel(const double* __restrict__ f_species, SpeciesTables tb, int nx_ce
         for (int k = 0; k < n_stages; ++k) arm(k, blockIdx.x + k * gridDim.x);          // prologue: fill the ring
     }
     for (int i = threadIdx.x; i < tb.n[0]; i += MOM_THREADS) px_tab[i] = fma((double)i + 0.5, tb.delta[0], tb.pmin[0]);
-    for (size_t j = threadIdx.x; j < np; j += MOM_THREADS) iEs[j] = __ldg(tb.iE + j);
+    if (IE_SMEM) {
+        double* dst = reinterpret_cast<double*>(mom_smem + head);
+        for (size_t j = threadIdx.x; j < np; j += MOM_THREADS) dst[j] = __ldg(tb.iE + j);
+    }
     __syncthreads();
     const double msq = tb.mass * tb.mass;
     const double dp3 = tb.delta[0] * tb.delta[1] * tb.delta[2];
@@ -140,7 +144,7 @@ moments_kernel(const double* __restrict__ f_species, SpeciesTables tb, int nx_ce
                         for (int i = 0; i < tb.n[0]; ++i) {
                             const double px = px_tab[i];
                             const double a = pf[(size_t)i * nyz];
-                            const double g = a * pe[(size_t)i * nyz];
+                            const double g = a * (IE_SMEM ? pe[(size_t)i * nyz] : __ldg(pe + (size_t)i * nyz));
                             const double pg = px * g;
                             x0 += a;
                             x1 = fma(px, a, x1);
