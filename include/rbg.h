@@ -175,6 +175,20 @@ int rbg_drift_step(rbg_handle* h, const double* f_dev, double* f_out_dev, const 
 int rbg_vlasov_step(rbg_handle* h, const double* f_dev, double* f_out_dev, double dt, const double* E_dev,
                     const double* B_dev, void* cuda_stream);
 
+/* One time step dt of the Boltzmann equation by the paper's splitting, Eq. 25-27 ("solving the BE is
+ * equivalent to solving above three equations"), in the order drift, Vlasov, collision (the paper does not state an
+ * order; reading R24):
+ *     f <- rbg_drift_step(f, dt)                       Eq. 25 / 30      (if do_drift)
+ *     f <- rbg_vlasov_step(f, dt, E, B)                Eq. 26 / 34      (if do_vlasov; E_dev, B_dev as above)
+ *     f <- f + 3 dt C[f]  (rbg_collision_update)       Eq. 27: (1/3) df/dt = C   (if do_collision; n_samples, seed)
+ * in place: on return (stream order) f_dev holds the new state; scratch_dev (rbg_f_elems() doubles, caller-owned, not
+ * overlapping f_dev) is clobbered.  *neg_flag_dev accumulates the cells the collision update left negative (may be
+ * NULL when do_collision == 0).  All launches go to cuda_stream back to back (capturable in a CUDA graph). */
+typedef struct { double dt; double dx[3]; int bc[3]; double zeta; int n_samples; uint64_t seed;
+                 int do_drift, do_vlasov, do_collision; } rbg_be_step_params;
+int rbg_be_step(rbg_handle* h, double* f_dev, double* scratch_dev, const rbg_be_step_params* p, const double* E_dev,
+                const double* B_dev, int* neg_flag_dev, void* cuda_stream);
+
 /* Number of doubles in f / C / f_out. */
 size_t rbg_f_elems(const rbg_handle* h);
 /* Number of roles (a process seen from one grid species; a+b with a != b gives two). */

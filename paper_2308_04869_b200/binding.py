@@ -38,6 +38,12 @@ class _DriftParams(C.Structure):
     _fields_ = [("dt", C.c_double), ("dx", C.c_double * 3), ("bc", C.c_int * 3), ("zeta", C.c_double)]
 
 
+class _BeStepParams(C.Structure):
+    _fields_ = [("dt", C.c_double), ("dx", C.c_double * 3), ("bc", C.c_int * 3), ("zeta", C.c_double),
+                ("n_samples", C.c_int), ("seed", C.c_uint64), ("do_drift", C.c_int), ("do_vlasov", C.c_int),
+                ("do_collision", C.c_int)]
+
+
 N_MOMENTS = 14
 
 
@@ -59,6 +65,7 @@ _SIGNATURES = {
     "rbg_moments": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "rbg_drift_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "rbg_vlasov_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "rbg_be_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "rbg_f_elems": (C.c_size_t, [C.c_void_p]),
     "rbg_n_roles": (C.c_int, [C.c_void_p]),
     "rbg_sample_evals": (C.c_uint64, [C.c_void_p, C.c_int]),
@@ -245,6 +252,21 @@ class Collision:
                                               C.c_void_p(E.data_ptr()), C.c_void_p(B.data_ptr()), _stream_ptr(stream)),
                self._h)
         return out
+
+    def be_step(self, f, dt: float, dx=(1.0, 1.0, 1.0), bc=(1, 1, 1), zeta: float = 0.0, E=None, B=None, n_samples: int = 0,
+                seed: int = 0, drift=True, vlasov=True, collision=True, scratch=None, neg_flag=None, stream=None):
+        """rbg_be_step: one time step of Eq. 25-27 in place (drift, Vlasov, collision with 3 dt)."""
+        import torch
+        if scratch is None:
+            scratch = torch.empty_like(f)
+        if neg_flag is None:
+            neg_flag = torch.zeros(1, dtype=torch.int32, device=f.device)
+        p = _BeStepParams(float(dt), (C.c_double * 3)(*[float(v) for v in dx]), (C.c_int * 3)(*[int(v) for v in bc]),
+                          float(zeta), int(n_samples), int(seed), int(bool(drift)), int(bool(vlasov)), int(bool(collision)))
+        ptr = lambda t: C.c_void_p(t.data_ptr()) if t is not None else None
+        _check(load_library().rbg_be_step(self._h, self._dev(f, "f"), self._dev(scratch, "scratch"), C.byref(p), ptr(E), ptr(B),
+                                          C.c_void_p(neg_flag.data_ptr()), _stream_ptr(stream)), self._h)
+        return f, neg_flag
 
     def collision_host(self, f_host, n_samples: int, seed: int, out=None):
         """rbg_collision_host: host buffers in, host buffers out (numpy float64 or pinned CPU tensors)."""

@@ -625,6 +625,37 @@ int rbg_vlasov_step(rbg_handle* h, const double* f_dev, double* f_out_dev, doubl
     return RBG_OK;
 }
 
+int rbg_be_step(rbg_handle* h, double* f_dev, double* scratch_dev, const rbg_be_step_params* p, const double* E_dev,
+                const double* B_dev, int* neg_flag_dev, void* cuda_stream) {
+    if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
+    if (!f_dev || !scratch_dev || !p) return fail(h, RBG_E_INVALID_ARG, "null argument");
+    const size_t bytes = h->f_elems * sizeof(double);
+    const char *a = (const char*)f_dev, *b = (const char*)scratch_dev;
+    if (a < b + bytes && b < a + bytes) return fail(h, RBG_E_INVALID_ARG, "scratch_dev overlaps f_dev");
+    if (p->do_vlasov && (!E_dev || !B_dev)) return fail(h, RBG_E_INVALID_ARG, "do_vlasov needs E_dev and B_dev");
+    if (p->do_collision && !neg_flag_dev) return fail(h, RBG_E_INVALID_ARG, "do_collision needs neg_flag_dev");
+    double *cur = f_dev, *nxt = scratch_dev;
+    int launches = 0, rc;
+    if (p->do_drift) {
+        rbg_drift_params dp;
+        dp.dt = p->dt; dp.zeta = p->zeta;
+        for (int d = 0; d < 3; ++d) { dp.dx[d] = p->dx[d]; dp.bc[d] = p->bc[d]; }
+        if ((rc = rbg_drift_step(h, cur, nxt, &dp, cuda_stream)) != RBG_OK) return rc;
+        launches += h->last_launches; std::swap(cur, nxt);
+    }
+    if (p->do_vlasov) {
+        if ((rc = rbg_vlasov_step(h, cur, nxt, p->dt, E_dev, B_dev, cuda_stream)) != RBG_OK) return rc;
+        launches += h->last_launches; std::swap(cur, nxt);
+    }
+    if (p->do_collision) {
+        if ((rc = run(h, cur, nxt, true, 3.0 * p->dt, neg_flag_dev, p->n_samples, p->seed, cuda_stream)) != RBG_OK) return rc;
+        launches += h->last_launches; std::swap(cur, nxt);
+    }
+    if (cur != f_dev) RBG_CUDA(h, cudaMemcpyAsync(f_dev, cur, bytes, cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
+    h->last_launches = launches;
+    return RBG_OK;
+}
+
 int rbg_selftest_math(uint64_t n_operands, uint32_t seed, uint64_t* mismatches) {
     if (!mismatches) return fail(nullptr, RBG_E_INVALID_ARG, "null argument");
     unsigned long long* d = nullptr;

@@ -118,3 +118,38 @@ def test_be_step_argument_errors():
         rbg.Collision(skew).drift_step(f, 0.1, (1.0, 1.0, 1.0), bc=(0, 1, 1), zeta=0.5)
     with pytest.raises(rbg.RbgError):
         col.vlasov_step(f, 0.1, torch.zeros(2, dtype=torch.float64, device="cuda"), torch.zeros(3, dtype=torch.float64, device="cuda"))
+
+
+def test_be_step_is_drift_then_vlasov_then_collision_with_3dt():
+    """rbg_be_step against the composition of the three oracles (Eq. 25-27; order: DESIGN.md reading R24)."""
+    import oracle
+    from test_gpu_parity import oracle_C_and_scale
+    rbg = _rbg()
+    nxyz = (3, 2, 2)
+    w = workloads.make(2, nx=12, np_side=6, n_samples=48)
+    prob = w["problem"]
+    rng = np.random.default_rng(4)
+    E = rng.normal(size=(12, 3)); B = rng.normal(size=(12, 3))
+    dt, dx = 0.004, (0.5, 0.7, 0.9)
+    f1 = bs.drift_upfd(prob, w["f"], nxyz, dt, dx, bc=(1, 0, 1), zeta=0.5)
+    f2 = bs.vlasov_upfd(prob, f1, dt, E, B)
+    orc = oracle.Oracle(prob)
+    C_ref, mag = oracle_C_and_scale(orc, f2, 48, 777)
+    ref, neg_ref = oracle.update(f2, C_ref, 3 * dt)
+    col = rbg.Collision(_with_grid(prob, nxyz))
+    f = torch.from_numpy(w["f"]).cuda()
+    out, flag = col.be_step(f, dt, dx=dx, bc=(1, 0, 1), zeta=0.5, E=torch.from_numpy(E).cuda(), B=torch.from_numpy(B).cuda(),
+                            n_samples=48, seed=777)
+    torch.cuda.synchronize()
+    assert out.data_ptr() == f.data_ptr()
+    got = out.cpu().numpy()
+    assert np.all(np.abs(got - ref) <= 3 * dt * 1e-10 * mag + 1e-13 * np.abs(ref))
+    assert int(flag.item()) == neg_ref
+    assert col.last_launch_count() == 2 + 2 + 4
+    # sub-steps can be switched off; two of them leave the result in f as well
+    g = torch.from_numpy(w["f"]).cuda()
+    col.be_step(g, dt, dx=dx, bc=(1, 0, 1), zeta=0.5, collision=False, E=torch.from_numpy(E).cuda(), B=torch.from_numpy(B).cuda())
+    torch.cuda.synchronize()
+    assert np.all(np.abs(g.cpu().numpy() - f2) <= 1e-13 * np.abs(f2))
+    with pytest.raises(rbg.RbgError):
+        col.be_step(g, dt, dx=dx, E=None, B=None)

@@ -154,7 +154,7 @@ def test_fullsize_be_steps_config4_and_config7():
         M_ref, tot_ref, em_ref = bs.moments(sub, fsub)
         scale = np.maximum(np.abs(M_ref[..., 0:1]), np.abs(M_ref[..., 4:5])) * 25.0
         assert np.all(np.abs(Mh[:, cells] - M_ref) <= 1e-12 * scale)
-        assert torch.allclose(tot, M.sum(0), rtol=1e-13, atol=0)
+        assert bool(((tot - M.sum(0)).abs() <= 1e-13 * M.abs().sum(0)).all())
         # ---- Vlasov: same sampled cells (the stencil is local in x); uniform E only: particle number conserved
         rng = np.random.default_rng(3)
         E = rng.normal(size=(nx, 3)); B = rng.normal(size=(nx, 3))
