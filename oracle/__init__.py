@@ -87,6 +87,7 @@ def lib():
                                           dp, C.c_void_p, C.c_void_p, C.c_int]
         L.orc_trace.argtypes = [C.c_void_p, dp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_uint64, dp,
                                 C.POINTER(C.c_int), C.c_void_p, C.c_void_p, C.c_int]
+        L.orc_collision_symmetric.argtypes = [C.c_void_p, dp, dp, dp, C.c_int, C.c_uint64, C.c_int, C.c_int, C.c_int, C.c_int]
         L.orc_m2_qcd.restype = C.c_double
         L.orc_m2_qcd.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_double]
         L.orc_update.restype = C.c_long
@@ -196,6 +197,20 @@ class Oracle:
         if rc != 0:
             raise ValueError("oracle: bad arguments")
         return (Cout, d) if detail else Cout
+
+    def collision_symmetric(self, f, n_samples, seed, ix_begin=0, ix_end=None, ix_stride=1, slot_mask=15):
+        """NEXT-3: the conservative ("symmetric") estimator (rbg_oracle.cpp, SymSink).  Returns (C, mag): mag is the sum
+        of the absolute deposits per cell, the scale of the parity tolerance.  slot_mask (tests): deposit only for the
+        slots whose bit is set, to isolate one slot's estimator."""
+        f = np.ascontiguousarray(f, dtype=np.float64)
+        assert f.size == self.f_elems
+        Cout, mag = np.zeros(self.f_elems), np.zeros(self.f_elems)
+        ix_end = self.nx if ix_end is None else ix_end
+        rc = lib().orc_collision_symmetric(self._h, _dp(f), _dp(Cout), _dp(mag), int(n_samples), int(seed), ix_begin, ix_end,
+                                           ix_stride, int(slot_mask))
+        if rc != 0:
+            raise ValueError("oracle: bad arguments")
+        return Cout, mag
 
     def point(self, f, role, ix, ip1, n_samples, seed, fcb=None, box_cut=True):
         """Scaled (G, L, Lin, Q) of one (role, ix, p1); C_role = G - L, stderr = sqrt(Q - (G-L)^2/N)."""

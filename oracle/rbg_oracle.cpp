@@ -102,7 +102,7 @@ enum Kind { M2_CONST = 0, M2_COULOMB_SCREENED = 1, M2_TCHAN_S2 = 2,
 // about the CM direction of particle 1 drawn from the t-channel shape 1/(t - mD^2)^2 by its inverse CDF
 // (steps S1..S7 below), azimuth uniform.  Both estimate the same integral (R).
 enum Sampler { SAMPLER_UNIFORM = 0, SAMPLER_TCHANNEL = 1 };
-struct Role { int s[4]; int kind; double par[4]; double sym; int process; int sampler; double gab; };
+struct Role { int s[4]; int kind; double par[4]; double sym; int process; int sampler; double gab; double sym_override; };
 
 typedef double (*FCallback)(int species, const double* p, void* user);
 
@@ -236,7 +236,19 @@ template <typename R> inline R dot3(const R* a, const R* b) {
     return rfma<R>(a[2], b[2], rfma<R>(a[1], b[1], a[0] * b[0]));
 }
 
-struct Accum { double G = 0, Ls = 0, Lin = 0, Q = 0, D = 0; };   // D: float chain's sum of (float)(w gain - w loss)
+struct Accum { double G = 0, Ls = 0, Lin = 0, Q = 0, D = 0; };
+
+// NEXT-3, "symmetric" (conservative) sampling -- PAPER.md:257 names "the symmetric sampling method [57]" for the
+// collision term but does not define it and Ref. [57] is not part of PAPER.md: PARITY UNPINNED BY THE REFERENCE
+// (reading R25).  The reading implemented: every Monte Carlo sample is one sampled reaction 1+2 <-> 3+4
+// with net rate q = pref0 * w (gain - loss); instead of crediting it to the grid particle alone it is credited to all
+// four particles, +q to the cells of 1 and 2 and -q to the cells of 3 and 4, so that what one cell gains another
+// loses, sample by sample.  Each of the four deposits is by itself an unbiased estimator of the collision term of
+// its slot's species (two-body phase space is symmetric under (1,2) <-> (3,4)), so C of a species is their average.
+// fac[k] = sigma_k * sym_k * (dp^3 of species 1 / dp^3 of slot k's species) / m, with sigma = (+,+,-,-), sym_k the
+// symmetry factor seen from slot k (1/2 iff the opposite pair is one species) and m the number of (role, slot) pairs
+// of the process that carry the slot's species.
+struct SymSink { double* C; double* mag; double fac[4]; };   // D: float chain's sum of (float)(w gain - w loss)
 
 template <typename R>
 struct Evaluator {
@@ -338,7 +350,7 @@ struct Evaluator {
     // One p1: N samples.  The f value of species s, spatial cell ix, momentum cell j is
     // f_all[sp_off[s] + ix*np[s] + j] (layout of DESIGN.md section 5).
     void eval_p1(const double* f_all, int ix, int ip1, int N, uint64_t seed, Accum& acc, Trace* trace,
-                 int trace_n) const {
+                 int trace_n, const SymSink* sink = nullptr) const {
         const uint32_t key0 = (uint32_t)seed, key1 = (uint32_t)(seed >> 32);
         // species table base pointers at this spatial cell (index = sp_off[s] + ix*np[s])
         auto fval = [&](int slot, int cell, const R* p) -> R {
@@ -505,6 +517,25 @@ struct Evaluator {
                 if (std::is_same<R, float>::value) acc.D += (double)(w * gain - w * loss);
                 if (j3 >= 0 && j4 >= 0) acc.Lin += wl;
                 acc.Q += (wg - wl) * (wg - wl);
+                if (sink) {
+                    // pref0 = V2 / (16 pi E1 N): the O13 prefactor without the symmetry factor
+                    const Grid& g2 = H.grid[role.s[1]];
+                    const double V2 = (g2.pmax[0] - g2.pmin[0]) * (g2.pmax[1] - g2.pmin[1]) * (g2.pmax[2] - g2.pmin[2]);
+                    const double pref0 = V2 / (16.0 * M_PI * (double)E1 * (double)N);
+                    const double val = std::is_same<R, float>::value ? (double)(w * gain - w * loss) : wg - wl;
+                    const int jc[4] = {ip1, j2, j3, j4};
+                    for (int k4 = 0; k4 < 4; ++k4) {
+                        if (jc[k4] < 0) continue;                      // left the momentum box: lost from the system
+                        const int sk = role.s[k4];
+                        const size_t idx = H.sp_off[sk] + (size_t)ix * H.np[sk] + (size_t)jc[k4];
+                        const double d = sink->fac[k4] * (pref0 * val);
+                        const double m = std::fabs(sink->fac[k4]) * (pref0 * (std::fabs(wg) + std::fabs(wl)));
+#pragma omp atomic
+                        sink->C[idx] += d;
+#pragma omp atomic
+                        sink->mag[idx] += m;
+                    }
+                }
             } while (false);
             if (want) {
                 for (int d = 0; d < 3; ++d) { tr.p1[d] = p1[d]; tr.p2[d] = p2[d]; tr.p3[d] = p3[d]; tr.p4[d] = p4[d]; }
@@ -622,6 +653,7 @@ void* orc_create(int nx, int n_species, const Species* sp, const Grid* grid, int
         if (p.sampler == SAMPLER_TCHANNEL && !(elastic && (p.kind == M2_COULOMB_SCREENED || p.kind == M2_TCHAN_S2) && p.par[1] != 0.0)) { delete H; return nullptr; }
         Role r; r.kind = p.kind; std::memcpy(r.par, p.par, sizeof r.par); r.process = i; r.sampler = p.sampler;
         r.gab = sp[p.a].g * sp[p.b].g;
+        r.sym_override = p.sym;
         auto add = [&](int s1, int s2, int s3, int s4) {
             r.s[0] = s1; r.s[1] = s2; r.s[2] = s3; r.s[3] = s4;
             r.sym = p.sym < 0 ? (s3 == s4 ? 0.5 : 1.0) : p.sym;
@@ -671,6 +703,50 @@ int orc_collision(void* h, const double* f, double* C, int n_samples, uint64_t s
     if (H->use_float)
         return run_collision<float>(*H, f, C, n_samples, seed, ix_begin, ix_end, ix_stride, dG, dL, dLin, dQ, fcb, user, box_cut);
     return run_collision<double>(*H, f, C, n_samples, seed, ix_begin, ix_end, ix_stride, dG, dL, dLin, dQ, fcb, user, box_cut);
+}
+
+// NEXT-3: the conservative ("symmetric") estimator, see SymSink.  C and mag (sum of the absolute deposits, the scale
+// of the parity tolerance) have orc_f_elems doubles; the visited spatial cells are overwritten.
+// slot_mask (tests only; 15 = the estimator proper): bit k set = deposit for slot k+1; the multiplicity m then counts only
+// the (role, slot) pairs in the mask, so that a single-slot mask isolates that slot's estimator of its species' C.
+int orc_collision_symmetric(void* h, const double* f, double* C, double* mag, int n_samples, uint64_t seed, int ix_begin,
+                            int ix_end, int ix_stride, int slot_mask) {
+    Handle* H = (Handle*)h;
+    if (n_samples <= 0 || ix_begin < 0 || ix_end > H->nx || ix_stride <= 0) return -1;
+    for (size_t s = 0; s < H->sp.size(); ++s)
+        for (int ix = ix_begin; ix < ix_end; ix += ix_stride)
+            for (size_t j = 0; j < H->np[s]; ++j) { C[H->sp_off[s] + (size_t)ix * H->np[s] + j] = 0.0; mag[H->sp_off[s] + (size_t)ix * H->np[s] + j] = 0.0; }
+    auto dp3 = [&](int s) {
+        const Grid& g = H->grid[s];
+        return ((g.pmax[0] - g.pmin[0]) / g.n[0]) * ((g.pmax[1] - g.pmin[1]) / g.n[1]) * ((g.pmax[2] - g.pmin[2]) / g.n[2]);
+    };
+    for (int ir = 0; ir < (int)H->roles.size(); ++ir) {
+        const Role& role = H->roles[ir];
+        SymSink sink; sink.C = C; sink.mag = mag;
+        for (int k = 0; k < 4; ++k) {
+            int m = 0;                                  // (role, slot) pairs of this process carrying species s_k
+            for (const Role& r2 : H->roles)
+                if (r2.process == role.process)
+                    for (int k2 = 0; k2 < 4; ++k2) m += ((slot_mask >> k2) & 1) && r2.s[k2] == role.s[k];
+            const int oa = k < 2 ? 2 : 0;               // the opposite pair
+            const double symk = role.sym_override >= 0 ? role.sym_override : (role.s[oa] == role.s[oa + 1] ? 0.5 : 1.0);
+            sink.fac[k] = ((slot_mask >> k) & 1) ? (k < 2 ? 1.0 : -1.0) * symk * (dp3(role.s[0]) / dp3(role.s[k])) / (double)m : 0.0;
+        }
+        const long np1 = (long)H->np[role.s[0]];
+        const long ncell = (ix_end - ix_begin + ix_stride - 1) / ix_stride;
+        auto body = [&](auto tag) {
+            using R = decltype(tag);
+            Evaluator<R> ev(*H, ir, nullptr, nullptr, 1);
+#pragma omp parallel for schedule(static)
+            for (long idx = 0; idx < ncell * np1; ++idx) {
+                const int ix = ix_begin + (int)(idx / np1) * ix_stride;
+                Accum acc;
+                ev.eval_p1(f, ix, (int)(idx % np1), n_samples, seed, acc, nullptr, -1, &sink);
+            }
+        };
+        if (H->use_float) body(float()); else body(double());
+    }
+    return 0;
 }
 
 // One p1 only (analytic or grid mode): returns scaled G, Ls, Lin, Q for (role, ix, ip1).
