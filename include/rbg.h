@@ -142,6 +142,16 @@ int rbg_collision_update(rbg_handle* h, const double* f_dev, double* f_out_dev, 
 int rbg_collision_evolve(rbg_handle* h, double* f_dev, double* scratch_dev, double dt, int n_steps,
                          int* neg_flag_dev, int n_samples, uint64_t seed, void* cuda_stream);
 
+/* NEXT-3: the conservative ("symmetric") estimator of the same collision term (PAPER.md:257 names "the symmetric
+ * sampling method [57]" without defining it; the reading implemented is DESIGN.md section 4c / R25).  Same samples as
+ * rbg_collision, but the net rate of every sample is credited to all four particles of the sampled reaction -- + to the
+ * cells of the grid particle and its partner, - to the cells of the other pair -- and C of a species is the average of
+ * the equivalent estimators, so that what one cell gains another loses sample by sample: particle number is conserved
+ * to rounding whenever no particle leaves the momentum box.  C_dev is overwritten.  fp64 only, uniform sampler only
+ * (RBG_E_UNSUPPORTED otherwise).  The deposits are atomic adds, so the result is reproducible to rounding, not bitwise. */
+int rbg_collision_symmetric(rbg_handle* h, const double* f_dev, double* C_dev, int n_samples, uint64_t seed,
+                            void* cuda_stream);
+
 /* Same as rbg_collision with HOST buffers: copies f_host to the device (handle-owned scratch),
  * runs the kernels, copies C back, synchronises.  Pinned host memory makes the copies faster but
  * is not required. */

@@ -57,6 +57,7 @@ _SIGNATURES = {
     "rbg_create": (C.c_int, [C.POINTER(C.c_void_p), C.POINTER(_SpatialGrid), C.c_int, C.POINTER(_Species),
                              C.POINTER(_MomentumGrid), C.c_int, C.POINTER(_Process), C.c_double, C.c_int]),
     "rbg_collision": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_uint64, C.c_void_p]),
+    "rbg_collision_symmetric": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_uint64, C.c_void_p]),
     "rbg_collision_update": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_int,
                                        C.c_uint64, C.c_void_p]),
     "rbg_collision_evolve": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int, C.c_void_p, C.c_int,
@@ -191,6 +192,15 @@ class Collision:
             out = torch.empty_like(f)
         _check(load_library().rbg_collision(self._h, self._dev(f, "f"), self._dev(out, "out"), int(n_samples),
                                             int(seed), _stream_ptr(stream)), self._h)
+        return out
+
+    def collision_symmetric(self, f, n_samples: int, seed: int, out=None, stream=None):
+        """rbg_collision_symmetric: the conservative ("symmetric") estimator of C[f] (NEXT-3)."""
+        import torch
+        if out is None:
+            out = torch.empty_like(f)
+        _check(load_library().rbg_collision_symmetric(self._h, self._dev(f, "f"), self._dev(out, "out"), int(n_samples),
+                                                      int(seed), _stream_ptr(stream)), self._h)
         return out
 
     def collision_update(self, f, dt: float, n_samples: int, seed: int, out=None, neg_flag=None, stream=None):

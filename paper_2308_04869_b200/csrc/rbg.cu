@@ -20,6 +20,8 @@ namespace {
 thread_local std::string g_create_error;
 
 struct Role {
+    int process;           // index of the process the role comes from
+    double sym_override;   // the process's sym field (< 0: paper rule)
     int s[4];              // species of the grid particle 1, its partner 2 and the incident pair 3, 4
     int kind;
     double par[4];
@@ -272,6 +274,25 @@ int run(rbg_handle* h, const double* f, double* out, bool update, double dt, int
 
 }  // namespace
 
+namespace {
+template <int KIND>
+cudaError_t launch_sym(bool q, bool inel, bool csmem, const rbg::RoleParams<double>& rp, const rbg::LaunchParams& lp,
+                       const rbg::SymParams& sp, int grid, size_t smem, cudaStream_t st) {
+    auto go = [&](auto kern) -> cudaError_t {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        kern<<<grid, 512, smem, st>>>(rp, lp, sp);
+        return cudaGetLastError();
+    };
+    if (q) {
+        if (inel) return csmem ? go(rbg::collision_symmetric_kernel<KIND, true, true, true>) : go(rbg::collision_symmetric_kernel<KIND, true, true, false>);
+        return csmem ? go(rbg::collision_symmetric_kernel<KIND, true, false, true>) : go(rbg::collision_symmetric_kernel<KIND, true, false, false>);
+    }
+    if (inel) return csmem ? go(rbg::collision_symmetric_kernel<KIND, false, true, true>) : go(rbg::collision_symmetric_kernel<KIND, false, true, false>);
+    return csmem ? go(rbg::collision_symmetric_kernel<KIND, false, false, true>) : go(rbg::collision_symmetric_kernel<KIND, false, false, false>);
+}
+}  // namespace
+
 extern "C" {
 
 int rbg_create(rbg_handle** out, const rbg_spatial_grid* grid, int n_species, const rbg_species* species,
@@ -328,6 +349,7 @@ int rbg_create(rbg_handle** out, const rbg_spatial_grid* grid, int n_species, co
         // averaged over those of a and b.
         const double sum_norm = p.kind >= RBG_M2_QCD_Q1Q2 ? 1.0 : species[p.a].g * species[p.b].g;
         Role r;
+        r.process = i; r.sym_override = p.sym;
         r.sampler = p.sampler;
         r.kind = p.kind; std::memcpy(r.par, p.par, sizeof r.par);
         r.elastic = elastic;
@@ -395,6 +417,84 @@ int rbg_collision(rbg_handle* h, const double* f_dev, double* C_dev, int n_sampl
 int rbg_collision_update(rbg_handle* h, const double* f_dev, double* f_out_dev, double dt, int* neg_flag_dev,
                          int n_samples, uint64_t seed, void* cuda_stream) {
     return run(h, f_dev, f_out_dev, true, dt, neg_flag_dev, n_samples, seed, cuda_stream);
+}
+
+int rbg_collision_symmetric(rbg_handle* h, const double* f_dev, double* C_dev, int n_samples, uint64_t seed, void* cuda_stream) {
+    if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
+    if (!f_dev || !C_dev) return fail(h, RBG_E_INVALID_ARG, "null buffer");
+    if (f_dev == C_dev) return fail(h, RBG_E_INVALID_ARG, "output must not alias f");
+    if (n_samples <= 0) return fail(h, RBG_E_INVALID_ARG, "n_samples must be positive");
+    if (h->flags & RBG_FP32_KINEMATICS) return fail(h, RBG_E_UNSUPPORTED, "rbg_collision_symmetric is fp64 only");
+    for (const Role& r : h->roles)
+        if (r.sampler != RBG_SAMPLER_UNIFORM) return fail(h, RBG_E_UNSUPPORTED, "rbg_collision_symmetric supports the uniform sampler only");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = -1;
+    RBG_CUDA(h, cudaGetDevice(&dev));
+    if (dev != h->device) RBG_CUDA(h, cudaSetDevice(h->device));
+    h->last_launches = 0;
+    RBG_CUDA(h, cudaMemsetAsync(C_dev, 0, h->f_elems * sizeof(double), st));
+    auto dp3 = [&](int s) {
+        const rbg_momentum_grid& g = h->grids[s];
+        return ((g.pmax[0] - g.pmin[0]) / g.n[0]) * ((g.pmax[1] - g.pmin[1]) / g.n[1]) * ((g.pmax[2] - g.pmin[2]) / g.n[2]);
+    };
+    for (size_t ir = 0; ir < h->roles.size(); ++ir) {
+        Role r = h->roles[ir];
+        r.sym = 1.0;                                     // the symmetry factor is per slot here (SymParams::fac)
+        const rbg::RoleParams<double> rp = make_role_params<double>(*h, r);
+        rbg::SymParams sp;
+        std::memset(&sp, 0, sizeof sp);
+        for (int k = 0; k < 4; ++k) {
+            int m = 0;                                   // (role, slot) pairs of the process that carry species s_k
+            for (const Role& r2 : h->roles)
+                if (r2.process == r.process)
+                    for (int k2 = 0; k2 < 4; ++k2) m += r2.s[k2] == r.s[k];
+            const int oa = k < 2 ? 2 : 0;                // the opposite pair
+            const double symk = r.sym_override >= 0 ? r.sym_override : (r.s[oa] == r.s[oa + 1] ? 0.5 : 1.0);
+            sp.fac[k] = (k < 2 ? 1.0 : -1.0) * symk * (dp3(r.s[0]) / dp3(r.s[k])) / (double)m;
+            sp.cb[k] = C_dev + h->sp_off[r.s[k]];
+        }
+        // accumulator tables of the distinct species among slots 2..4
+        size_t tabs = 0;
+        for (int i = 1; i < 4; ++i) {
+            int owner = i;
+            for (int j = 1; j < i; ++j) if (r.s[j] == r.s[i]) { owner = j; break; }
+            if (owner == i) { sp.ctab_own[i] = 1; sp.ctab_off[i] = (int)tabs; tabs += ((size_t)rp.np[i] * 8 + 15) & ~(size_t)15; }
+            else { sp.ctab_own[i] = 0; sp.ctab_off[i] = sp.ctab_off[owner]; }
+        }
+        const bool csmem = tabs <= (size_t)h->max_smem_optin;
+        rbg::LaunchParams lp;
+        std::memset(&lp, 0, sizeof lp);
+        for (int i = 0; i < 4; ++i) lp.fb[i] = f_dev + h->sp_off[r.s[i]];
+        lp.nx_local = h->nx; lp.ix_offset = h->ix_offset; lp.n_samples = n_samples;
+        lp.key0 = (uint32_t)seed; lp.key1 = (uint32_t)(seed >> 32);
+        for (int rr = 0; rr < 10; ++rr) {
+            lp.rk[2 * rr] = lp.key0 + (uint32_t)rr * 0x9E3779B9u;
+            lp.rk[2 * rr + 1] = lp.key1 + (uint32_t)rr * 0xBB67AE85u;
+        }
+        // few, large tiles: every CTA flushes its tables with one global atomic per touched cell
+        const int np1 = rp.np[0];
+        int tiles = 1;
+        while ((long)tiles * h->nx < 2L * h->sm_count && tiles * 32 < np1) tiles *= 2;
+        lp.p1_per_cta = (np1 + tiles - 1) / tiles;
+        lp.tiles = (np1 + lp.p1_per_cta - 1) / lp.p1_per_cta;
+        const long grid = (long)lp.tiles * h->nx;
+        if (grid > 0x7fffffffL) return fail(h, RBG_E_UNSUPPORTED, "grid too large");
+        bool q = false;
+        for (int i = 0; i < 4; ++i) q = q || h->species[r.s[i]].stat != 0;
+        const size_t smem = csmem ? tabs : 0;
+        cudaError_t e;
+        switch (r.kind) {
+            case RBG_M2_CONST: e = launch_sym<rbg::KIND_CONST>(q, !r.elastic, csmem, rp, lp, sp, (int)grid, smem, st); break;
+            case RBG_M2_COULOMB_SCREENED: e = launch_sym<rbg::KIND_COULOMB>(q, !r.elastic, csmem, rp, lp, sp, (int)grid, smem, st); break;
+            case RBG_M2_TCHAN_S2: e = launch_sym<rbg::KIND_TCHAN_S2>(q, !r.elastic, csmem, rp, lp, sp, (int)grid, smem, st); break;
+            case RBG_M2_ISO_DSIGMA: e = launch_sym<rbg::KIND_ISO_DSIGMA>(q, !r.elastic, csmem, rp, lp, sp, (int)grid, smem, st); break;
+            default: e = launch_sym<rbg::KIND_QCD>(q, !r.elastic, csmem, rp, lp, sp, (int)grid, smem, st); break;
+        }
+        if (e != cudaSuccess) return fail(h, RBG_E_CUDA, std::string("kernel launch: ") + cudaGetErrorString(e));
+        ++h->last_launches;
+    }
+    if (dev != h->device && dev >= 0) cudaSetDevice(dev);
+    return RBG_OK;
 }
 
 int rbg_collision_evolve(rbg_handle* h, double* f_dev, double* scratch_dev, double dt, int n_steps, int* neg_flag_dev,
