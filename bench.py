@@ -251,6 +251,8 @@ def main():
                     "the JSON line then names the reduced workload)")
     ap.add_argument("--sampler", type=int, default=0, choices=[0, 1], help="1: t-channel importance sampler on the "
                     "t-channel processes (configs 2, 3, 5); the JSON line then names it")
+    ap.add_argument("--estimator", default="standard", choices=["standard", "symmetric"], help="symmetric: the conservative "
+                    "estimator rbg_collision_symmetric (NEXT-3); the JSON line then names it")
     ap.add_argument("--opt", action="append", default=[], help="librbg option key=value (launch geometry)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -275,6 +277,10 @@ def main():
     w = workloads.make(args.config, nx=args.nx, sampler=args.sampler)
     if args.nx is not None:
         w["name"] += f" [nx overridden to {args.nx}]"
+    sym = args.estimator == "symmetric"
+    if sym:
+        w["name"] += " [conservative (symmetric) estimator]"
+        w["dt"] = 0.0
     prob = w["problem"]
     # weak scaling: every rank sweeps one copy of the workload; rank r holds global cells [r*Nx, (r+1)*Nx)
     col = rbg.Collision(prob, fp32_kinematics=w["fp32"], ix_offset=rank * prob["nx"])
@@ -291,6 +297,8 @@ def main():
     def step():
         if w["dt"] > 0:
             col.collision_update(f, w["dt"], w["n_samples"], w["seed"], out=out, neg_flag=flag, stream=stream)
+        elif sym:
+            col.collision_symmetric(f, w["n_samples"], w["seed"], out=out, stream=stream)
         else:
             col.collision(f, w["n_samples"], w["seed"], out=out, stream=stream)
 
@@ -320,14 +328,21 @@ def main():
     # ---- e2e: the same sweep through the C ABI with HOST buffers (pinned), copies inside the timing
     f_host = torch.from_numpy(w["f"]).pin_memory()
     c_host = torch.empty_like(f_host).pin_memory()
-    col.collision_host(f_host, w["n_samples"], w["seed"], out=c_host)       # warm: allocates scratch
+    def host_call():
+        if sym:                                  # no host entry point for this estimator: pinned copies around the device call
+            fd = f_host.cuda(non_blocking=True)
+            c_host.copy_(col.collision_symmetric(fd, w["n_samples"], w["seed"]), non_blocking=True)
+            torch.cuda.synchronize()
+        else:
+            col.collision_host(f_host, w["n_samples"], w["seed"], out=c_host)
+    host_call()                                  # warm: allocates scratch
     barrier()
     e2e_steps = max(1, min(args.steps, 3))
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        col.collision_host(f_host, w["n_samples"], w["seed"], out=c_host)
+        host_call()
     t_e2e = max_over_ranks((time.perf_counter() - t0) / e2e_steps)
-    same = bool(torch.equal(c_host.cuda(), out)) if w["dt"] == 0 else None
+    same = bool(torch.equal(c_host.cuda(), out)) if (w["dt"] == 0 and not sym) else None
 
     if rank != 0:
         if world > 1:
@@ -349,11 +364,11 @@ def main():
     if w["fp32"]:
         peak_nominal *= 2                       # 128 fp32 lanes per SM
     roof = {"bound": "alu", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s", "frac": achieved / peak_nominal,
-            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.config) if args.nx is None and not args.sampler else None,
+            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.config) if args.nx is None and not args.sampler and not sym else None,
             "traffic_unit": "bytes per launch (ncu capture, profiles/r1c_chain_v2_cfg2.md)", "peak_source": f"{sms} SM x {FP64_LANES_PER_SM * (2 if w['fp32'] else 1)} FMA/clk x 2 x "
                                             f"{max_mhz:.0f} MHz (DESIGN.md section 8)",
             "peak_probe_tflops": probe, "frac_of_probe": achieved / probe,
-            "kernel": "rbg::collision_role_kernel", "launch_ms": t_launch * 1e3,
+            "kernel": "rbg::collision_symmetric_kernel" if sym else "rbg::collision_role_kernel", "launch_ms": t_launch * 1e3,
             "flops_per_sample": fl / n_evals}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),

@@ -30,7 +30,9 @@
 // deterministic brute-force quadrature of (R) (oracle/quadrature.py), H-theorem sign,
 // thread-count independence; Table III kinds against textbook values, crossing symmetry and regulator limits;
 // inelastic roles against per-sample kinematics, detailed balance, the quadrature and cross-species bookkeeping
-// (tests/test_oracle_qcd.py).  No function here is "parity unpinned".
+// (tests/test_oracle_qcd.py).  PARITY UNPINNED (by the reference): orc_collision_symmetric -- the paper names the
+// "symmetric sampling method [57]" but defines it outside PAPER.md; it is pinned by invariants only
+// (tests/test_oracle_symmetric.py).  Every other function here is pinned.
 #include <cmath>
 #include <cstdint>
 #include <cstdlib>
