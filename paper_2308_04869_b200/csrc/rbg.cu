@@ -629,7 +629,8 @@ int rbg_moments(rbg_handle* h, const double* f_dev, double* M_dev, double* total
         const double* fs = f_dev + h->sp_off[s];
         double* Ms = M_dev + (size_t)s * h->nx * rbg::N_MOMENTS;
         const int nyz = tb.n[1] * tb.n[2];
-        const size_t head = (64 + (2 * (rbg::MOM_THREADS / 32) * 16 + (size_t)tb.n[0]) * 8 + 127) & ~(size_t)127;
+        // head: mbarriers, counters, MOM_RED reduction buffers, p_x table
+        const size_t head = (128 + ((size_t)rbg::MOM_RED * (rbg::MOM_THREADS / 32) * 16 + (size_t)tb.n[0]) * 8 + 127) & ~(size_t)127;
         // the 1/E table lives in shared memory when it fits next to two stages (measured: reading it through L1 and
         // spending its shared memory on a third stage is slower, 0.73 vs 0.58 ms on config 4: the kernel is bound by the
         // CTA's own instruction latency, the two-stage ring alone streams at 6.2 TB/s); otherwise it is read through L1
@@ -637,14 +638,20 @@ int rbg_moments(rbg_handle* h, const double* f_dev, double* M_dev, double* total
         StagedGeometry g = staged_geometry(h, s, fs, head, true);
         if (!g.ok) { ie_smem = false; g = staged_geometry(h, s, fs, head, false); }
         if (!g.ok) return fail(h, RBG_E_UNSUPPORTED, "rbg_moments: two spatial cells of one species must fit in shared memory");
+        const bool one_team = g.team == rbg::MOM_THREADS && g.n_stages * g.group <= rbg::MOM_RED;
         auto launch = [&](auto kern) -> cudaError_t {
             cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem);
             if (e != cudaSuccess) return e;
             kern<<<g.ctas, rbg::MOM_THREADS, g.smem, st>>>(fs, tb, h->nx, Ms, g.group, g.n_stages, g.team, g.lead);
             return cudaSuccess;
         };
-        if (g.team >= nyz) RBG_CUDA(h, ie_smem ? launch(rbg::moments_kernel<1, true>) : launch(rbg::moments_kernel<1, false>));
-        else               RBG_CUDA(h, ie_smem ? launch(rbg::moments_kernel<4, true>) : launch(rbg::moments_kernel<4, false>));
+        if (one_team) {
+            if (g.team >= nyz) RBG_CUDA(h, ie_smem ? launch(rbg::moments_kernel<1, true, true>) : launch(rbg::moments_kernel<1, false, true>));
+            else               RBG_CUDA(h, ie_smem ? launch(rbg::moments_kernel<4, true, true>) : launch(rbg::moments_kernel<4, false, true>));
+        } else {
+            if (g.team >= nyz) RBG_CUDA(h, ie_smem ? launch(rbg::moments_kernel<1, true, false>) : launch(rbg::moments_kernel<1, false, false>));
+            else               RBG_CUDA(h, ie_smem ? launch(rbg::moments_kernel<4, true, false>) : launch(rbg::moments_kernel<4, false, false>));
+        }
         RBG_CUDA(h, cudaGetLastError());
         ++h->last_launches;
     }
@@ -709,7 +716,7 @@ int rbg_vlasov_step(rbg_handle* h, const double* f_dev, double* f_out_dev, doubl
         const double* fs = f_dev + h->sp_off[s];
         double* os = f_out_dev + h->sp_off[s];
         const int nyz = tb.n[1] * tb.n[2];
-        const size_t head = (64 + (size_t)tb.n[0] * 8 + 127) & ~(size_t)127;
+        const size_t head = (128 + (size_t)tb.n[0] * 8 + 127) & ~(size_t)127;
         const StagedGeometry g = staged_geometry(h, s, fs, head, true);
         if (!g.ok) return fail(h, RBG_E_UNSUPPORTED, "rbg_vlasov_step: two spatial cells of one species plus its 1/E table must fit in shared memory");
         if (g.team >= nyz) {

@@ -39,7 +39,7 @@ struct SpeciesTables {
 // not a multiple of 16 (an odd leading cell, the tail of the domain) is copied cooperatively with plain loads instead.
 // The cells of a stage are shared out among teams of `team` threads (a power of two, 32..512: about one thread per
 // (ipy, ipz) column), so small momentum grids keep every warp busy.
-enum { MOM_MAX_STAGES = 8, MOM_THREADS = 512 };
+enum { MOM_MAX_STAGES = 8, MOM_THREADS = 512, MOM_RED = 4 };   // MOM_RED: reduction buffers ([16 warps][16] doubles each)
 
 // Sum of v[m] over the 32 lanes for 16 values at once: each step halves the number of values a lane carries, so the
 // whole reduction takes 8 + 4 + 2 + 1 + 1 shuffles instead of 16 x 5.  On return lane l (l < 16) holds the total of
@@ -62,15 +62,22 @@ __device__ __forceinline__ int mom_slot(int l) { return ((l & 1) << 3) | ((l & 2
 
 // MOM_MAXC = columns a thread owns at a time (1 when the team covers the (ipy, ipz) plane)
 // IE_SMEM: the 1/E table is copied to shared memory; when it does not fit next to two stages it is read through L1.
-template <int MOM_MAXC, bool IE_SMEM>
+// ONE_TEAM (the whole CTA works on one spatial cell at a time: large momentum grids): no CTA barrier in the steady state.
+// Each warp leaves its 14 partial sums in shared memory and bumps a counter; the warp that arrives last adds the 16
+// partials in a fixed order and writes the result, and the warp that finishes last with a stage refills it, so warps
+// that are done (or own no columns) run ahead to the next stage instead of waiting.
+template <int MOM_MAXC, bool IE_SMEM, bool ONE_TEAM>
 __global__ void __launch_bounds__(MOM_THREADS, 1)
 moments_kernel(const double* __restrict__ f_species, SpeciesTables tb, int nx_cells, double* __restrict__ M_species,
                int group, int n_stages, int team, int lead) {
     extern __shared__ __align__(128) unsigned char mom_smem[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(mom_smem);                             // MOM_MAX_STAGES mbarriers
-    double* red = reinterpret_cast<double*>(mom_smem + 64);                             // [2][16 warps][16]
-    double* px_tab = red + 2 * (MOM_THREADS / 32) * 16;                                 // p_x of the n[0] cell centres
-    const size_t head = (64 + (2 * (MOM_THREADS / 32) * 16 + (size_t)tb.n[0]) * 8 + 127) & ~(size_t)127;
+    int* done = reinterpret_cast<int*>(mom_smem + 64);                                  // [8] warps done with stage k
+    int* cnt = done + MOM_MAX_STAGES;                                                   // [MOM_RED] warps done with a cell
+    // reduction buffers: ONE_TEAM one per (stage, cell of the stage) (n_stages * group <= MOM_RED), else two (alternating)
+    double* red = reinterpret_cast<double*>(mom_smem + 128);
+    double* px_tab = red + (size_t)MOM_RED * (MOM_THREADS / 32) * 16;                   // p_x of the n[0] cell centres
+    const size_t head = (128 + ((size_t)MOM_RED * (MOM_THREADS / 32) * 16 + (size_t)tb.n[0]) * 8 + 127) & ~(size_t)127;
     const size_t np = (size_t)tb.np;
     const size_t tab_bytes = IE_SMEM ? (np * 8 + 127) & ~(size_t)127 : 0;
     const double* __restrict__ iEs = IE_SMEM ? reinterpret_cast<const double*>(mom_smem + head) : tb.iE;
@@ -93,7 +100,8 @@ moments_kernel(const double* __restrict__ f_species, SpeciesTables tb, int nx_ce
         }
     };
     if (threadIdx.x == 0) {
-        for (int k = 0; k < n_stages; ++k) mbar_init(&bars[k], 1);
+        for (int k = 0; k < n_stages; ++k) { mbar_init(&bars[k], 1); done[k] = 0; }
+        for (int k = 0; k < MOM_RED; ++k) cnt[k] = 0;
         fence_mbar_init();
         for (int k = 0; k < n_stages; ++k) arm(k, blockIdx.x + k * gridDim.x);          // prologue: fill the ring
     }
@@ -117,6 +125,7 @@ moments_kernel(const double* __restrict__ f_species, SpeciesTables tb, int nx_ce
             mbar_wait(&bars[slot], (phases >> slot) & 1u);
             phases ^= 1u << slot;
         } else {
+            if (ONE_TEAM) __syncthreads();                     // nobody still reads the unit this slot held before
             const double* src = f_species + (size_t)first * np;
             for (size_t j = threadIdx.x; j < (size_t)cells * np; j += MOM_THREADS) fs[j] = __ldcs(src + j);
             __syncthreads();
@@ -174,18 +183,54 @@ moments_kernel(const double* __restrict__ f_species, SpeciesTables tb, int nx_ce
                 }
             }
             const double tot = warp_reduce16(acc, lane);
-            double* rb = red + (size_t)flip * (MOM_THREADS / 32) * 16;
-            if (lane < 16) rb[warp * 16 + mom_slot(lane)] = tot;
-            __syncthreads();
-            if (active && t_in_team < N_MOMENTS) {
-                double v = 0.0;
-                for (int w = 0; w < warps_per_team; ++w) v += rb[(my_team * warps_per_team + w) * 16 + t_in_team];
-                M_species[((size_t)first + cell) * N_MOMENTS + t_in_team] = v * dp3;
+            if (ONE_TEAM) {
+                const int rbi = slot * group + cell;
+                double* rb = red + (size_t)rbi * (MOM_THREADS / 32) * 16;
+                if (lane < 16) rb[warp * 16 + mom_slot(lane)] = tot;
+                __syncwarp();
+                int last = 0;
+                if (lane == 0) {
+                    __threadfence_block();
+                    last = atomicAdd(&cnt[rbi], 1) == MOM_THREADS / 32 - 1;
+                    if (last) cnt[rbi] = 0;
+                }
+                last = __shfl_sync(0xffffffffu, last, 0);
+                if (last) {                                    // every warp's partial sums are in rb
+                    __threadfence_block();
+                    if (lane < N_MOMENTS) {
+                        double v = 0.0;
+#pragma unroll
+                        for (int w = 0; w < MOM_THREADS / 32; ++w) v += rb[w * 16 + lane];
+                        M_species[((size_t)first + cell) * N_MOMENTS + lane] = v * dp3;
+                    }
+                }
+            } else {
+                double* rb = red + (size_t)flip * (MOM_THREADS / 32) * 16;
+                if (lane < 16) rb[warp * 16 + mom_slot(lane)] = tot;
+                __syncthreads();
+                if (active && t_in_team < N_MOMENTS) {
+                    double v = 0.0;
+                    for (int w = 0; w < warps_per_team; ++w) v += rb[(my_team * warps_per_team + w) * 16 + t_in_team];
+                    M_species[((size_t)first + cell) * N_MOMENTS + t_in_team] = v * dp3;
+                }
+                flip ^= 1;                                     // the next round writes the other buffer: one barrier per round
             }
-            flip ^= 1;                                         // the next round writes the other buffer: one barrier per round
         }
-        __syncthreads();                                       // every team has finished reading the stage
-        if (threadIdx.x == 0) arm(slot, u + n_stages * gridDim.x);       // refill with the unit n_stages iterations ahead
+        if (ONE_TEAM) {
+            // the warp that finishes last with this stage refills it (its reads of the stage and of the reduction
+            // buffers are complete: their values were consumed above)
+            __syncwarp();
+            if (lane == 0) {
+                __threadfence_block();
+                if (atomicAdd(&done[slot], 1) == MOM_THREADS / 32 - 1) {
+                    done[slot] = 0;
+                    arm(slot, u + n_stages * gridDim.x);
+                }
+            }
+        } else {
+            __syncthreads();                                   // every team has finished reading the stage
+            if (threadIdx.x == 0) arm(slot, u + n_stages * gridDim.x);   // refill with the unit n_stages iterations ahead
+        }
     }
     (void)warp_in_team;
 }
@@ -319,8 +364,9 @@ vlasov_upfd_kernel(const double* __restrict__ f_species, double* __restrict__ ou
                    int group, int n_stages, int team, int lead) {
     extern __shared__ __align__(128) unsigned char mom_smem[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(mom_smem);
-    double* px_tab = reinterpret_cast<double*>(mom_smem + 64);
-    const size_t head = (64 + (size_t)tb.n[0] * 8 + 127) & ~(size_t)127;
+    int* done = reinterpret_cast<int*>(mom_smem + 64);                                  // warps done with stage k
+    double* px_tab = reinterpret_cast<double*>(mom_smem + 128);
+    const size_t head = (128 + (size_t)tb.n[0] * 8 + 127) & ~(size_t)127;
     double* iEs = reinterpret_cast<double*>(mom_smem + head);
     const size_t np = (size_t)tb.np;
     const size_t tab_bytes = (np * 8 + 127) & ~(size_t)127;
@@ -343,7 +389,7 @@ vlasov_upfd_kernel(const double* __restrict__ f_species, double* __restrict__ ou
         }
     };
     if (threadIdx.x == 0) {
-        for (int k = 0; k < n_stages; ++k) mbar_init(&bars[k], 1);
+        for (int k = 0; k < n_stages; ++k) { mbar_init(&bars[k], 1); done[k] = 0; }
         fence_mbar_init();
         for (int k = 0; k < n_stages; ++k) arm(k, blockIdx.x + k * gridDim.x);
     }
@@ -363,6 +409,7 @@ vlasov_upfd_kernel(const double* __restrict__ f_species, double* __restrict__ ou
             mbar_wait(&bars[slot], (phases >> slot) & 1u);
             phases ^= 1u << slot;
         } else {
+            __syncthreads();                                   // nobody still reads the unit this slot held before
             const double* src = f_species + (size_t)first * np;
             for (size_t j = threadIdx.x; j < (size_t)cells * np; j += MOM_THREADS) fs[j] = __ldcs(src + j);
             __syncthreads();
@@ -408,8 +455,16 @@ vlasov_upfd_kernel(const double* __restrict__ f_species, double* __restrict__ ou
                 }
             }
         }
-        __syncthreads();                                       // every team has finished reading the stage
-        if (threadIdx.x == 0) arm(slot, u + n_stages * gridDim.x);
+        // no CTA barrier: a warp that is done moves on to the next stage; the last warp to finish with this one (its
+        // shared-memory reads have completed: their values were consumed by the stores above) refills it
+        __syncwarp();
+        if (lane == 0) {
+            __threadfence_block();
+            if (atomicAdd(&done[slot], 1) == MOM_THREADS / 32 - 1) {
+                done[slot] = 0;
+                arm(slot, u + n_stages * gridDim.x);
+            }
+        }
     }
 }
 

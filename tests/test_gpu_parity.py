@@ -20,13 +20,22 @@ def _rbg():
 
 
 def oracle_C_and_scale(orc, f, n_samples, seed, **kw):
-    """Oracle C and the per-cell tolerance scale sum_roles (G + L)."""
+    """Oracle C and the per-cell tolerance scale sum_roles (|G| + |L|).  With ix_begin / ix_end / ix_stride only the
+    visited spatial cells are touched (the detail arrays of a full-size problem are gigabytes of untouched zeros)."""
     C_ref, d = orc.collision(f, n_samples, seed, detail=True, **kw)
     mag = np.zeros_like(C_ref)
+    cells = range(kw.get("ix_begin", 0), kw.get("ix_end", None) or orc.nx, kw.get("ix_stride", 1))
     for r in range(orc.n_roles):
         s1 = orc.roles[r]["s"][0]
-        n = orc.nx * orc.np[s1]
-        mag[orc.sp_off[s1]:orc.sp_off[s1] + n] += (np.abs(d["G"]) + np.abs(d["L"]))[orc.role_off[r]:orc.role_off[r] + n]
+        n = orc.np[s1]
+        if len(cells) == orc.nx:
+            sl_c, sl_d = slice(orc.sp_off[s1], orc.sp_off[s1] + orc.nx * n), slice(orc.role_off[r], orc.role_off[r] + orc.nx * n)
+            mag[sl_c] += np.abs(d["G"][sl_d]) + np.abs(d["L"][sl_d])
+            continue
+        for ix in cells:
+            sl_c = slice(orc.sp_off[s1] + ix * n, orc.sp_off[s1] + (ix + 1) * n)
+            sl_d = slice(orc.role_off[r] + ix * n, orc.role_off[r] + (ix + 1) * n)
+            mag[sl_c] += np.abs(d["G"][sl_d]) + np.abs(d["L"][sl_d])
     return C_ref, mag
 
 
