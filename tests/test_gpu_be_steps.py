@@ -153,3 +153,37 @@ def test_be_step_is_drift_then_vlasov_then_collision_with_3dt():
     assert np.all(np.abs(g.cpu().numpy() - f2) <= 1e-13 * np.abs(f2))
     with pytest.raises(rbg.RbgError):
         col.be_step(g, dt, dx=dx, E=None, B=None)
+
+
+@pytest.mark.parametrize("cfg,kw,nx", [(2, dict(np_side=20), 1300),      # one cell per stage, two stages: every CTA reuses its slots 4-5 times
+                                       (7, dict(np_side=11), 2500),      # four cells per stage, odd np: leading cell, cooperative tails
+                                       (1, dict(np_side=16), 1000)])     # two cells per stage (4096-cell grid)
+def test_staged_kernels_are_race_free_under_ring_reuse(cfg, kw, nx):
+    """The persistent moments / Vlasov kernels recycle their shared-memory stages through mbarrier phases and warp
+    arrival counters.  Many units per CTA, repeated runs: every run must equal the oracle and, bit for bit, every
+    other run (both kernels add in a fixed order)."""
+    rbg = _rbg()
+    w = workloads.make(cfg, nx=nx, **kw)
+    prob = w["problem"]
+    for s, q in zip(prob["species"], (-1.0, 1.0, 2.0, 0.5, -0.5, 0.3, 1.5)):
+        s["charge"] = q
+    rng = np.random.default_rng(8)
+    E = rng.normal(size=(nx, 3)); B = rng.normal(size=(nx, 3))
+    M_ref, _, _ = bs.moments(prob, w["f"])
+    V_ref = bs.vlasov_upfd(prob, w["f"], 0.02, E, B)
+    col = rbg.Collision(prob)
+    f = torch.from_numpy(w["f"]).cuda()
+    Ed, Bd = torch.from_numpy(E).cuda(), torch.from_numpy(B).cuda()
+    first = None
+    for rep in range(6):
+        M, _, _ = col.moments(f)
+        V = col.vlasov_step(f, 0.02, Ed, Bd)
+        torch.cuda.synchronize()
+        if first is None:
+            first = (M.clone(), V.clone())
+            Mh = M.cpu().numpy()
+            scale = np.maximum(np.abs(M_ref[..., 0:1]), np.abs(M_ref[..., 4:5])) * 30.0
+            assert np.all(np.abs(Mh - M_ref) <= 1e-12 * scale)
+            assert np.all(np.abs(V.cpu().numpy() - V_ref) <= 1e-14 * np.abs(V_ref))
+        else:
+            assert torch.equal(M, first[0]) and torch.equal(V, first[1]), rep
