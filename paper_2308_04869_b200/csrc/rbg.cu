@@ -637,7 +637,12 @@ int rbg_moments(rbg_handle* h, const double* f_dev, double* M_dev, double* total
         bool ie_smem = true;
         StagedGeometry g = staged_geometry(h, s, fs, head, true);
         if (!g.ok) { ie_smem = false; g = staged_geometry(h, s, fs, head, false); }
-        if (!g.ok) return fail(h, RBG_E_UNSUPPORTED, "rbg_moments: two spatial cells of one species must fit in shared memory");
+        if (!g.ok) {                                   // the block does not fit twice: read f straight from global memory
+            rbg::moments_direct_kernel<<<h->nx, 128, 0, st>>>(fs, tb, h->nx, Ms);
+            RBG_CUDA(h, cudaGetLastError());
+            ++h->last_launches;
+            continue;
+        }
         const bool one_team = g.team == rbg::MOM_THREADS && g.n_stages * g.group <= rbg::MOM_RED;
         auto launch = [&](auto kern) -> cudaError_t {
             cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem);
@@ -718,7 +723,14 @@ int rbg_vlasov_step(rbg_handle* h, const double* f_dev, double* f_out_dev, doubl
         const int nyz = tb.n[1] * tb.n[2];
         const size_t head = (128 + (size_t)tb.n[0] * 8 + 127) & ~(size_t)127;
         const StagedGeometry g = staged_geometry(h, s, fs, head, true);
-        if (!g.ok) return fail(h, RBG_E_UNSUPPORTED, "rbg_vlasov_step: two spatial cells of one species plus its 1/E table must fit in shared memory");
+        if (!g.ok) {                                   // the block does not fit twice next to the table: direct kernel
+            const int slab = 16, nchunks = (tb.np + 255) / 256;
+            const long grid = (long)nchunks * ((h->nx + slab - 1) / slab);
+            rbg::vlasov_direct_kernel<<<(unsigned)grid, 256, 0, st>>>(fs, os, tb, vp, slab);
+            RBG_CUDA(h, cudaGetLastError());
+            ++h->last_launches;
+            continue;
+        }
         if (g.team >= nyz) {
             RBG_CUDA(h, cudaFuncSetAttribute(rbg::vlasov_upfd_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
             rbg::vlasov_upfd_kernel<1><<<g.ctas, rbg::MOM_THREADS, g.smem, st>>>(fs, os, tb, vp, g.group, g.n_stages, g.team, g.lead);

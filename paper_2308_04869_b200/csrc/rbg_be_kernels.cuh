@@ -468,4 +468,104 @@ vlasov_upfd_kernel(const double* __restrict__ f_species, double* __restrict__ ou
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Direct (unstaged) variants for momentum grids whose block of one spatial cell does not fit in shared memory twice
+// (e.g. the paper's 35^3 test grid, 343 KB): same arithmetic, f read straight from global memory / L2.
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+moments_direct_kernel(const double* __restrict__ f_species, SpeciesTables tb, int nx_cells, double* __restrict__ M_species) {
+    __shared__ double red[4][N_MOMENTS];
+    const int ix = blockIdx.x;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const double* __restrict__ f = f_species + (size_t)ix * tb.np;
+    const double* __restrict__ iE = tb.iE;
+    const int nyz = tb.n[1] * tb.n[2];
+    const double msq = tb.mass * tb.mass;
+    double acc[N_MOMENTS];
+#pragma unroll
+    for (int m = 0; m < N_MOMENTS; ++m) acc[m] = 0.0;
+    for (int c = warp * 32 + lane; c < nyz; c += nwarps * 32) {
+        const int iy = c / tb.n[2], iz = c - iy * tb.n[2];
+        const double py = fma((double)iy + 0.5, tb.delta[1], tb.pmin[1]);
+        const double pz = fma((double)iz + 0.5, tb.delta[2], tb.pmin[2]);
+        double X0 = 0.0, X1 = 0.0, G0 = 0.0, G1 = 0.0, G2 = 0.0;
+#pragma unroll 4
+        for (int i = 0; i < tb.n[0]; ++i) {
+            const double px = fma((double)i + 0.5, tb.delta[0], tb.pmin[0]);
+            const size_t j = (size_t)i * nyz + c;
+            const double a = __ldcs(f + j);
+            const double g = a * __ldg(iE + j);
+            const double pg = px * g;
+            X0 += a;
+            X1 = fma(px, a, X1);
+            G0 += g;
+            G1 += pg;
+            G2 = fma(px, pg, G2);
+        }
+        const double r = fma(py, py, fma(pz, pz, msq));
+        const double yG0 = py * G0, zG0 = pz * G0;
+        acc[0] += X0;
+        acc[1] += G1; acc[2] += yG0; acc[3] += zG0;
+        acc[4] += fma(r, G0, G2);
+        acc[5] += X1; acc[6] = fma(py, X0, acc[6]); acc[7] = fma(pz, X0, acc[7]);
+        acc[8] += G2; acc[9] = fma(py, G1, acc[9]); acc[10] = fma(pz, G1, acc[10]);
+        acc[11] = fma(py, yG0, acc[11]); acc[12] = fma(py, zG0, acc[12]); acc[13] = fma(pz, zG0, acc[13]);
+    }
+#pragma unroll
+    for (int m = 0; m < N_MOMENTS; ++m) {
+        double v = acc[m];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) red[warp][m] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < N_MOMENTS) {
+        double v = 0.0;
+        for (int w = 0; w < nwarps; ++w) v += red[w][threadIdx.x];
+        M_species[(size_t)ix * N_MOMENTS + threadIdx.x] = v * (tb.delta[0] * tb.delta[1] * tb.delta[2]);
+    }
+}
+
+// thread = one momentum cell (velocity in registers), walking over `slab` consecutive spatial cells
+__global__ void __launch_bounds__(256)
+vlasov_direct_kernel(const double* __restrict__ f_species, double* __restrict__ out_species, SpeciesTables tb, VlasovParams vp, int slab) {
+    const int nchunks = (tb.np + blockDim.x - 1) / blockDim.x;
+    const int chunk = blockIdx.x % nchunks, sl = blockIdx.x / nchunks;
+    const int ip = chunk * blockDim.x + threadIdx.x;
+    if (ip >= tb.np) return;
+    const int ix_begin = sl * slab, ix_end = min(ix_begin + slab, vp.nx_cells);
+    const int nyz = tb.n[1] * tb.n[2];
+    const int i0 = ip / nyz, i1 = (ip - i0 * nyz) / tb.n[2], i2 = ip - i0 * nyz - i1 * tb.n[2];
+    // periodic momentum neighbours: m at p_d - dp_d, p at p_d + dp_d
+    const int x_m = ip + (i0 > 0 ? -nyz : (tb.n[0] - 1) * nyz), x_p = ip + (i0 < tb.n[0] - 1 ? nyz : -(tb.n[0] - 1) * nyz);
+    const int y_m = ip + (i1 > 0 ? -tb.n[2] : (tb.n[1] - 1) * tb.n[2]), y_p = ip + (i1 < tb.n[1] - 1 ? tb.n[2] : -(tb.n[1] - 1) * tb.n[2]);
+    const int z_m = ip + (i2 > 0 ? -1 : tb.n[2] - 1), z_p = ip + (i2 < tb.n[2] - 1 ? 1 : -(tb.n[2] - 1));
+    // the same v = p * (1/E) as the staged kernel
+    const double iE = __ldg(tb.iE + ip);
+    const double vx = fma((double)i0 + 0.5, tb.delta[0], tb.pmin[0]) * iE;
+    const double vy = fma((double)i1 + 0.5, tb.delta[1], tb.pmin[1]) * iE;
+    const double vz = fma((double)i2 + 0.5, tb.delta[2], tb.pmin[2]) * iE;
+    const double k0 = vp.dt / tb.delta[0], k1 = vp.dt / tb.delta[1], k2 = vp.dt / tb.delta[2];
+    const double Q = tb.charge;
+    const size_t np = (size_t)tb.np;
+    for (int ix = ix_begin; ix < ix_end; ++ix) {
+        const double* __restrict__ row = f_species + (size_t)ix * np;
+        const double* __restrict__ Ev = vp.E + (size_t)ix * 3;
+        const double* __restrict__ Bv = vp.B + (size_t)ix * 3;
+        const double QEx = Q * __ldg(Ev), QEy = Q * __ldg(Ev + 1), QEz = Q * __ldg(Ev + 2);
+        const double QBx = Q * __ldg(Bv), QBy = Q * __ldg(Bv + 1), QBz = Q * __ldg(Bv + 2);
+        const double Fx = fma(vy, QBz, fma(-vz, QBy, QEx));
+        const double Fy = fma(vz, QBx, fma(-vx, QBz, QEy));
+        const double Fz = fma(vx, QBy, fma(-vy, QBx, QEz));
+        const double c0 = fabs(Fx) * k0, c1 = fabs(Fy) * k1, c2 = fabs(Fz) * k2;
+        const double self = __ldg(row + ip);
+        const double u0 = __ldg(row + (Fx > 0.0 ? x_m : x_p));
+        const double u1 = __ldg(row + (Fy > 0.0 ? y_m : y_p));
+        const double u2 = __ldg(row + (Fz > 0.0 ? z_m : z_p));
+        const double num = fma(c2, u2, fma(c1, u1, fma(c0, u0, self * (1.0 / 3.0))));
+        const double den = ((1.0 / 3.0 + c0) + c1) + c2;
+        __stcs(out_species + (size_t)ix * np + ip, num * rcp_fast(den));
+    }
+}
+
 }  // namespace rbg

@@ -187,3 +187,54 @@ def test_staged_kernels_are_race_free_under_ring_reuse(cfg, kw, nx):
             assert np.all(np.abs(V.cpu().numpy() - V_ref) <= 1e-14 * np.abs(V_ref))
         else:
             assert torch.equal(M, first[0]) and torch.equal(V, first[1]), rep
+
+
+def _tiny_problem(n, nx):
+    return dict(nx=nx, species=[dict(mass=0.4, charge=-1.0, stat=0, g=1.0), dict(mass=0.0, charge=2.0, stat=0, g=1.0)],
+                grids=[dict(n=list(n), pmin=[-1.0, -2.0, -1.5], pmax=[1.0, 2.0, 1.5]), dict(n=list(n[::-1]), pmin=[-2.0] * 3, pmax=[2.0] * 3)],
+                processes=[], hbar=1.0)
+
+
+@pytest.mark.parametrize("n,nx", [((1, 1, 1), 1), ((1, 1, 1), 37), ((2, 1, 3), 5), ((3, 7, 1), 64), ((1, 40, 33), 3)])
+def test_be_steps_on_degenerate_momentum_grids(n, nx):
+    """Edge cases: one momentum cell (its own periodic neighbour), extents of 1 along some axes, a (ipy, ipz) plane wider
+    than a team (1 x 40 x 33), a massless species with a cell at p = 0, no processes at all."""
+    rbg = _rbg()
+    prob = _tiny_problem(n, nx)
+    rng = np.random.default_rng(21)
+    npc = int(np.prod(n))
+    f = rng.random(2 * nx * npc) + 0.05
+    E = rng.normal(size=(nx, 3)); B = rng.normal(size=(nx, 3))
+    col = rbg.Collision(prob)
+    fd = torch.from_numpy(f).cuda()
+    M, tot, em = col.moments(fd)
+    V = col.vlasov_step(fd, 0.03, torch.from_numpy(E).cuda(), torch.from_numpy(B).cuda())
+    D = col.drift_step(fd, 0.03, (0.4, 0.5, 0.6), bc=(1, 1, 1))
+    torch.cuda.synchronize()
+    M_ref, tot_ref, em_ref = bs.moments(prob, f)
+    scale = np.maximum(M_ref[..., 0:1], M_ref[..., 4:5]) * 16.0
+    assert np.all(np.abs(M.cpu().numpy() - M_ref) <= 1e-12 * scale)
+    assert np.all(np.abs(em.cpu().numpy() - em_ref) <= 1e-12 * scale.sum(0)[:, :1])
+    V_ref = bs.vlasov_upfd(prob, f, 0.03, E, B)
+    assert np.all(np.abs(V.cpu().numpy() - V_ref) <= 1e-14 * np.abs(V_ref))
+    D_ref = bs.drift_upfd(prob, f, (nx, 1, 1), 0.03, (0.4, 0.5, 0.6))
+    assert np.all(np.abs(D.cpu().numpy() - D_ref) <= 1e-14 * np.abs(D_ref))
+
+
+def test_be_steps_on_the_papers_35_cubed_grid_use_the_direct_kernels():
+    """A 35^3 block (343 KB) does not fit in shared memory: moments and Vlasov fall back to their direct kernels."""
+    rbg = _rbg()
+    w = workloads.make(6, nx=3)
+    prob = w["problem"]
+    prob["species"][0]["charge"], prob["species"][1]["charge"] = -1.0, 1.0
+    rng = np.random.default_rng(2)
+    f = w["f"] + 0.01 * rng.random(w["f"].size)
+    E = rng.normal(size=(3, 3)); B = rng.normal(size=(3, 3))
+    col = rbg.Collision(prob)
+    fd = torch.from_numpy(f).cuda()
+    M = col.moments(fd)[0].cpu().numpy()
+    V = col.vlasov_step(fd, 0.01, torch.from_numpy(E).cuda(), torch.from_numpy(B).cuda()).cpu().numpy()
+    M_ref = bs.moments(prob, f)[0]
+    assert np.all(np.abs(M - M_ref) <= 1e-12 * np.maximum(M_ref[..., 0:1], M_ref[..., 4:5]) * 4.0)
+    V_ref = bs.vlasov_upfd(prob, f, 0.01, E, B)
+    assert np.all(np.abs(V - V_ref) <= 1e-14 * np.abs(V_ref))
