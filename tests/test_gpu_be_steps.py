@@ -238,3 +238,35 @@ def test_be_steps_on_the_papers_35_cubed_grid_use_the_direct_kernels():
     assert np.all(np.abs(M - M_ref) <= 1e-12 * np.maximum(M_ref[..., 0:1], M_ref[..., 4:5]) * 4.0)
     V_ref = bs.vlasov_upfd(prob, f, 0.01, E, B)
     assert np.all(np.abs(V - V_ref) <= 1e-14 * np.abs(V_ref))
+
+
+def test_be_step_is_capturable_in_a_cuda_graph():
+    """All launches of rbg_be_step go to the caller's stream back to back: a CUDA graph of one step replays to the same
+    result as direct calls (launch-bound small problems are the use case)."""
+    rbg = _rbg()
+    nxyz = (2, 2, 2)
+    w = workloads.make(2, nx=8, np_side=6, n_samples=32)
+    prob = w["problem"]
+    rng = np.random.default_rng(6)
+    E = torch.from_numpy(rng.normal(size=(8, 3))).cuda(); B = torch.from_numpy(rng.normal(size=(8, 3))).cuda()
+    col = rbg.Collision(_with_grid(prob, nxyz))
+    kw = dict(dx=(0.5, 0.5, 0.5), E=E, B=B, n_samples=32, seed=5)
+    ref = torch.from_numpy(w["f"]).cuda()
+    for _ in range(3):
+        col.be_step(ref, 0.002, **kw)
+    torch.cuda.synchronize()
+    f = torch.from_numpy(w["f"]).cuda()
+    scratch, flag = torch.empty_like(f), torch.zeros(1, dtype=torch.int32, device="cuda")
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        col.be_step(f, 0.002, scratch=scratch, neg_flag=flag, stream=side, **kw)       # warm-up outside the capture
+        f.copy_(torch.from_numpy(w["f"]).cuda())
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            col.be_step(f, 0.002, scratch=scratch, neg_flag=flag, stream=torch.cuda.current_stream(), **kw)
+    torch.cuda.current_stream().wait_stream(side)
+    for _ in range(3):
+        graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(f, ref)
