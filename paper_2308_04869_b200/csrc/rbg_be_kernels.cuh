@@ -148,19 +148,32 @@ moments_kernel(const double* __restrict__ f_species, SpeciesTables tb, int nx_ce
                     if (c < nyz) {
                         const double* __restrict__ pf = fc + c;
                         const double* __restrict__ pe = iEs + c;
+                        // two independent sets of running sums (even / odd planes) halve the dependent-add chains
                         double x0 = 0.0, x1 = 0.0, g0 = 0.0, g1 = 0.0, g2 = 0.0;
-#pragma unroll 4
-                        for (int i = 0; i < tb.n[0]; ++i) {
+                        double y0 = 0.0, y1 = 0.0, h0 = 0.0, h1 = 0.0, h2 = 0.0;
+                        const int n0e = tb.n[0] & ~1;
+#pragma unroll 2
+                        for (int i = 0; i < n0e; i += 2) {
+                            const double pxa = px_tab[i], pxb = px_tab[i + 1];
+                            const double a = pf[(size_t)i * nyz], b = pf[(size_t)(i + 1) * nyz];
+                            const double ga = a * (IE_SMEM ? pe[(size_t)i * nyz] : __ldg(pe + (size_t)i * nyz));
+                            const double gb = b * (IE_SMEM ? pe[(size_t)(i + 1) * nyz] : __ldg(pe + (size_t)(i + 1) * nyz));
+                            const double pga = pxa * ga, pgb = pxb * gb;
+                            x0 += a;                 y0 += b;
+                            x1 = fma(pxa, a, x1);    y1 = fma(pxb, b, y1);
+                            g0 += ga;                h0 += gb;
+                            g1 += pga;               h1 += pgb;
+                            g2 = fma(pxa, pga, g2);  h2 = fma(pxb, pgb, h2);
+                        }
+                        if (n0e < tb.n[0]) {
+                            const int i = n0e;
                             const double px = px_tab[i];
                             const double a = pf[(size_t)i * nyz];
                             const double g = a * (IE_SMEM ? pe[(size_t)i * nyz] : __ldg(pe + (size_t)i * nyz));
                             const double pg = px * g;
-                            x0 += a;
-                            x1 = fma(px, a, x1);
-                            g0 += g;
-                            g1 += pg;
-                            g2 = fma(px, pg, g2);
+                            x0 += a; x1 = fma(px, a, x1); g0 += g; g1 += pg; g2 = fma(px, pg, g2);
                         }
+                        x0 += y0; x1 += y1; g0 += h0; g1 += h1; g2 += h2;
                         X0[q] = x0; X1[q] = x1; G0[q] = g0; G1[q] = g1; G2[q] = g2;
                     }
                 }
