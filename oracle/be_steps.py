@@ -7,6 +7,8 @@ the CUDA path and never imports it.
                  species (Eq. 7) and the charge and current densities rho, J (Eq. 15).
 * drift_upfd()   the first-order unconditionally-positivity-preserving upwind step of the drift term
                  (Eq. 25, 28-30), all three directions at once (reading R23).
+* drift_pfl()    the second-order positivity-preserving flux-limited step of the drift term (Eq. 31-33,
+                 PAPER.md:300-319), periodic (reading R26).
 * vlasov_upfd()  the same scheme for the Vlasov term (Eq. 26, 34), F = Q (E + v x B)
                  (PAPER.md:162), periodic in momentum (PAPER.md:336).
 
@@ -146,4 +148,45 @@ def vlasov_upfd(problem, f, dt, E, B):
             num = num + c * up
             den = den + c
         outs.append((num / den).reshape(-1))
+    return np.concatenate(outs)
+
+
+def _limited_face(fl, fc, fr, theta):
+    """Face value of the flux-limited scheme, Eq. 32-33, between the upwind cell c and the downwind
+    cell r, with l the cell upwind of c:  fc + 1/2 phi (fc - fl),
+        phi = max(0, min(1, (fr - fc)/(fc - fl), 2 / max(theta, (fl - fc)/fc))).
+    The velocity does not depend on x, so the v^+- of Eq. 32-33 factor out.  phi multiplies (fc - fl), so where that
+    difference vanishes the face value is fc whatever phi is (phi := 0 there); where fc = 0 (and fl > 0) the positivity
+    limiter 2/((fl - fc)/fc) is 0 (reading R26)."""
+    d = fc - fl
+    with np.errstate(divide="ignore", invalid="ignore"):
+        r = (fr - fc) / d
+        lim = 2.0 / np.maximum(theta, (fl - fc) / fc)
+        phi = np.maximum(0.0, np.minimum(1.0, np.minimum(r, lim)))
+    phi = np.where((d == 0.0) | (fc == 0.0), 0.0, phi)
+    return fc + 0.5 * phi * d
+
+
+def drift_pfl(problem, f, nxyz, dt, dx, theta=1e-10):
+    """One step of the second-order positivity-preserving flux-limited drift scheme, Eq. 31-33,
+    periodic in x, y, z:
+        f(t+dt) = f - 3 dt Sum_d (F_{i+1/2} - F_{i-1/2}) / dx_d,
+    F_{i+1/2} of Eq. 32 with the limiters of Eq. 33 (first printing; the second printing of phi^- is garbled) and
+    theta = 1e-10.  With s = sign(v_d): (F_{i+1/2} - F_{i-1/2}) = |v_d| (O - I), O the face value leaving
+    cell i (upwind cell i, its upwind neighbour i-s, downwind i+s) and I the face value entering it (upwind cell i-s)."""
+    f = np.asarray(f, dtype=np.float64)
+    nx, blocks = _blocks(dict(problem, nx=int(np.prod(nxyz))), f)
+    outs = []
+    for g, sp, fb in zip(problem["grids"], problem["species"], blocks):
+        _, _, V = cell_tables(g, sp["mass"])
+        a = fb.reshape(*nxyz, -1)
+        div = np.zeros_like(a)
+        for d in range(3):
+            pos = V[:, d] > 0
+            sh = lambda k: np.roll(a, k, axis=d)                 # sh(k)[i] = a[i - k]
+            # v > 0: upwind is i-1;  v < 0: upwind is i+1
+            O = np.where(pos, _limited_face(sh(1), a, sh(-1), theta), _limited_face(sh(-1), a, sh(1), theta))
+            I = np.where(pos, _limited_face(sh(2), sh(1), a, theta), _limited_face(sh(-2), sh(-1), a, theta))
+            div = div + (np.abs(V[:, d]) / dx[d]) * (O - I)
+        outs.append((a - 3.0 * dt * div).reshape(-1))
     return np.concatenate(outs)
