@@ -178,6 +178,13 @@ int rbg_moments(rbg_handle* h, const double* f_dev, double* M_dev, double* total
 typedef struct { double dt; double dx[3]; int bc[3]; double zeta; } rbg_drift_params;
 int rbg_drift_step(rbg_handle* h, const double* f_dev, double* f_out_dev, const rbg_drift_params* p, void* cuda_stream);
 
+/* One step of the second-order positivity-preserving flux-limited drift scheme, Eq. 31-33 (the first
+ * printing of Eq. 33, theta = 1e-10; reading R26), periodic in x, y and z:
+ *   f_out = f - 3 dt Sum_d (F_{i+1/2} - F_{i-1/2}) / dx_d.
+ * Explicit: positive for 3 dt Sum_d |v_d| / dx_d <= 1/2.  Same buffers and restrictions as rbg_drift_step. */
+int rbg_drift_step_pfl(rbg_handle* h, const double* f_dev, double* f_out_dev, double dt, const double* dx /* [3], host */,
+                       void* cuda_stream);
+
 /* One first-order UPFD step of the Vlasov term, Eq. 26 with Eq. 34, all three directions at once:
  *   f_out(p) = [ f/3 + dt Sum_d |F_d| f(p - sign(F_d) dp_d e_d) / dp_d ] / [ 1/3 + dt Sum_d |F_d| / dp_d ],
  * F = Q (E + v x B) with the species' charge and the fields of the spatial cell, E_dev and B_dev being

@@ -65,6 +65,7 @@ _SIGNATURES = {
     "rbg_collision_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_uint64]),
     "rbg_moments": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "rbg_drift_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "rbg_drift_step_pfl": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.POINTER(C.c_double), C.c_void_p]),
     "rbg_vlasov_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]),
     "rbg_be_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "rbg_f_elems": (C.c_size_t, [C.c_void_p]),
@@ -247,6 +248,15 @@ class Collision:
         p = _DriftParams(float(dt), (C.c_double * 3)(*[float(v) for v in dx]), (C.c_int * 3)(*[int(v) for v in bc]), float(zeta))
         _check(load_library().rbg_drift_step(self._h, self._dev(f, "f"), self._dev(out, "out"), C.byref(p),
                                              _stream_ptr(stream)), self._h)
+        return out
+
+    def drift_step_pfl(self, f, dt: float, dx, out=None, stream=None):
+        """rbg_drift_step_pfl: one step of the second-order flux-limited drift scheme (Eq. 31-33), periodic."""
+        import torch
+        if out is None:
+            out = torch.empty_like(f)
+        _check(load_library().rbg_drift_step_pfl(self._h, self._dev(f, "f"), self._dev(out, "out"), float(dt),
+                                                 (C.c_double * 3)(*[float(v) for v in dx]), _stream_ptr(stream)), self._h)
         return out
 
     def vlasov_step(self, f, dt: float, E, B, out=None, stream=None):

@@ -705,6 +705,35 @@ int rbg_drift_step(rbg_handle* h, const double* f_dev, double* f_out_dev, const 
     return RBG_OK;
 }
 
+int rbg_drift_step_pfl(rbg_handle* h, const double* f_dev, double* f_out_dev, double dt, const double* dx, void* cuda_stream) {
+    if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
+    if (!f_dev || !f_out_dev || !dx) return fail(h, RBG_E_INVALID_ARG, "null argument");
+    if (f_dev == f_out_dev) return fail(h, RBG_E_INVALID_ARG, "output must not alias f (the stencil reads neighbours)");
+    if (!(dt >= 0.0)) return fail(h, RBG_E_INVALID_ARG, "dt must be >= 0");
+    if (h->ix_offset != 0) return fail(h, RBG_E_UNSUPPORTED, "the drift stencil needs the whole spatial domain on one GPU (no ghost-layer exchange)");
+    rbg::DriftParams dp;
+    dp.dt = dt; dp.zeta = 0.0;
+    for (int d = 0; d < 3; ++d) {
+        if (!(dx[d] > 0.0)) return fail(h, RBG_E_INVALID_ARG, "dx must be positive");
+        dp.inv_dx[d] = 1.0 / dx[d]; dp.nxyz[d] = h->nxyz[d]; dp.bc[d] = 1;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    DeviceGuard guard(h->device);
+    h->last_launches = 0;
+    dp.zseg = std::min(16, h->nxyz[2]);
+    dp.tile_y = std::min(8, h->nxyz[1]);
+    const long nzseg = (h->nxyz[2] + dp.zseg - 1) / dp.zseg, nyt = (h->nxyz[1] + dp.tile_y - 1) / dp.tile_y;
+    for (int s = 0; s < h->n_species; ++s) {
+        const long nchunks = ((long)h->np[s] + 255) / 256;
+        const long grid = nchunks * nzseg * dp.tile_y * h->nxyz[0] * nyt;
+        if (grid > 0x7fffffffL) return fail(h, RBG_E_UNSUPPORTED, "rbg_drift_step_pfl: grid too large");
+        rbg::drift_pfl_kernel<<<(unsigned)grid, 256, 0, st>>>(f_dev + h->sp_off[s], f_out_dev + h->sp_off[s], species_tables(h, s), dp);
+        RBG_CUDA(h, cudaGetLastError());
+        ++h->last_launches;
+    }
+    return RBG_OK;
+}
+
 int rbg_vlasov_step(rbg_handle* h, const double* f_dev, double* f_out_dev, double dt, const double* E_dev, const double* B_dev,
                     void* cuda_stream) {
     if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");

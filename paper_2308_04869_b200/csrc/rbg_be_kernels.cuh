@@ -360,6 +360,70 @@ drift_upfd_kernel(const double* __restrict__ f_species, double* __restrict__ out
     }
 }
 
+// Second-order positivity-preserving flux-limited drift step, Eq. 31-33, periodic.  Face value
+// between the upwind cell c and the downwind cell r, l being the cell upwind of c (reading R26):
+//   fc + 1/2 phi (fc - fl),  phi = max(0, min(1, (fr - fc)/(fc - fl), 2 / max(theta, (fl - fc)/fc))).
+// Division-free form of the same value: with a = fr - fc and d = fc - fl, phi d = 0 when a d <= 0 (r <= 0); otherwise
+// min(1, r) d = (|a| < |d| ? a : d), and the positivity limiter 2 fc / (fl - fc) (binding only for fl > fc, i.e. d < 0,
+// where 2/theta never is) caps |phi d| at 2 fc.
+__device__ __forceinline__ double limited_face(double fl, double fc, double fr) {
+    const double d = fc - fl, a = fr - fc;
+    double t = fabs(a) < fabs(d) ? a : d;
+    if (d < 0.0) t = fmax(t, -2.0 * fc);
+    if (!(a * d > 0.0) || fc == 0.0) t = 0.0;
+    return fma(0.5, t, fc);
+}
+
+// Same decomposition and CTA order as drift_upfd_kernel.  f(t+dt) = f - 3 dt Sum_d |v_d| (O_d - I_d) / dx_d with O the face
+// value leaving the cell and I the one entering it.
+__global__ void __launch_bounds__(256)
+drift_pfl_kernel(const double* __restrict__ f_species, double* __restrict__ out_species, SpeciesTables tb, DriftParams dp) {
+    const int nchunks = (tb.np + blockDim.x - 1) / blockDim.x;
+    const int nzseg = (dp.nxyz[2] + dp.zseg - 1) / dp.zseg;
+    int b = blockIdx.x;
+    const int chunk = b % nchunks; b /= nchunks;
+    const int zs = b % nzseg; b /= nzseg;
+    const int iy_in = b % dp.tile_y; b /= dp.tile_y;
+    const int ixx = b % dp.nxyz[0];
+    const int iy = (b / dp.nxyz[0]) * dp.tile_y + iy_in;
+    const int ip = chunk * blockDim.x + threadIdx.x;
+    if (ip >= tb.np || iy >= dp.nxyz[1]) return;
+    const int z0 = zs * dp.zseg, z1 = min(z0 + dp.zseg, dp.nxyz[2]);
+    const ptrdiff_t np = tb.np;
+    double c[3];
+    int sgn[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const double v = __ldg(tb.v + (size_t)d * tb.np + ip);
+        c[d] = (3.0 * dp.dt * fabs(v)) * dp.inv_dx[d];
+        sgn[d] = v > 0.0 ? 1 : -1;
+    }
+    const int stride[3] = {dp.nxyz[1] * dp.nxyz[2], dp.nxyz[2], 1};
+    // periodic offset (in spatial cells) from index i along d to index i + k
+    auto wrap = [&](int d, int i, int k) {                      // |k| <= 2; extents of 1 or 2 wrap more than once
+        const int n = dp.nxyz[d];
+        int j = i + k;
+        j = j < 0 ? j + n : j; j = j < 0 ? j + n : j;
+        j = j >= n ? j - n : j; j = j >= n ? j - n : j;
+        return (ptrdiff_t)((j - i) * stride[d]) * np;
+    };
+    ptrdiff_t ox[3], oy[3];                                   // upwind-2, upwind-1, downwind along x and y
+    ox[0] = wrap(0, ixx, -2 * sgn[0]); ox[1] = wrap(0, ixx, -sgn[0]); ox[2] = wrap(0, ixx, sgn[0]);
+    oy[0] = wrap(1, iy, -2 * sgn[1]);  oy[1] = wrap(1, iy, -sgn[1]);  oy[2] = wrap(1, iy, sgn[1]);
+    const size_t row0 = ((size_t)ixx * dp.nxyz[1] + iy) * dp.nxyz[2];
+    for (int z = z0; z < z1; ++z) {
+        const double* __restrict__ row = f_species + (row0 + z) * np + ip;
+        const double fc = __ldg(row);
+        const double x2 = __ldg(row + ox[0]), x1 = __ldg(row + ox[1]), xd = __ldg(row + ox[2]);
+        const double y2 = __ldg(row + oy[0]), y1 = __ldg(row + oy[1]), yd = __ldg(row + oy[2]);
+        const double w2 = __ldg(row + wrap(2, z, -2 * sgn[2])), w1 = __ldg(row + wrap(2, z, -sgn[2])), wd = __ldg(row + wrap(2, z, sgn[2]));
+        double div = c[0] * (limited_face(x1, fc, xd) - limited_face(x2, x1, fc));
+        div = fma(c[1], limited_face(y1, fc, yd) - limited_face(y2, y1, fc), div);
+        div = fma(c[2], limited_face(w1, fc, wd) - limited_face(w2, w1, fc), div);
+        __stcs(out_species + (row0 + z) * np + ip, fc - div);
+    }
+}
+
 struct VlasovParams {
     double dt;
     int nx_cells;

@@ -270,3 +270,33 @@ def test_be_step_is_capturable_in_a_cuda_graph():
         graph.replay()
     torch.cuda.synchronize()
     assert torch.equal(f, ref)
+
+
+@pytest.mark.parametrize("cfg,kw,nxyz", [(2, dict(np_side=8), (5, 4, 3)), (7, dict(np_side=5), (3, 6, 4)),
+                                         (4, dict(np_side=20), (2, 2, 19)), (1, dict(np_side=16), (1, 1, 1)),
+                                         (1, dict(np_side=6), (2, 1, 2))])
+def test_drift_step_pfl_parity(cfg, kw, nxyz):
+    """Second-order flux-limited drift (Eq. 31-33) against oracle.be_steps.drift_pfl.  Tolerance: the update subtracts
+    six limited face values scaled by 3 dt |v| / dx from f; 1e-13 of the local scale max(f, neighbours)."""
+    rbg = _rbg()
+    w = workloads.make(cfg, nx=int(np.prod(nxyz)), **kw)
+    prob = w["problem"]
+    f = w["f"].copy()
+    f[::11] = 0.0                                              # empty cells exercise the limiter's special cases
+    f[5::13] = f[4::13][:f[5::13].size]                        # equal neighbours along the momentum axis only (harmless)
+    dt, dx = 0.02, (0.5, 0.8, 0.3)
+    ref = bs.drift_pfl(prob, f, nxyz, dt, dx)
+    col = rbg.Collision(_with_grid(prob, nxyz))
+    out = col.drift_step_pfl(torch.from_numpy(f).cuda(), dt, dx)
+    torch.cuda.synchronize()
+    out = out.cpu().numpy()
+    scale = np.abs(f).max()
+    # per species block the scale differs by orders of magnitude: use the block maximum
+    offs, _ = workloads.f_layout(dict(prob, nx=int(np.prod(nxyz))))
+    tol = np.empty_like(f)
+    ends = offs[1:] + [f.size]
+    for o, e in zip(offs, ends):
+        blk = f[o:e].reshape(int(np.prod(nxyz)), -1)
+        tol[o:e] = np.broadcast_to(1e-13 * blk.max(axis=0, keepdims=True), blk.shape).reshape(-1)
+    assert np.all(np.abs(out - ref) <= tol + 1e-300), float(np.max(np.abs(out - ref) / (tol + 1e-300)))
+    assert scale > 0
