@@ -411,16 +411,27 @@ drift_pfl_kernel(const double* __restrict__ f_species, double* __restrict__ out_
     ox[0] = wrap(0, ixx, -2 * sgn[0]); ox[1] = wrap(0, ixx, -sgn[0]); ox[2] = wrap(0, ixx, sgn[0]);
     oy[0] = wrap(1, iy, -2 * sgn[1]);  oy[1] = wrap(1, iy, -sgn[1]);  oy[2] = wrap(1, iy, sgn[1]);
     const size_t row0 = ((size_t)ixx * dp.nxyz[1] + iy) * dp.nxyz[2];
-    for (int z = z0; z < z1; ++z) {
-        const double* __restrict__ row = f_species + (row0 + z) * np + ip;
-        const double fc = __ldg(row);
-        const double x2 = __ldg(row + ox[0]), x1 = __ldg(row + ox[1]), xd = __ldg(row + ox[2]);
-        const double y2 = __ldg(row + oy[0]), y1 = __ldg(row + oy[1]), yd = __ldg(row + oy[2]);
-        const double w2 = __ldg(row + wrap(2, z, -2 * sgn[2])), w1 = __ldg(row + wrap(2, z, -sgn[2])), wd = __ldg(row + wrap(2, z, sgn[2]));
-        double div = c[0] * (limited_face(x1, fc, xd) - limited_face(x2, x1, fc));
-        div = fma(c[1], limited_face(y1, fc, yd) - limited_face(y2, y1, fc), div);
-        div = fma(c[2], limited_face(w1, fc, wd) - limited_face(w2, w1, fc), div);
-        __stcs(out_species + (row0 + z) * np + ip, fc - div);
+    constexpr int PB = 2;                                     // cells whose ten loads are issued together
+    for (int zb = z0; zb < z1; zb += PB) {
+        double fc[PB], x2[PB], x1[PB], xd[PB], y2[PB], y1[PB], yd[PB], w2[PB], w1[PB], wd[PB];
+#pragma unroll
+        for (int k = 0; k < PB; ++k) {
+            const int z = min(zb + k, z1 - 1);                       // the tail repeats the last cell (not stored)
+            const double* __restrict__ row = f_species + (row0 + z) * np + ip;
+            fc[k] = __ldg(row);
+            x2[k] = __ldg(row + ox[0]); x1[k] = __ldg(row + ox[1]); xd[k] = __ldg(row + ox[2]);
+            y2[k] = __ldg(row + oy[0]); y1[k] = __ldg(row + oy[1]); yd[k] = __ldg(row + oy[2]);
+            w2[k] = __ldg(row + wrap(2, z, -2 * sgn[2])); w1[k] = __ldg(row + wrap(2, z, -sgn[2])); wd[k] = __ldg(row + wrap(2, z, sgn[2]));
+        }
+#pragma unroll
+        for (int k = 0; k < PB; ++k) {
+            if (zb + k < z1) {
+                double div = c[0] * (limited_face(x1[k], fc[k], xd[k]) - limited_face(x2[k], x1[k], fc[k]));
+                div = fma(c[1], limited_face(y1[k], fc[k], yd[k]) - limited_face(y2[k], y1[k], fc[k]), div);
+                div = fma(c[2], limited_face(w1[k], fc[k], wd[k]) - limited_face(w2[k], w1[k], fc[k]), div);
+                __stcs(out_species + (row0 + zb + k) * np + ip, fc[k] - div);
+            }
+        }
     }
 }
 
