@@ -141,6 +141,12 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the NEXT-4 kernels on config 4 at full size, from the committed
+# `ncu --set full` captures (profiles/r1d_be_steps_and_qgp.md, captures D and F); null for other workloads.
+NCU_TRAFFIC_BE_CFG4 = {"moments": 2.097e9 + 7.1e6, "drift": 2.460e9 + 2.087e9, "vlasov": 2.099e9 + 2.042e9,
+                       "drift_pfl": 5.233e9 + 2.083e9}
+
+
 def run_be_steps(args):
     """--path be: the NEXT-4 kernels (rbg_moments, rbg_drift_step, rbg_vlasov_step) on the chosen config, one JSON line.
     A step = moments + one drift step + one Vlasov step over every phase-space cell.  HBM roofline: algorithmic bytes
@@ -197,7 +203,8 @@ def run_be_steps(args):
             launches += col.last_launch_count() * args.steps
             ms = sum(ts) / len(ts)
             gbs = bytes_per_cell * cells / (ms * 1e-3) / 1e9
-            res[name] = {"ms": ms, "algorithmic_bytes_per_cell": bytes_per_cell, "achieved_gbs": gbs, "frac": gbs / peak}
+            res[name] = {"ms": ms, "algorithmic_bytes_per_cell": bytes_per_cell, "achieved_gbs": gbs, "frac": gbs / peak,
+                         "traffic": NCU_TRAFFIC_BE_CFG4.get(name) if (args.config == 4 and args.nx is None) else None}
     clocks = cs.summary()
     t_step = sum(r["ms"] for k, r in res.items() if k != "drift_pfl") * 1e-3
     # e2e: host buffers in, host buffers out, for the three calls of one step
@@ -221,7 +228,7 @@ def run_be_steps(args):
             "e2e": {"value": cells / t_e2e, "unit": "cells/s", "h2d_bytes_per_step": int(w["f"].nbytes),
                     "d2h_bytes_per_step": int(w["f"].nbytes) + int(em.numel() * 8), "ms_per_step": t_e2e * 1e3},
             "roofline": {"bound": "hbm", "achieved": res[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s", "frac": res[dom]["frac"],
-                         "traffic": None, "kernel": f"rbg::{dom}_upfd_kernel", "peak_source": peak_src},
+                         "traffic": res[dom]["traffic"], "kernel": f"rbg::{dom}_upfd_kernel", "peak_source": peak_src},
             "kernels": res}
     if not args.no_cpu_baseline:
         from oracle import be_steps as bs
