@@ -197,7 +197,8 @@ int rbg_vlasov_step(rbg_handle* h, const double* f_dev, double* f_out_dev, doubl
  * order; reading R24):
  *     f <- rbg_drift_step(f, dt)                       Eq. 25 / 30      (if do_drift)
  *     f <- rbg_vlasov_step(f, dt, E, B)                Eq. 26 / 34      (if do_vlasov; E_dev, B_dev as above)
- *     f <- f + 3 dt C[f]  (rbg_collision_update)       Eq. 27: (1/3) df/dt = C   (if do_collision; n_samples, seed)
+ *     f <- f + 3 dt C[f]  (rbg_collision_update)       Eq. 27: (1/3) df/dt = C   (if do_collision; n_samples, seed;
+ *                                                       do_collision == 2: C from rbg_collision_symmetric instead)
  * in place: on return (stream order) f_dev holds the new state; scratch_dev (rbg_f_elems() doubles, caller-owned, not
  * overlapping f_dev) is clobbered.  *neg_flag_dev accumulates the cells the collision update left negative (may be
  * NULL when do_collision == 0).  All launches go to cuda_stream back to back (capturable in a CUDA graph). */

@@ -275,14 +275,15 @@ class Collision:
 
     def be_step(self, f, dt: float, dx=(1.0, 1.0, 1.0), bc=(1, 1, 1), zeta: float = 0.0, E=None, B=None, n_samples: int = 0,
                 seed: int = 0, drift=True, vlasov=True, collision=True, scratch=None, neg_flag=None, stream=None):
-        """rbg_be_step: one time step of Eq. 25-27 in place (drift, Vlasov, collision with 3 dt)."""
+        """rbg_be_step: one time step of Eq. 25-27 in place (drift, Vlasov, collision with 3 dt).  collision="symmetric"
+        uses the conservative estimator for the collision sub-step."""
         import torch
         if scratch is None:
             scratch = torch.empty_like(f)
         if neg_flag is None:
             neg_flag = torch.zeros(1, dtype=torch.int32, device=f.device)
         p = _BeStepParams(float(dt), (C.c_double * 3)(*[float(v) for v in dx]), (C.c_int * 3)(*[int(v) for v in bc]),
-                          float(zeta), int(n_samples), int(seed), int(bool(drift)), int(bool(vlasov)), int(bool(collision)))
+                          float(zeta), int(n_samples), int(seed), int(bool(drift)), int(bool(vlasov)), 2 if collision == "symmetric" else int(bool(collision)))
         ptr = lambda t: C.c_void_p(t.data_ptr()) if t is not None else None
         _check(load_library().rbg_be_step(self._h, self._dev(f, "f"), self._dev(scratch, "scratch"), C.byref(p), ptr(E), ptr(B),
                                           C.c_void_p(neg_flag.data_ptr()), _stream_ptr(stream)), self._h)

@@ -795,7 +795,14 @@ int rbg_be_step(rbg_handle* h, double* f_dev, double* scratch_dev, const rbg_be_
         if ((rc = rbg_vlasov_step(h, cur, nxt, p->dt, E_dev, B_dev, cuda_stream)) != RBG_OK) return rc;
         launches += h->last_launches; std::swap(cur, nxt);
     }
-    if (p->do_collision) {
+    if (p->do_collision == 2) {
+        // conservative estimator: C into the free buffer, then cur += 3 dt C in place
+        if ((rc = rbg_collision_symmetric(h, cur, nxt, p->n_samples, p->seed, cuda_stream)) != RBG_OK) return rc;
+        launches += h->last_launches;
+        rbg::axpy_count_kernel<<<h->sm_count * 8, 256, 0, (cudaStream_t)cuda_stream>>>(cur, nxt, 3.0 * p->dt, h->f_elems, neg_flag_dev);
+        RBG_CUDA(h, cudaGetLastError());
+        ++launches;
+    } else if (p->do_collision) {
         if ((rc = run(h, cur, nxt, true, 3.0 * p->dt, neg_flag_dev, p->n_samples, p->seed, cuda_stream)) != RBG_OK) return rc;
         launches += h->last_launches; std::swap(cur, nxt);
     }

@@ -119,3 +119,42 @@ def test_symmetric_and_local_be_steps_shard_over_spatial_cells():
     assert np.all(np.abs(C_sh - C_full) <= 1e-13 * np.abs(C_full).max())
     assert np.array_equal(sharding.unshard(prob, V_parts), V_full)
     assert np.array_equal(np.concatenate(M_parts, axis=1), M_full)
+
+
+def test_be_step_with_the_conservative_estimator():
+    """rbg_be_step(do_collision = 2): f <- f + 3 dt C_sym[f] after the drift and Vlasov sub-steps, against the composed
+    oracles; with the transport sub-steps off and an input that cannot leak, particle number is conserved to rounding."""
+    from oracle import be_steps as bs
+    rbg = _rbg()
+    nxyz = (2, 2, 1)
+    w = workloads.make(2, nx=4, np_side=6, n_samples=40)
+    prob = w["problem"]
+    rng = np.random.default_rng(3)
+    E = rng.normal(size=(4, 3)); B = rng.normal(size=(4, 3))
+    dt, dx = 0.003, (0.5, 0.6, 0.7)
+    f1 = bs.drift_upfd(prob, w["f"], nxyz, dt, dx)
+    f2 = bs.vlasov_upfd(prob, f1, dt, E, B)
+    orc = oracle.Oracle(prob)
+    C_ref, mag = orc.collision_symmetric(f2, 40, 11)
+    ref, neg_ref = oracle.update(f2, C_ref, 3 * dt)
+    col = rbg.Collision(dict(prob, nx=nxyz))
+    f = torch.from_numpy(w["f"]).cuda()
+    out, flag = col.be_step(f, dt, dx=dx, E=torch.from_numpy(E).cuda(), B=torch.from_numpy(B).cuda(), n_samples=40, seed=11,
+                            collision="symmetric")
+    torch.cuda.synchronize()
+    assert out.data_ptr() == f.data_ptr()
+    assert np.all(np.abs(out.cpu().numpy() - ref) <= 3 * dt * TOL * mag + 1e-13 * np.abs(ref))
+    assert int(flag.item()) == neg_ref
+    # collision only, compact input (config-1-like, |p| < 1 in a [-2,2]^3 box): number conserved per spatial cell
+    w1 = workloads.make(1, nx=3, np_side=16, n_samples=128)
+    p1 = w1["problem"]
+    p1["grids"][0] = dict(n=[16] * 3, pmin=[-2.0] * 3, pmax=[2.0] * 3)
+    P = workloads.configs.cell_centres(p1["grids"][0])
+    f0 = (w1["f"].reshape(3, -1) * ((P * P).sum(1) < 1.0)[None, :]).reshape(-1)
+    c1 = rbg.Collision(p1)
+    g = torch.from_numpy(f0).cuda()
+    for k in range(5):
+        c1.be_step(g, 0.01, n_samples=128, seed=50 + k, drift=False, vlasov=False, collision="symmetric")
+    torch.cuda.synchronize()
+    n0, n1 = f0.reshape(3, -1).sum(1), g.cpu().numpy().reshape(3, -1).sum(1)
+    assert np.all(np.abs(n1 - n0) <= 1e-12 * n0) and not np.allclose(g.cpu().numpy(), f0)
