@@ -143,7 +143,8 @@ class Oracle:
                                             p.get("sym", -1.0), int(p.get("sampler", 0))) for p in pr])
         self._h = L.orc_create(self.nx, len(sp), S, G, len(pr), P, float(problem.get("hbar", 1.0)), int(use_float))
         if not self._h:
-            raise ValueError("oracle: unsupported problem (unknown kind or sampler; a+b->b+a must be written a+b->a+b; sampler 1 needs an elastic t-channel kind)")
+            raise ValueError("oracle: unsupported problem (unknown kind or sampler; a+b->b+a must be written a+b->a+b; sampler 1 needs "
+                             "an elastic t-channel kind; a species in a process must have no cell centre with p0 = 0, Eq. 16's 1/p0)")
         self.n_species = len(sp)
         self.np = [int(np.prod(g["n"])) for g in gr]
         self.f_elems = int(L.orc_f_elems(self._h))

@@ -520,10 +520,10 @@ struct Evaluator {
                 if (j3 >= 0 && j4 >= 0) acc.Lin += wl;
                 acc.Q += (wg - wl) * (wg - wl);
                 if (sink) {
-                    // pref0 = V2 / (16 pi E1 N): the O13 prefactor without the symmetry factor
+                    // pref0 = hbar^2 V2 / (16 pi E1 N): the O13 prefactor without the symmetry factor
                     const Grid& g2 = H.grid[role.s[1]];
                     const double V2 = (g2.pmax[0] - g2.pmin[0]) * (g2.pmax[1] - g2.pmin[1]) * (g2.pmax[2] - g2.pmin[2]);
-                    const double pref0 = V2 / (16.0 * M_PI * (double)E1 * (double)N);
+                    const double pref0 = (H.hbar * H.hbar) * V2 / (16.0 * M_PI * (double)E1 * (double)N);
                     const double val = std::is_same<R, float>::value ? (double)(w * gain - w * loss) : wg - wl;
                     const int jc[4] = {ip1, j2, j3, j4};
                     for (int k4 = 0; k4 < 4; ++k4) {
@@ -550,7 +550,8 @@ struct Evaluator {
         (void)T1;
     }
 
-    // O13: scale.  C_role = sym V2 / (16 pi E1 N) (G - Ls), in double.
+    // O13: scale.  C_role = hbar^2 sym V2 / (16 pi E1 N) (G - Ls), in double.  hbar^2 is the "hbar^2 c" of Eq. 16
+    // with c = 1 (reading R8); the other place hbar enters is nbar of Eq. 18.
     double prefactor(int ip1, int N) const {
         const Grid& g1 = H.grid[role.s[0]];
         int i1[3];
@@ -563,7 +564,7 @@ struct Evaluator {
         const R E1 = std::sqrt(dot3<R>(p1, p1) + k.msq[0]);
         const Grid& g2 = H.grid[role.s[1]];
         const double V2 = (g2.pmax[0] - g2.pmin[0]) * (g2.pmax[1] - g2.pmin[1]) * (g2.pmax[2] - g2.pmin[2]);
-        return (role.sym * V2) / (16.0 * M_PI * (double)E1 * (double)N);
+        return ((H.hbar * H.hbar) * (role.sym * V2)) / (16.0 * M_PI * (double)E1 * (double)N);
     }
 };
 
@@ -643,6 +644,26 @@ void* orc_create(int nx, int n_species, const Species* sp, const Grid* grid, int
     // Symmetry factor ("1/2 ... when all incident particles are of the same type"): the incident
     // pair of a role is (3,4), so sym = 1/2 iff species 3 == species 4, else 1; sym >= 0 in the process
     // overrides it for every role of that process.
+    // Eq. 16 carries 1/p^0 of the grid particle: a massless species whose grid has a cell centre at
+    // p = 0 (odd cell counts on a box symmetric about 0) has no finite collision term there.  Such a problem is
+    // refused (reading R14): smallest cell-centre energy E_min = sqrt(Sum_d min_i p_d(i)^2 + m^2), with
+    // p_d(i) the centre as O0 computes it, must exceed 1e-6 of the smallest cell width.
+    for (int i = 0; i < n_process; ++i) {
+        const int idx[4] = {pr[i].a, pr[i].b, pr[i].c, pr[i].d};
+        for (int j = 0; j < 4; ++j) {
+            if (idx[j] < 0 || idx[j] >= n_species) { delete H; return nullptr; }
+            const Grid& g = grid[idx[j]];
+            double q = sp[idx[j]].mass * sp[idx[j]].mass, dmin = std::numeric_limits<double>::infinity();
+            for (int d = 0; d < 3; ++d) {
+                const double delta = (g.pmax[d] - g.pmin[d]) / (double)g.n[d];
+                double best = std::numeric_limits<double>::infinity();
+                for (int c = 0; c < g.n[d]; ++c) best = std::fmin(best, std::fabs(std::fma((double)c + 0.5, delta, g.pmin[d])));
+                q += best * best;
+                dmin = std::fmin(dmin, delta);
+            }
+            if (!(std::sqrt(q) > 1e-6 * dmin)) { delete H; return nullptr; }
+        }
+    }
     size_t roff = 0;
     for (int i = 0; i < n_process; ++i) {
         const Process& p = pr[i];

@@ -10,10 +10,10 @@ import oracle
 from conftest import read_golden
 
 
-def _one_species(m, n, lo, hi, kind=0, par=(1.0,), sym=-1.0):
+def _one_species(m, n, lo, hi, kind=0, par=(1.0,), sym=-1.0, hbar=1.0):
     return dict(nx=1, species=[dict(mass=m, charge=0, stat=0, g=1.0)],
                 grids=[dict(n=[n] * 3, pmin=[lo] * 3, pmax=[hi] * 3)],
-                processes=[dict(a=0, b=0, c=0, d=0, kind=kind, par=list(par), sym=sym)], hbar=1.0)
+                processes=[dict(a=0, b=0, c=0, d=0, kind=kind, par=list(par), sym=sym)], hbar=hbar)
 
 
 def _loss_with_error(o, ip1, fcb, seed, batches=16, n=1 << 20):
@@ -34,6 +34,32 @@ def test_p3_massless_closed_form():
         L, se = _loss_with_error(o, ip1, thermal, 4242 + ip1)
         assert se < 0.02 * exact
         assert abs(L - exact) < 4 * se + 1e-3 * exact, (L, exact, se)
+
+
+def test_p3_hbar_squared_prefactor_of_eq16():
+    """Eq. 16 carries hbar^2 c |M|^2 / (64 pi^2 ...): with c = 1 the closed form of P3 becomes
+    hbar^2 sym |M|^2 T^2 / (8 E1) for classical particles (no nbar).  A dropped or single power of hbar fails."""
+    T, M2, hbar = 0.5, 2.5, 0.5
+    o = oracle.Oracle(_one_species(0.0, 24, -6.0, 6.0, par=(M2,), hbar=hbar))
+    thermal = ("thermal", [[1.0, T, 0.0, 0.0, 0.0, 0, 0, 0]])
+    ip1 = (13 * 24 + 9) * 24 + 16
+    tr = o.trace(None, 0, 0, ip1, 0, 1, fcb=thermal, box_cut=False)
+    exact = hbar * hbar * 0.5 * M2 * T * T / (8 * tr["E1"]) * tr["f1"]
+    L, se = _loss_with_error(o, ip1, thermal, 99)
+    assert se < 0.02 * exact
+    assert abs(L - exact) < 4 * se + 1e-3 * exact, (L, exact, se)
+
+
+def test_cell_centre_with_zero_energy_is_refused():
+    """1/p^0 of Eq. 16: a massless species with a cell centre at p = 0 (odd grid, symmetric box) has no
+    finite collision term there (reading R14): refused.  The same grid with a mass, or an even grid, is accepted."""
+    with pytest.raises(ValueError):
+        oracle.Oracle(_one_species(0.0, 7, -3.0, 3.0))
+    with pytest.raises(ValueError):
+        oracle.Oracle(_one_species(0.0, 7, -0.7, 0.7))            # centre = fma(3.5, 0.2, -0.7) ~ 1e-17, not exactly 0
+    oracle.Oracle(_one_species(0.3, 7, -3.0, 3.0))
+    oracle.Oracle(_one_species(0.0, 8, -3.0, 3.0))
+    oracle.Oracle(_one_species(0.0, 7, -3.0, 4.0))                # odd but not symmetric: no centre at 0
 
 
 def _rate_quadrature(p1, m, T):
