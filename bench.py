@@ -1,17 +1,27 @@
 #!/usr/bin/env python
-"""bench.py -- one JSON line for the collision-term hot path (contract: task prompt, section 4).
+"""bench.py -- one JSON line for the collision-term hot path.
 
-A "step" is one full collision-term sweep (rbg_collision: every role, spatial cell, momentum cell,
-sample) of BASELINE.json configs[1] (e-/H+, screened Coulomb, 8^3 x 20^3 x 2 species, 1024 samples).
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference]
-N > 1: launched by torchrun, one rank per GPU; each rank sweeps its own copy of the workload with a
-distinct global cell offset (weak scaling; the path has no collective).
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--scaling strong|weak] [--impl reference]
+
+A "step" is one full collision-term sweep (rbg_collision, or rbg_collision_update for the fused-Euler config: every
+role, spatial cell, momentum cell and sample) of one workload.  The headline workload is BASELINE.json's largest
+single-GPU fp64 config, config 4 (32^3 spatial x 20^3 momentum cells, 512 samples, 1.34e11 sample evaluations,
+2.1 GB of f) -- "the most significant challenge ... high-dimensional integration at each phase space grid"
+(PAPER.md:340).  At N = 1 the same line carries a `configs` object with the other BASELINE configs (1, 2, 3, 5), each
+timed the same way, so that "every config at a stated fraction of the roofline" is one record.
+
+N > 1: `--gpus N` launches N ranks by itself (torchrun, one rank per GPU) unless it already runs under torchrun.
+`--scaling strong` (default): the workload's spatial cells are sharded over the ranks (paper_2308_04869_b200.sharding; the
+paper's spatial sub-domains); `--scaling weak`: every rank sweeps its own copy at a distinct global
+cell offset.  The path has no data-path collective; the only collective is the MAX all-reduce
+of the timing.  value = sample evaluations of all ranks / max-over-ranks time.
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
+import socket
 import statistics
 import subprocess
 import sys
@@ -28,9 +38,11 @@ import workloads  # noqa: E402
 from workloads import configs as wl  # noqa: E402
 
 METRIC, UNIT = "collision_samples_per_s", "samples/s"
+HEADLINE_CONFIG = 4
+BLOCK_CONFIGS = (1, 2, 3, 5)
 
 # Algorithmic FP64 work per sample of chain O1-O12 (FMA = 2 flops, every other
-# add/mul/compare/sqrt/divide = 1), by |M|^2 kind, classical statistics (+12 with quantum factors).
+# add/mul/compare/sqrt/divide = 1), by |M|^2 kind, classical statistics (+10 with quantum factors).
 FLOPS_PER_SAMPLE = {0: 141.0, 1: 155.0, 2: 157.0, 3: 142.0,
                     # Table III kinds: 138 (O2-O7, O10-O12) + t 11 + u 2 + T, U 2 + squares 3 + weight 3 + the row's
                     # rational function (5 / 14 / 14 / 5 / 12 / 12 / 16; a reciprocal = 1)
@@ -39,9 +51,9 @@ QUANTUM_EXTRA_FLOPS = 10.0
 # the same count for the t-channel importance sampler (steps S1-S7), kinds 1 and 2
 FLOPS_PER_SAMPLE_TCHANNEL = {1: 185.0, 2: 187.0}
 FP64_LANES_PER_SM = 64          # FMA/clk/SM; confirmed by the live probe
-# dram__bytes_read.sum + dram__bytes_write.sum of one role launch from the committed `ncu --set full`
-# capture (profiles/r1c_chain_v2_cfg2.md: 32.87 MB + 2.15 MB, config 2 at full size); null elsewhere.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {2: 35.02e6}
+# dram__bytes_read.sum + dram__bytes_write.sum of one role launch at full size, from the committed `ncu --set full`
+# captures (file named beside each); null for workloads without a capture.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {2: (35.02e6, "profiles/r1c_chain_v2_cfg2.md")}
 
 
 def flops_per_sweep(problem, n_samples):
@@ -100,51 +112,71 @@ class ClockSampler:
         return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def oracle_leg(w, cells, label):
-    """Time the oracle, as it stands, on the given spatial cells (host cores of this box)."""
+# ---- the oracle legs (cpu_baseline and --impl reference): the only places bench.py executes oracle/ ----------------
+def oracle_leg(w, target_seconds, warmups=1):
+    """Time the oracle, as it stands, on an evenly strided subset of the workload's spatial cells sized (from one
+    calibration cell, which is also the warm-up) for about target_seconds of wall time on this box's host cores."""
     import oracle
+    oracle.build()
     orc = oracle.Oracle(w["problem"], use_float=w["fp32"])
+    nx = w["problem"]["nx"]
     per_cell = wl.sample_evals(dict(w["problem"], nx=1), w["n_samples"])
+    for _ in range(max(1, warmups)):
+        t0 = time.perf_counter()
+        orc.collision(w["f"], w["n_samples"], w["seed"], ix_begin=0, ix_end=1)
+        t_cell = time.perf_counter() - t0
+    stride = max(1, int(np.ceil(nx * t_cell / max(target_seconds, 1e-3))))
+    ncell = (nx + stride - 1) // stride
     t0 = time.perf_counter()
-    for ix in cells:
-        orc.collision(w["f"], w["n_samples"], w["seed"], ix_begin=ix, ix_end=ix + 1)
+    orc.collision(w["f"], w["n_samples"], w["seed"], ix_begin=0, ix_end=nx, ix_stride=stride)
     dt = time.perf_counter() - t0
-    return {"value": per_cell * len(cells) / dt, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle",
-            "sample": f"{len(cells)} of {w['problem']['nx']} spatial cells ({label}); every role, momentum cell "
-                      f"and sample of those cells", "seconds": dt}
+    return {"value": per_cell * ncell / dt, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle",
+            "sample": f"{ncell} of {nx} spatial cells (every {stride}-th linear cell index from 0); every role, momentum "
+                      f"cell and sample of those cells ({per_cell * ncell:.3g} sample evaluations)", "seconds": dt}
 
 
 def run_reference(args):
-    """--impl reference: the oracle on this box's host cores, same config/metric (rank 0 only)."""
+    """--impl reference: the oracle on this box's host cores, same config / metric (rank 0 only).  A step is a bounded
+    sample of the workload (about --ref-seconds of CPU wall time)."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    w = workloads.make(args.config, sampler=args.sampler)
-    nx = w["problem"]["nx"]
-    ncell = max(1, min(nx, args.ref_cells))
-    cells = [int(i) for i in np.linspace(0, nx - 1, ncell).astype(int)]
-    import oracle
-    oracle.build()
-    for _ in range(args.warmup):
-        oracle_leg(w, cells[:1], "warm-up")
-    times, vals = [], []
-    for _ in range(args.steps):
-        r = oracle_leg(w, cells, "evenly spaced")
+    w = workloads.make(args.config, nx=args.nx, sampler=args.sampler)
+    if args.nx is not None:
+        w["name"] += f" [nx overridden to {args.nx}]"
+    times, vals, r = [], [], None
+    for i in range(args.steps):
+        r = oracle_leg(w, args.ref_seconds, warmups=args.warmup if i == 0 else 1)
         times.append(r["seconds"]); vals.append(r["value"])
     value = float(np.mean(vals))
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(times)), "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32" if w["fp32"] else "f64", "data": "synthetic",
-            "config": {"workload": w["name"], "cfg": args.config},
+            "scaling": args.scaling, "vs_baseline": None, "dtype": "f32" if w["fp32"] else "f64", "data": "synthetic",
+            "config": config_block(w, args, 1),
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
 
 
+def config_block(w, args, world):
+    """The `config` object: identical for our arm and the reference arm of the same command."""
+    return {"workload": w["name"], "cfg": w["cfg"], "nx": w.get("nx_global", w["problem"]["nx"]), "n_samples": w["n_samples"],
+            "l2": "L2 flushed (256 MB write) between timed iterations", "parallelism": f"spatial-shard x{world}"}
+
+
+# ---- the NEXT-4 kernels -----------------------------------------------------------------------------------------
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the NEXT-4 kernels on config 4 at full size, from the committed
 # `ncu --set full` captures (profiles/r1d_be_steps_and_qgp.md, captures D and F); null for other workloads.
 NCU_TRAFFIC_BE_CFG4 = {"moments": 2.097e9 + 7.1e6, "drift": 2.460e9 + 2.087e9, "vlasov": 2.099e9 + 2.042e9,
                        "drift_pfl": 5.233e9 + 2.083e9}
+
+
+def hbm_peak():
+    try:
+        peaks = json.loads((ROOT / "MEASURED_PEAKS.json").read_text())
+        return float(peaks["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+    except (OSError, ValueError, KeyError):
+        return 6500.0, "B200_PROFILING.md fallback"
 
 
 def run_be_steps(args):
@@ -167,6 +199,9 @@ def run_be_steps(args):
         if sp.get("charge", 0.0) == 0.0:
             sp["charge"] = q                       # the Vlasov step needs charged species
     col = rbg.Collision(dict(prob, nx=nxyz))
+    for kv in args.opt:
+        k, v = kv.split("=")
+        col.set_option(k, int(v))
     f = torch.from_numpy(w["f"]).cuda()
     out = torch.empty_like(f)
     rng = np.random.default_rng(5)
@@ -182,11 +217,7 @@ def run_be_steps(args):
                # second-order flux-limited drift (Eq. 31-33): same 16 B per cell, but ~260 FP64 instructions per cell
                # (FP64-pipe-bound); reported against the same HBM peak, not part of the step
                "drift_pfl": (lambda: col.drift_step_pfl(f, 0.01, dx, out=out, stream=stream), 16.0)}
-    try:
-        peaks = json.loads((ROOT / "MEASURED_PEAKS.json").read_text())
-        peak, peak_src = float(peaks["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
-    except (OSError, ValueError, KeyError):
-        peak, peak_src = 6500.0, "B200_PROFILING.md fallback"
+    peak, peak_src = hbm_peak()
     res, launches = {}, 0
     with ClockSampler(0) as cs:
         for name, (fn, bytes_per_cell) in kernels.items():
@@ -245,55 +276,85 @@ def run_be_steps(args):
     print(json.dumps(line))
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--path", default="collision", choices=["collision", "be"], help="collision: the hot path "
-                    "(default); be: the NEXT-4 kernels (moments, UPFD drift, UPFD Vlasov)")
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5); 2 = configs[1]; 6, 7 = the paper's own workloads")
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--ref-cells", type=int, default=6, help="spatial cells per step of the reference arm")
-    ap.add_argument("--cpu-cells", type=int, default=48, help="spatial cells of the cpu_baseline leg")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--nx", type=int, default=None, help="override the number of spatial cells (profiling runs; "
-                    "the JSON line then names the reduced workload)")
-    ap.add_argument("--sampler", type=int, default=0, choices=[0, 1], help="1: t-channel importance sampler on the "
-                    "t-channel processes (configs 2, 3, 5); the JSON line then names it")
-    ap.add_argument("--estimator", default="standard", choices=["standard", "symmetric"], help="symmetric: the conservative "
-                    "estimator rbg_collision_symmetric (NEXT-3); the JSON line then names it")
-    ap.add_argument("--opt", action="append", default=[], help="librbg option key=value (launch geometry)")
-    args = ap.parse_args()
-    if args.impl == "reference":
-        return run_reference(args)
-    if args.path == "be":
-        return run_be_steps(args)
+# ---- launcher -------------------------------------------------------------------------------------------------------
+def free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
 
+
+def self_launch(args):
+    """`python bench.py --gpus N` with N > 1 outside torchrun: start N ranks (one per GPU) and pass the arguments on."""
+    if not args.launch_check:
+        import torch
+        have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if have < args.gpus:
+            raise SystemExit(f"bench.py: --gpus {args.gpus} requested but only {have} CUDA device(s) are visible; refusing to "
+                             f"run fewer ranks than asked for")
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")                  # the communicator lines (nranks, NVLS) go to the log
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(free_port()), str(Path(__file__).resolve()), *sys.argv[1:]]
+    raise SystemExit(subprocess.run(cmd, env=env).returncode)
+
+
+def rank_env(args):
+    """(rank, world, local_rank) from the torchrun environment; refuses a world size that contradicts --gpus."""
+    rank, world, local = (int(os.environ.get(k, d)) for k, d in (("RANK", "0"), ("WORLD_SIZE", "1"), ("LOCAL_RANK", "0")))
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; launch with --nproc-per-node {args.gpus}")
+    return rank, world, local
+
+
+def launch_check(args):
+    """--launch-check: the launcher and rank plumbing alone (gloo, no GPU work): every rank reports its environment and
+    the spatial cells it would own; rank 0 prints one JSON line.  Used by tests/test_sharding_gloo.py."""
     import torch
     import torch.distributed as dist
-    import paper_2308_04869_b200 as rbg
-    from paper_2308_04869_b200.sharding import max_over_ranks
-
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
-    torch.cuda.set_device(local)
+    from paper_2308_04869_b200.sharding import cell_range, max_over_ranks
+    rank, world, local = rank_env(args)
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist.init_process_group("gloo")
+    nx = wl.NOMINAL_NX[args.config] if args.nx is None else args.nx
+    lo, hi = cell_range(nx, rank, world) if args.scaling == "strong" else (rank * nx, (rank + 1) * nx)
+    mine = torch.tensor([rank, local, lo, hi], dtype=torch.int64)
+    rows = [torch.zeros_like(mine) for _ in range(world)]
+    if world > 1:
+        dist.all_gather(rows, mine)
+    else:
+        rows = [mine]
+    tmax = max_over_ranks(float(rank + 1))                 # the timing reduction: MAX over ranks
+    if rank == 0:
+        print(json.dumps({"launch_check": True, "n_gpus": world, "scaling": args.scaling, "nx": nx,
+                          "ranks": [[int(v) for v in r] for r in rows], "max_over_ranks": tmax,
+                          "nccl_debug": os.environ.get("NCCL_DEBUG")}))
+    if world > 1:
+        dist.destroy_process_group()
 
-    w = workloads.make(args.config, nx=args.nx, sampler=args.sampler)
+
+# ---- the collision path ----------------------------------------------------------------------------------------------
+def time_config(rbg, torch, cfg, args, steps, warmup, rank, world, local, e2e=True):
+    """Times one workload on this rank (its shard under strong scaling) and returns the measurements; the caller reduces
+    over ranks.  Timed region: `steps` sweeps, each preceded by an L2 flush, CUDA events on the launching stream."""
+    from paper_2308_04869_b200.sharding import cell_range, max_over_ranks
+    nx_all = wl.NOMINAL_NX[cfg] if args.nx is None else args.nx
+    if args.scaling == "strong" and world > 1:
+        if nx_all < world:
+            raise SystemExit(f"bench.py: config {cfg} has {nx_all} spatial cell(s), fewer than {world} ranks; use --scaling weak")
+        w = workloads.make(cfg, nx=args.nx, sampler=args.sampler, cells=cell_range(nx_all, rank, world))
+        ix_offset = w["ix_offset"]
+    else:
+        w = workloads.make(cfg, nx=args.nx, sampler=args.sampler)
+        ix_offset = rank * w["problem"]["nx"]              # weak: every rank sweeps one copy at its own global offset
     if args.nx is not None:
         w["name"] += f" [nx overridden to {args.nx}]"
     sym = args.estimator == "symmetric"
     if sym:
-        w["name"] += " [conservative (symmetric) estimator]"
+        w["name"] += " [conservative estimator]"
         w["dt"] = 0.0
     prob = w["problem"]
-    # weak scaling: every rank sweeps one copy of the workload; rank r holds global cells [r*Nx, (r+1)*Nx)
-    col = rbg.Collision(prob, fp32_kinematics=w["fp32"], ix_offset=rank * prob["nx"])
+    col = rbg.Collision(prob, fp32_kinematics=w["fp32"], ix_offset=ix_offset)
     for kv in args.opt:
         k, v = kv.split("=")
         col.set_option(k, int(v))
@@ -314,14 +375,15 @@ def main():
 
     def barrier():
         if world > 1:
+            import torch.distributed as dist
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
+    for _ in range(warmup):
         step()
     barrier()
     launches_per_step = col.last_launch_count()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     with ClockSampler(local) as cs:
         barrier()
         for e0, e1 in ev:
@@ -333,74 +395,167 @@ def main():
     clocks = cs.summary()
     times_ms = [e0.elapsed_time(e1) for e0, e1 in ev]
     t_step = max_over_ranks(sum(times_ms) / len(times_ms)) * 1e-3
-    value = world * n_evals / t_step
+    total_evals = n_evals
+    if world > 1:
+        import torch.distributed as dist
+        t = torch.tensor([float(n_evals)], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        total_evals = int(t.item())
+    res = {"w": w, "t_step": t_step, "n_evals_total": total_evals, "n_evals_rank": n_evals, "launches_per_step": launches_per_step,
+           "clocks": clocks, "times_ms": times_ms, "fl_rank": flops_per_sweep(prob, w["n_samples"])}
 
-    # ---- e2e: the same sweep through the C ABI with HOST buffers (pinned), copies inside the timing
-    f_host = torch.from_numpy(w["f"]).pin_memory()
-    c_host = torch.empty_like(f_host).pin_memory()
-    def host_call():
-        if sym:                                  # no host entry point for this estimator: pinned copies around the device call
-            fd = f_host.cuda(non_blocking=True)
-            c_host.copy_(col.collision_symmetric(fd, w["n_samples"], w["seed"]), non_blocking=True)
-            torch.cuda.synchronize()
-        else:
-            col.collision_host(f_host, w["n_samples"], w["seed"], out=c_host)
-    host_call()                                  # warm: allocates scratch
-    barrier()
-    e2e_steps = max(1, min(args.steps, 3))
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        host_call()
-    t_e2e = max_over_ranks((time.perf_counter() - t0) / e2e_steps)
-    same = bool(torch.equal(c_host.cuda(), out)) if (w["dt"] == 0 and not sym) else None
+    if e2e:
+        # the same sweep through the C ABI with HOST buffers (pinned): copies inside the timed region
+        f_host = torch.from_numpy(w["f"]).pin_memory()
+        c_host = torch.empty_like(f_host).pin_memory()
 
-    if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return
+        def host_call():
+            if sym or w["dt"] > 0:               # no host entry point for these: pinned copies around the device call
+                fd = f_host.cuda(non_blocking=True)
+                if sym:
+                    r = col.collision_symmetric(fd, w["n_samples"], w["seed"])
+                else:
+                    r, _ = col.collision_update(fd, w["dt"], w["n_samples"], w["seed"], neg_flag=flag)
+                c_host.copy_(r, non_blocking=True)
+                torch.cuda.synchronize()
+            else:
+                col.collision_host(f_host, w["n_samples"], w["seed"], out=c_host)
+        host_call()                              # warm: allocates scratch
+        barrier()
+        e2e_steps = max(1, min(steps, 3))
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            host_call()
+        res["t_e2e"] = max_over_ranks((time.perf_counter() - t0) / e2e_steps)
+        res["same"] = bool(torch.equal(c_host.cuda(), out)) if not sym else None
+        res["bytes"] = int(w["f"].nbytes)
+        del f_host, c_host
+    del f, out, flush, col
+    torch.cuda.empty_cache()
+    return res
 
-    # ---- roofline of the dominant kernel (all role launches are the same template here) ---------
-    fl = flops_per_sweep(prob, w["n_samples"])
-    t_launch = t_step / launches_per_step
-    achieved = fl / launches_per_step / t_launch / 1e12
+
+def roofline_of(rbg, torch, res, args, local, probe_cache):
+    """ALU roofline of the dominant kernel (every role launch of a sweep is an instance of one template)."""
+    w = res["w"]
+    t_launch = res["t_step"] / res["launches_per_step"]
+    achieved = res["fl_rank"] / res["launches_per_step"] / t_launch / 1e12      # this rank's flops over the max-over-ranks time
     sms = torch.cuda.get_device_properties(local).multi_processor_count
     try:
-        peaks = json.loads((ROOT / "MEASURED_PEAKS.json").read_text())
-        max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+        max_mhz = float(json.loads((ROOT / "MEASURED_PEAKS.json").read_text()).get("sm_max_mhz", 1965.0))
     except (OSError, ValueError):
         max_mhz = 1965.0
-    peak_nominal = sms * FP64_LANES_PER_SM * 2 * max_mhz * 1e6 / 1e12
-    probe = rbg.probe_alu_peak(0 if not w["fp32"] else 1, 1 << 17) * 2 / 1e12
-    if w["fp32"]:
-        peak_nominal *= 2                       # 128 fp32 lanes per SM
-    roof = {"bound": "alu", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s", "frac": achieved / peak_nominal,
-            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.config) if args.nx is None and not args.sampler and not sym else None,
-            "traffic_unit": "bytes per launch (ncu capture, profiles/r1c_chain_v2_cfg2.md)", "peak_source": f"{sms} SM x {FP64_LANES_PER_SM * (2 if w['fp32'] else 1)} FMA/clk x 2 x "
-                                            f"{max_mhz:.0f} MHz (DESIGN.md section 8)",
+    lanes = FP64_LANES_PER_SM * (2 if w["fp32"] else 1)       # 128 fp32 lanes per SM
+    peak_nominal = sms * lanes * 2 * max_mhz * 1e6 / 1e12
+    what = 1 if w["fp32"] else 0
+    if what not in probe_cache:
+        probe_cache[what] = rbg.probe_alu_peak(what, 1 << 17) * 2 / 1e12
+    probe = probe_cache[what]
+    sym = args.estimator == "symmetric"
+    traffic = NCU_TRAFFIC_BYTES_PER_LAUNCH.get(w["cfg"]) if (args.nx is None and not args.sampler and not sym and not args.opt) else None
+    return {"bound": "alu", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s", "frac": achieved / peak_nominal,
+            "traffic": traffic[0] if traffic else None,
+            "traffic_unit": f"bytes per launch (dram read + write, {traffic[1]})" if traffic else None,
+            "peak_source": f"{sms} SM x {lanes} FMA/clk x 2 x {max_mhz:.0f} MHz ({'FP32' if w['fp32'] else 'FP64'} FMA pipe; DESIGN.md section 8)",
             "peak_probe_tflops": probe, "frac_of_probe": achieved / probe,
             "kernel": "rbg::collision_symmetric_kernel" if sym else "rbg::collision_role_kernel", "launch_ms": t_launch * 1e3,
-            "flops_per_sample": fl / n_evals}
+            "flops_per_sample": res["fl_rank"] / res["n_evals_rank"]}
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-            "ms_per_step": t_step * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32" if w["fp32"] else "f64", "data": "synthetic",
-            "config": {"workload": w["name"], "cfg": args.config, "nx": prob["nx"], "n_samples": w["n_samples"],
-                       "sample_evals_per_sweep": n_evals, "f_bytes": int(w["f"].nbytes),
-                       "l2": "L2 flushed (256 MB write) between timed iterations", "parallelism": f"spatial-shard x{world}"},
-            "clocks": clocks, "gpu_launches": launches_per_step * args.steps,
-            "e2e": {"value": world * n_evals / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(w["f"].nbytes),
-                    "d2h_bytes_per_step": int(w["f"].nbytes), "ms_per_step": t_e2e * 1e3, "matches_device_path": same},
-            "roofline": roof}
-    if not args.no_cpu_baseline:
-        import oracle
-        oracle.build()
-        nx = prob["nx"]
-        cells = [int(i) for i in np.linspace(0, nx - 1, max(1, min(nx, args.cpu_cells))).astype(int)]
-        cb = oracle_leg(w, cells, "evenly spaced")
-        cb.pop("seconds")
-        line["cpu_baseline"] = cb
-    print(json.dumps(line))
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--path", default="collision", choices=["collision", "be"], help="collision: the hot path "
+                    "(default); be: the NEXT-4 kernels (moments, UPFD drift, UPFD Vlasov)")
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=HEADLINE_CONFIG, help="BASELINE.json config number (1-5; default 4, the "
+                    "largest single-GPU fp64 config); 6, 7 = the paper's own workloads")
+    ap.add_argument("--scaling", default="strong", choices=["strong", "weak"], help="N > 1: strong = the workload's spatial "
+                    "cells sharded over the ranks (default); weak = one copy of the workload per rank")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-seconds", type=float, default=3.0, help="CPU wall time per step of the reference arm (bounded sample)")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="CPU wall time of the cpu_baseline leg (bounded sample)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-config-block", action="store_true", help="skip the per-config block (configs 1, 2, 3, 5) of the N = 1 line")
+    ap.add_argument("--block-steps", type=int, default=3, help="timed sweeps per config of the per-config block")
+    ap.add_argument("--nx", type=int, default=None, help="override the number of spatial cells (profiling runs; "
+                    "the JSON line then names the reduced workload)")
+    ap.add_argument("--sampler", type=int, default=0, choices=[0, 1], help="1: t-channel importance sampler on the "
+                    "t-channel processes (configs 2, 3, 5); the JSON line then names it")
+    ap.add_argument("--estimator", default="standard", choices=["standard", "symmetric"], help="symmetric: the conservative "
+                    "estimator rbg_collision_symmetric (NEXT-3); the JSON line then names it")
+    ap.add_argument("--opt", action="append", default=[], help="librbg option key=value (launch geometry)")
+    ap.add_argument("--launch-check", action="store_true", help="launcher / rank plumbing only (gloo, no GPU work)")
+    args = ap.parse_args()
+    if args.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return self_launch(args)
+    if args.launch_check:
+        return launch_check(args)
+    if args.path == "be":
+        return run_be_steps(args)
+
+    import torch
+    import paper_2308_04869_b200 as rbg
+
+    rank, world, local = rank_env(args)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    if torch.cuda.device_count() <= local:
+        raise SystemExit(f"bench.py: rank {rank} needs CUDA device {local}, only {torch.cuda.device_count()} visible")
+    torch.cuda.set_device(local)
     if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("NCCL_DEBUG", "INFO")
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    warmup = max(args.warmup, 3)
+    res = time_config(rbg, torch, args.config, args, args.steps, warmup, rank, world, local)
+    w = res["w"]
+    value = res["n_evals_total"] / res["t_step"]
+    probe_cache = {}
+
+    if rank == 0:
+        cfgd = config_block(w, args, world)
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warmup,
+                "ms_per_step": res["t_step"] * 1e3, "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None,
+                "dtype": "f32" if w["fp32"] else "f64", "data": "synthetic", "config": cfgd,
+                "workload_detail": {"sample_evals_per_sweep": res["n_evals_total"], "f_bytes_per_rank": res["bytes"],
+                                    "nx_per_rank": w["problem"]["nx"], "roles": len(wl.roles(w["problem"]))},
+                "clocks": res["clocks"], "gpu_launches": res["launches_per_step"] * args.steps,
+                "e2e": {"value": res["n_evals_total"] / res["t_e2e"], "unit": UNIT, "h2d_bytes_per_step": res["bytes"] * world,
+                        "d2h_bytes_per_step": res["bytes"] * world, "ms_per_step": res["t_e2e"] * 1e3,
+                        "matches_device_path": res["same"],
+                        "api": "rbg_collision_host (pinned host buffers in and out)" if (w["dt"] == 0 and args.estimator == "standard")
+                               else "pinned host -> device copy, device entry point, device -> pinned host copy"},
+                "roofline": roofline_of(rbg, torch, res, args, local, probe_cache)}
+        # ---- every other BASELINE config in the same record (N = 1 only) -------------------------------------------
+        if world == 1 and not args.no_config_block and args.config == HEADLINE_CONFIG and args.nx is None and not args.opt:
+            block = {}
+            for cfg in BLOCK_CONFIGS:
+                r = time_config(rbg, torch, cfg, args, args.block_steps, 3, 0, 1, local, e2e=False)
+                roof = roofline_of(rbg, torch, r, args, local, probe_cache)
+                block[str(cfg)] = {"workload": r["w"]["name"], "dtype": "f32" if r["w"]["fp32"] else "f64",
+                                   "value": r["n_evals_total"] / r["t_step"], "unit": UNIT, "ms_per_step": r["t_step"] * 1e3,
+                                   "steps": args.block_steps, "warmup": 3, "sample_evals_per_sweep": r["n_evals_total"],
+                                   "gpu_launches_per_step": r["launches_per_step"],
+                                   "roofline": {k: roof[k] for k in ("bound", "achieved", "peak", "unit", "frac", "frac_of_probe",
+                                                                     "flops_per_sample", "launch_ms", "traffic")},
+                                   "clocks": r["clocks"]}
+            line["configs"] = block
+        if not args.no_cpu_baseline and world == 1:          # rank 0 at N = 1 only
+            cb = oracle_leg(w, args.cpu_seconds)
+            cb.pop("seconds")
+            line["cpu_baseline"] = cb
+        print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
         dist.destroy_process_group()
 
 

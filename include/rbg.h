@@ -10,8 +10,9 @@
  * estimator, sampler and arithmetic order implemented here are fixed in DESIGN.md sections 2-4.
  *
  * Conventions
- *   - hbar = c = 1 (as in the paper's own collision test); `hbar` below enters only
- *     the occupation number nbar = (2 pi hbar)^3 f / g of Eq. 18.
+ *   - c = 1.  `hbar` (1 in the paper's own collision test) enters in two places: the occupation number
+ *     nbar = (2 pi hbar)^3 f / g of Eq. 18 and the prefactor hbar^2 c |M|^2 / (64 pi^2 ...) of Eq. 16,
+ *     i.e. C scales as hbar^2 for classical species.
  *   - All pointers named *_dev are DEVICE pointers (cudaMalloc / torch CUDA tensors); pointers
  *     named *_host are HOST pointers; everything else (structs, out-params) is host memory.
  *   - Layout of f, C, f_out: one contiguous array of doubles, species-major, then spatial cell,
@@ -27,9 +28,11 @@
  *   - Errors: every int-returning entry point returns RBG_OK (0) or a negative RBG_E_* code; the
  *     text is available from rbg_last_error().  No exception crosses this boundary.  There is no
  *     CPU fallback: anything the CUDA path does not support is an error, never a slow path.
- *   - Determinism: the result is a pure function of (f, the rbg_create arguments, n_samples, seed);
- *     it does not depend on the stream, the launch geometry (rbg_set_option) or how spatial cells
- *     are partitioned across calls or GPUs (the sample stream is keyed by the global cell index).
+ *   - Determinism: the result of rbg_collision / _update / _evolve / _host is a pure function of (f, the rbg_create
+ *     arguments, n_samples, seed), bit for bit: it does not depend on the stream, on any rbg_set_option knob (CTA
+ *     size, tile size, samples per lane, gather path) or on how spatial cells are partitioned across calls or GPUs
+ *     (the sample stream is keyed by the global cell index; a lane always sums the even 32-sample blocks and the odd
+ *     ones separately, in ascending order).  rbg_collision_symmetric uses atomics: reproducible to rounding only.
  */
 #ifndef RBG_H_
 #define RBG_H_
@@ -117,7 +120,9 @@ typedef struct { int a, b, c, d; int kind; double par[4]; double sym; int sample
  * is NULL and rbg_last_error(NULL) has the text).  Rejects: non-positive grid counts,
  * pmax <= pmin, negative mass, stat not in {0,+1,-1}, g <= 0, species index out of range,
  * unknown kind, sampler or flags, a sampler that does not fit the kind or an inelastic process, a process
- * written a + b -> b + a, no CUDA device. */
+ * written a + b -> b + a, no CUDA device.  RBG_E_UNSUPPORTED: a species that takes part in a process has a momentum
+ * cell centre of (numerically) zero energy, sqrt(|p|^2 + m^2) <= 1e-6 of the smallest cell width -- a massless species
+ * on an odd grid symmetric about 0: Eq. 16 carries 1/p^0 of the grid particle, which diverges there. */
 int rbg_create(rbg_handle** out, const rbg_spatial_grid* grid, int n_species, const rbg_species* species,
                const rbg_momentum_grid* momentum_grids /* [n_species] */, int n_process,
                const rbg_process* processes, double hbar, int flags);
@@ -128,22 +133,25 @@ int rbg_create(rbg_handle** out, const rbg_spatial_grid* grid, int n_species, co
 int rbg_collision(rbg_handle* h, const double* f_dev, double* C_dev, int n_samples, uint64_t seed,
                   void* cuda_stream);
 
-/* Fused explicit Euler step of Eq. 27: f_out_dev = f_dev + dt * C[f_dev].  *neg_flag_dev (one int in
- * device memory, zeroed by the caller) is incremented by the number of cells with f_out < 0; f_out
- * is stored unclamped (policy is the caller's).  f_out_dev must not alias f_dev. */
+/* Fused explicit Euler step: f_out_dev = f_dev + dt * C[f_dev].  `dt` is the EFFECTIVE step: Eq. 27 of the paper's
+ * splitting reads (1/3) df/dt = C, so a caller reproducing it passes 3 * (the time step), as
+ * rbg_be_step does; the same holds for rbg_collision_evolve.  *neg_flag_dev (one int in device memory, zeroed by the
+ * caller) is incremented by the number of cells with f_out < 0; f_out is stored unclamped (policy is the caller's).
+ * f_out_dev must not alias f_dev. */
 int rbg_collision_update(rbg_handle* h, const double* f_dev, double* f_out_dev, double dt, int* neg_flag_dev,
                          int n_samples, uint64_t seed, void* cuda_stream);
 
-/* n_steps explicit Euler steps of Eq. 27 in a row (the paper's collision test runs 25 000 of them,
- * PAPER.md:504): f <- f + dt * C[f], step k (k = 0 .. n_steps-1) drawing its samples with seed + k, i.e.
+/* n_steps explicit Euler steps in a row (the paper's collision test runs 25 000 of them,
+ * PAPER.md:504): f <- f + dt * C[f] with dt the effective step (see rbg_collision_update), step k (k = 0 .. n_steps-1) drawing its samples with seed + k, i.e.
  * exactly n_steps calls of rbg_collision_update ping-ponging between f_dev and scratch_dev (rbg_f_elems()
  * doubles, caller-owned, must not overlap f_dev).  On return (stream order) f_dev holds the final state;
  * scratch_dev is clobbered.  *neg_flag_dev accumulates the negative cells of every step.  n_steps >= 0. */
 int rbg_collision_evolve(rbg_handle* h, double* f_dev, double* scratch_dev, double dt, int n_steps,
                          int* neg_flag_dev, int n_samples, uint64_t seed, void* cuda_stream);
 
-/* NEXT-3: the conservative ("symmetric") estimator of the same collision term (PAPER.md:257 names "the symmetric
- * sampling method [57]" without defining it; the reading implemented is DESIGN.md section 4c / R25).  Same samples as
+/* NEXT-3: this repo's conservative estimator of the same collision term.  PAPER.md:257 names "the symmetric sampling
+ * method [57]" without defining it and Ref. [57] is not part of PAPER.md, so whether this is that method cannot be
+ * checked; the reading implemented is DESIGN.md section 4c / R25.  Same samples as
  * rbg_collision, but the net rate of every sample is credited to all four particles of the sampled reaction -- + to the
  * cells of the grid particle and its partner, - to the cells of the other pair -- and C of a species is the average of
  * the equivalent estimators, so that what one cell gains another loses sample by sample: particle number is conserved
@@ -228,13 +236,6 @@ void rbg_destroy(rbg_handle* h);
  * the achieved rate.  what: 0 = fp64 FMA, 1 = fp32 FMA, 2 = int32 multiply-add.  *ops_per_s counts
  * one FMA as one operation.  Used by bench.py for the live roofline denominator. */
 int rbg_probe_alu_peak(int what, int iters, double* ops_per_s, void* cuda_stream);
-
-/* Measurement helper for the instruction-issue bound: one CTA of warps_per_sm warps per SM
- * loops over n_fp64 DFMA + n_imad IMAD + n_lop3 LOP3 on independent registers; *cycles_per_iter is the SM clock
- * span of one loop iteration of the whole CTA (divide by warps_per_sm / 4 for cycles per warp-iteration per
- * scheduler).  Supported mixes (n_fp64, n_imad, n_lop3): (8,0,0) (0,8,0) (0,0,8) (0,4,4) (0,8,8) (8,2,2) (8,4,4)
- * (8,8,0) (8,0,8) (8,8,8).  Synchronous, default stream. */
-int rbg_probe_issue_mix(int n_fp64, int n_imad, int n_lop3, int warps_per_sm, int iters, double* cycles_per_iter);
 
 /* Diagnostic: compares the kernels' own fp64 and fp32 divide / reciprocal / square-root sequences
  * (the round-to-nearest fast paths without range checks) bit for bit with the

@@ -76,7 +76,6 @@ _SIGNATURES = {
     "rbg_last_error": (C.c_char_p, [C.c_void_p]),
     "rbg_destroy": (None, [C.c_void_p]),
     "rbg_probe_alu_peak": (C.c_int, [C.c_int, C.c_int, C.POINTER(C.c_double), C.c_void_p]),
-    "rbg_probe_issue_mix": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_double)]),
     "rbg_selftest_math": (C.c_int, [C.c_uint64, C.c_uint32, C.POINTER(C.c_uint64)]),
 }
 
@@ -110,13 +109,6 @@ def probe_alu_peak(what: int, iters: int = 1 << 16, stream=None) -> float:
     """FMA/s (one FMA = one op) of a register-resident chain: 0 fp64, 1 fp32, 2 int32."""
     out = C.c_double()
     _check(load_library().rbg_probe_alu_peak(what, iters, C.byref(out), _stream_ptr(stream)))
-    return out.value
-
-
-def probe_issue_mix(n_fp64: int, n_imad: int, n_lop3: int, warps_per_sm: int = 16, iters: int = 20000) -> float:
-    """rbg_probe_issue_mix: SM cycles per loop iteration of a CTA of warps_per_sm warps."""
-    out = C.c_double()
-    _check(load_library().rbg_probe_issue_mix(n_fp64, n_imad, n_lop3, warps_per_sm, iters, C.byref(out)))
     return out.value
 
 

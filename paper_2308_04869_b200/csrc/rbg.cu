@@ -67,6 +67,13 @@ int fail(rbg_handle* h, int code, const std::string& msg) {
     return code;
 }
 
+// Makes the handle's device current for the duration of an entry point and restores the caller's on every exit path.
+struct DeviceGuard {
+    int prev = -1; int want;
+    explicit DeviceGuard(int w) : want(w) { cudaGetDevice(&prev); if (prev != want) cudaSetDevice(want); }
+    ~DeviceGuard() { if (prev >= 0 && prev != want) cudaSetDevice(prev); }
+};
+
 #define RBG_CUDA(h, call)                                                                          \
     do {                                                                                           \
         cudaError_t e_ = (call);                                                                   \
@@ -124,19 +131,32 @@ rbg::RoleParams<R> make_role_params(const rbg_handle& H, const Role& r) {
     k.qG = (R)(16.0 * g4d * dA * CA * CA);
     k.qcd = r.kind >= RBG_M2_QCD_Q1Q2 ? r.kind - RBG_M2_QCD_Q1Q2 : 0;
     k.rho = (R)(r.cg / r.cl);
-    k.symV2 = r.sym * V2 * r.cl;
+    k.symV2 = (H.hbar * H.hbar) * (r.sym * V2) * r.cl;     // hbar^2 c of Eq. 16, c = 1
     for (int i = 0; i < 4; ++i) k.np[i] = (int)H.np[r.s[i]];
     k.role = r.index;
     return k;
 }
 
+// Opt a kernel in to the device's largest dynamic shared-memory size once per (template instantiation, device) instead of
+// before every launch; the function-local static makes the cache per instantiation.
+constexpr int kMaxDevices = 64;
+template <typename K>
+cudaError_t ensure_max_smem(K kern, int device, int max_optin) {
+    static bool done[kMaxDevices] = {};
+    if (device >= 0 && device < kMaxDevices && done[device]) return cudaSuccess;
+    const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, max_optin);
+    if (e == cudaSuccess && device >= 0 && device < kMaxDevices) done[device] = true;
+    return e;
+}
+struct LaunchCtx { int device, max_optin; cudaStream_t st; };
+
 template <typename R, int KIND, bool Q, bool SMEM, int MAXT, int SPL, bool TCH, bool INEL>
 cudaError_t launch_one(const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp, int grid, int threads, size_t smem,
-                       cudaStream_t st) {
+                       const LaunchCtx& cx) {
     auto kern = rbg::collision_role_kernel<R, KIND, Q, SMEM, MAXT, SPL, TCH, INEL>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const cudaError_t e = ensure_max_smem(kern, cx.device, cx.max_optin);
     if (e != cudaSuccess) return e;
-    kern<<<grid, threads, smem, st>>>(rp, lp);
+    kern<<<grid, threads, smem, cx.st>>>(rp, lp);
     return cudaGetLastError();
 }
 
@@ -144,7 +164,7 @@ cudaError_t launch_one(const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp
 // (up to 128 registers per thread); CTAs of up to 1024 threads evaluate 1 (64 registers).
 template <typename R, int KIND, bool Q, bool SMEM, bool TCH>
 cudaError_t launch_geo(int spl, const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp, int grid, int threads,
-                       size_t smem, cudaStream_t st) {
+                       size_t smem, const LaunchCtx& st) {
     if (threads > 512) return launch_one<R, KIND, Q, SMEM, 1024, 1, TCH, false>(rp, lp, grid, threads, smem, st);
     if (spl == 2) return launch_one<R, KIND, Q, SMEM, 512, 2, TCH, false>(rp, lp, grid, threads, smem, st);
     return launch_one<R, KIND, Q, SMEM, 512, 1, TCH, false>(rp, lp, grid, threads, smem, st);
@@ -153,7 +173,7 @@ cudaError_t launch_geo(int spl, const rbg::RoleParams<R>& rp, const rbg::LaunchP
 // inel: general roles (species 3,4 differ from 1,2) run one geometry (up to 16 warps, 2 samples per lane), uniform sampler
 template <typename R, int KIND, bool TCH>
 cudaError_t launch_kq(bool q, bool smem_path, bool inel, int spl, const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp,
-                      int grid, int threads, size_t smem, cudaStream_t st) {
+                      int grid, int threads, size_t smem, const LaunchCtx& st) {
     if (inel) {
         if (q) return smem_path ? launch_one<R, KIND, true, true, 512, 2, false, true>(rp, lp, grid, threads, smem, st)
                                 : launch_one<R, KIND, true, false, 512, 2, false, true>(rp, lp, grid, threads, smem, st);
@@ -168,7 +188,8 @@ cudaError_t launch_kq(bool q, bool smem_path, bool inel, int spl, const rbg::Rol
 
 template <typename R>
 int run_roles(rbg_handle* h, const double* f, double* out, bool update, double dt, int* neg_flag, int n_samples,
-              uint64_t seed, cudaStream_t st) {
+              uint64_t seed, cudaStream_t stream) {
+    const LaunchCtx st{h->device, h->max_smem_optin, stream};
     h->last_launches = 0;
     // last role per species (update mode counts negatives there); species with no role: C = 0 / f_out = f
     std::vector<int> first_role(h->n_species, -1), last_role(h->n_species, -1);
@@ -180,11 +201,11 @@ int run_roles(rbg_handle* h, const double* f, double* out, bool update, double d
         if (first_role[s] >= 0) continue;
         const size_t n = (size_t)h->nx * h->np[s];
         if (update) {
-            rbg::copy_count_kernel<<<h->sm_count * 4, 256, 0, st>>>(f + h->sp_off[s], out + h->sp_off[s], n, neg_flag);
+            rbg::copy_count_kernel<<<h->sm_count * 4, 256, 0, stream>>>(f + h->sp_off[s], out + h->sp_off[s], n, neg_flag);
             RBG_CUDA(h, cudaGetLastError());
             ++h->last_launches;
         } else {
-            RBG_CUDA(h, cudaMemsetAsync(out + h->sp_off[s], 0, n * sizeof(double), st));
+            RBG_CUDA(h, cudaMemsetAsync(out + h->sp_off[s], 0, n * sizeof(double), stream));
         }
     }
     for (size_t ir = 0; ir < h->roles.size(); ++ir) {
@@ -263,13 +284,9 @@ int run(rbg_handle* h, const double* f, double* out, bool update, double dt, int
     if (n_samples <= 0) return fail(h, RBG_E_INVALID_ARG, "n_samples must be positive");
     if (update && !neg_flag) return fail(h, RBG_E_INVALID_ARG, "null neg_flag_dev");
     cudaStream_t st = (cudaStream_t)stream;
-    int dev = -1;
-    RBG_CUDA(h, cudaGetDevice(&dev));
-    if (dev != h->device) RBG_CUDA(h, cudaSetDevice(h->device));
-    int rc = (h->flags & RBG_FP32_KINEMATICS) ? run_roles<float>(h, f, out, update, dt, neg_flag, n_samples, seed, st)
-                                               : run_roles<double>(h, f, out, update, dt, neg_flag, n_samples, seed, st);
-    if (dev != h->device && dev >= 0) cudaSetDevice(dev);
-    return rc;
+    DeviceGuard guard(h->device);
+    return (h->flags & RBG_FP32_KINEMATICS) ? run_roles<float>(h, f, out, update, dt, neg_flag, n_samples, seed, st)
+                                            : run_roles<double>(h, f, out, update, dt, neg_flag, n_samples, seed, st);
 }
 
 }  // namespace
@@ -277,11 +294,11 @@ int run(rbg_handle* h, const double* f, double* out, bool update, double dt, int
 namespace {
 template <int KIND>
 cudaError_t launch_sym(bool q, bool inel, bool csmem, const rbg::RoleParams<double>& rp, const rbg::LaunchParams& lp,
-                       const rbg::SymParams& sp, int grid, size_t smem, cudaStream_t st) {
+                       const rbg::SymParams& sp, int grid, size_t smem, const LaunchCtx& cx) {
     auto go = [&](auto kern) -> cudaError_t {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        const cudaError_t e = ensure_max_smem(kern, cx.device, cx.max_optin);
         if (e != cudaSuccess) return e;
-        kern<<<grid, 512, smem, st>>>(rp, lp, sp);
+        kern<<<grid, 512, smem, cx.st>>>(rp, lp, sp);
         return cudaGetLastError();
     };
     if (q) {
@@ -336,6 +353,30 @@ int rbg_create(rbg_handle** out, const rbg_spatial_grid* grid, int n_species, co
         const int idx[4] = {p.a, p.b, p.c, p.d};
         for (int j = 0; j < 4; ++j)
             if (idx[j] < 0 || idx[j] >= n_species) { delete h; return fail(nullptr, RBG_E_INVALID_ARG, "process " + std::to_string(i) + ": species index out of range"); }
+        // 1/p^0 of Eq. 16: a species that takes part in a process must have no momentum cell whose centre
+        // has (numerically) zero energy -- a massless species on an odd grid symmetric about 0 (reading R14)
+        for (int j = 0; j < 4; ++j) {
+            const rbg_momentum_grid& G = mg[idx[j]];
+            double e2 = species[idx[j]].mass * species[idx[j]].mass, wmin = 0.0;
+            for (int d = 0; d < 3; ++d) {
+                const double w = (G.pmax[d] - G.pmin[d]) / (double)G.n[d];
+                // centre nearest to 0 along this axis: cell floor(-pmin / w) or one of its neighbours
+                const double c0 = std::floor(-G.pmin[d] / w);
+                double best = HUGE_VAL;
+                for (double c = c0 - 1.0; c <= c0 + 1.0; c += 1.0) {
+                    if (c < 0.0 || c > (double)(G.n[d] - 1)) continue;
+                    best = std::fmin(best, std::fabs(std::fma(c + 0.5, w, G.pmin[d])));
+                }
+                if (best == HUGE_VAL) best = std::fmin(std::fabs(std::fma(0.5, w, G.pmin[d])), std::fabs(std::fma((double)G.n[d] - 0.5, w, G.pmin[d])));
+                e2 += best * best;
+                wmin = d == 0 ? w : std::fmin(wmin, w);
+            }
+            if (!(std::sqrt(e2) > 1e-6 * wmin)) {
+                delete h;
+                return fail(nullptr, RBG_E_UNSUPPORTED, "process " + std::to_string(i) + ": species " + std::to_string(idx[j]) +
+                            " has a momentum cell centre with zero energy (massless, centre at p = 0): 1/p0 of Eq. 16 diverges there");
+            }
+        }
         if (p.kind < RBG_M2_CONST || p.kind > RBG_M2_QCD_GG) { delete h; return fail(nullptr, RBG_E_INVALID_ARG, "process " + std::to_string(i) + ": unknown |M|^2 kind"); }
         const bool elastic = p.c == p.a && p.d == p.b;
         if (!elastic && p.c == p.b && p.d == p.a) { delete h; return fail(nullptr, RBG_E_INVALID_ARG, "process " + std::to_string(i) + ": write a+b -> b+a as a+b -> a+b (t and u would be ambiguous)"); }
@@ -427,12 +468,10 @@ int rbg_collision_symmetric(rbg_handle* h, const double* f_dev, double* C_dev, i
     if (h->flags & RBG_FP32_KINEMATICS) return fail(h, RBG_E_UNSUPPORTED, "rbg_collision_symmetric is fp64 only");
     for (const Role& r : h->roles)
         if (r.sampler != RBG_SAMPLER_UNIFORM) return fail(h, RBG_E_UNSUPPORTED, "rbg_collision_symmetric supports the uniform sampler only");
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    int dev = -1;
-    RBG_CUDA(h, cudaGetDevice(&dev));
-    if (dev != h->device) RBG_CUDA(h, cudaSetDevice(h->device));
+    DeviceGuard guard(h->device);
+    const LaunchCtx st{h->device, h->max_smem_optin, (cudaStream_t)cuda_stream};
     h->last_launches = 0;
-    RBG_CUDA(h, cudaMemsetAsync(C_dev, 0, h->f_elems * sizeof(double), st));
+    RBG_CUDA(h, cudaMemsetAsync(C_dev, 0, h->f_elems * sizeof(double), st.st));
     auto dp3 = [&](int s) {
         const rbg_momentum_grid& g = h->grids[s];
         return ((g.pmax[0] - g.pmin[0]) / g.n[0]) * ((g.pmax[1] - g.pmin[1]) / g.n[1]) * ((g.pmax[2] - g.pmin[2]) / g.n[2]);
@@ -493,7 +532,6 @@ int rbg_collision_symmetric(rbg_handle* h, const double* f_dev, double* C_dev, i
         if (e != cudaSuccess) return fail(h, RBG_E_CUDA, std::string("kernel launch: ") + cudaGetErrorString(e));
         ++h->last_launches;
     }
-    if (dev != h->device && dev >= 0) cudaSetDevice(dev);
     return RBG_OK;
 }
 
@@ -505,6 +543,7 @@ int rbg_collision_evolve(rbg_handle* h, double* f_dev, double* scratch_dev, doub
     const size_t bytes = h->f_elems * sizeof(double);
     const char *a = (const char*)f_dev, *b = (const char*)scratch_dev;
     if (a < b + bytes && b < a + bytes) return fail(h, RBG_E_INVALID_ARG, "scratch_dev overlaps f_dev");
+    DeviceGuard guard(h->device);
     double *cur = f_dev, *nxt = scratch_dev;
     int launches = 0;
     for (int k = 0; k < n_steps; ++k) {
@@ -521,6 +560,7 @@ int rbg_collision_evolve(rbg_handle* h, double* f_dev, double* scratch_dev, doub
 int rbg_collision_host(rbg_handle* h, const double* f_host, double* C_host, int n_samples, uint64_t seed) {
     if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
     if (!f_host || !C_host) return fail(h, RBG_E_INVALID_ARG, "null buffer");
+    DeviceGuard guard(h->device);
     if (h->scratch_elems < h->f_elems) {
         cudaFree(h->scratch_f); cudaFree(h->scratch_c); h->scratch_f = h->scratch_c = nullptr; h->scratch_elems = 0;
         RBG_CUDA(h, cudaMalloc(&h->scratch_f, h->f_elems * sizeof(double)));
@@ -581,11 +621,6 @@ rbg::SpeciesTables species_tables(const rbg_handle* h, int s) {
     t.mass = h->species[s].mass; t.charge = h->species[s].charge;
     return t;
 }
-struct DeviceGuard {
-    int prev = -1; int want;
-    explicit DeviceGuard(int w) : want(w) { cudaGetDevice(&prev); if (prev != want) cudaSetDevice(want); }
-    ~DeviceGuard() { if (prev >= 0 && prev != want) cudaSetDevice(prev); }
-};
 }  // namespace
 
 namespace {
@@ -782,6 +817,29 @@ int rbg_be_step(rbg_handle* h, double* f_dev, double* scratch_dev, const rbg_be_
     if (a < b + bytes && b < a + bytes) return fail(h, RBG_E_INVALID_ARG, "scratch_dev overlaps f_dev");
     if (p->do_vlasov && (!E_dev || !B_dev)) return fail(h, RBG_E_INVALID_ARG, "do_vlasov needs E_dev and B_dev");
     if (p->do_collision && !neg_flag_dev) return fail(h, RBG_E_INVALID_ARG, "do_collision needs neg_flag_dev");
+    // everything the sub-steps would refuse is refused here, before the first launch touches f_dev
+    if (p->do_collision != 0 && p->do_collision != 1 && p->do_collision != 2) return fail(h, RBG_E_INVALID_ARG, "do_collision must be 0, 1 or 2");
+    if (p->do_collision && p->n_samples <= 0) return fail(h, RBG_E_INVALID_ARG, "n_samples must be positive");
+    if (p->do_collision == 2) {
+        if (h->flags & RBG_FP32_KINEMATICS) return fail(h, RBG_E_UNSUPPORTED, "rbg_collision_symmetric is fp64 only");
+        for (const Role& r : h->roles)
+            if (r.sampler != RBG_SAMPLER_UNIFORM) return fail(h, RBG_E_UNSUPPORTED, "rbg_collision_symmetric supports the uniform sampler only");
+    }
+    if ((p->do_drift || p->do_vlasov) && !(p->dt >= 0.0)) return fail(h, RBG_E_INVALID_ARG, "dt must be >= 0");
+    if (p->do_drift) {
+        if (h->ix_offset != 0) return fail(h, RBG_E_UNSUPPORTED, "the drift stencil needs the whole spatial domain on one GPU (no ghost-layer exchange)");
+        if (!(p->zeta >= 0.0 && p->zeta <= 1.0)) return fail(h, RBG_E_INVALID_ARG, "zeta must be in [0, 1]");
+        for (int d = 0; d < 3; ++d) {
+            if (!(p->dx[d] > 0.0)) return fail(h, RBG_E_INVALID_ARG, "dx must be positive");
+            if (p->bc[d] != 0 && p->bc[d] != 1) return fail(h, RBG_E_INVALID_ARG, "bc must be 0 (wall) or 1 (periodic)");
+        }
+        if (p->zeta != 0.0)
+            for (int s = 0; s < h->n_species; ++s)
+                for (int d = 0; d < 3; ++d)
+                    if (p->bc[d] == 0 && std::fabs(h->grids[s].pmin[d] + h->grids[s].pmax[d]) > 1e-12 * (h->grids[s].pmax[d] - h->grids[s].pmin[d]))
+                        return fail(h, RBG_E_UNSUPPORTED, "reflecting walls need momentum grids symmetric about 0 (the mirrored momentum must be a grid cell)");
+    }
+    DeviceGuard guard(h->device);
     double *cur = f_dev, *nxt = scratch_dev;
     int launches = 0, rc;
     if (p->do_drift) {
@@ -853,39 +911,6 @@ int rbg_probe_alu_peak(int what, int iters, double* ops_per_s, void* cuda_stream
     }
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(buf);
     *ops_per_s = (double)ctas * threads * 8.0 * (double)iters / (best * 1e-3);
-    return RBG_OK;
-}
-
-int rbg_probe_issue_mix(int n_fp64, int n_imad, int n_lop3, int warps_per_sm, int iters, double* cycles_per_iter) {
-    if (!cycles_per_iter || iters <= 0 || warps_per_sm < 1 || warps_per_sm > 32) return fail(nullptr, RBG_E_INVALID_ARG, "bad probe arguments");
-    int dev = 0, sms = 0;
-    RBG_CUDA(nullptr, cudaGetDevice(&dev));
-    RBG_CUDA(nullptr, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    void (*kern)(double*, int, long long*) = nullptr;
-    const int key = n_fp64 * 100 + n_imad * 10 + n_lop3;
-    switch (key) {
-        case 800: kern = rbg::issue_mix_kernel<8, 0, 0>; break;
-        case 80:  kern = rbg::issue_mix_kernel<0, 8, 0>; break;
-        case 8:   kern = rbg::issue_mix_kernel<0, 0, 8>; break;
-        case 44:  kern = rbg::issue_mix_kernel<0, 4, 4>; break;
-        case 88:  kern = rbg::issue_mix_kernel<0, 8, 8>; break;
-        case 822: kern = rbg::issue_mix_kernel<8, 2, 2>; break;
-        case 844: kern = rbg::issue_mix_kernel<8, 4, 4>; break;
-        case 880: kern = rbg::issue_mix_kernel<8, 8, 0>; break;
-        case 808: kern = rbg::issue_mix_kernel<8, 0, 8>; break;
-        case 888: kern = rbg::issue_mix_kernel<8, 8, 8>; break;
-        default: return fail(nullptr, RBG_E_INVALID_ARG, "unsupported mix (see include/rbg.h)");
-    }
-    double* out = nullptr; long long* cyc = nullptr;
-    RBG_CUDA(nullptr, cudaMalloc(&out, (size_t)sms * 1024 * sizeof(double)));
-    RBG_CUDA(nullptr, cudaMalloc(&cyc, sizeof(long long)));
-    for (int rep = 0; rep < 2; ++rep) kern<<<sms, warps_per_sm * 32>>>(out, iters, cyc);
-    cudaError_t e = cudaDeviceSynchronize();
-    long long h = 0;
-    if (e == cudaSuccess) e = cudaMemcpy(&h, cyc, sizeof h, cudaMemcpyDeviceToHost);
-    cudaFree(out); cudaFree(cyc);
-    if (e != cudaSuccess) return fail(nullptr, RBG_E_CUDA, cudaGetErrorString(e));
-    *cycles_per_iter = (double)h / iters;
     return RBG_OK;
 }
 

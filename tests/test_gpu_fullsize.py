@@ -24,14 +24,28 @@ def _check_cells(w, C, cells, fp32):
             assert np.any(C_ref[sl] != 0)
 
 
-@pytest.mark.parametrize("cfg,cells", [(2, (0, 255, 511)), (3, (17,)), (4, (0, 32767))])
-def test_fullsize_sampled_parity(cfg, cells):
+def _sample_cells(problem, n=16):
+    """At least n spatial cells of a full-size problem: the first and the last two (both ends of every species block in the
+    species-major layout), the two cells either side of the first CTA-wave boundary (one CTA per SM, 148 SMs, tiles of at
+    most 512 momentum cells of the first species), the two in the middle, and an even spread over the rest."""
+    nx = problem["nx"]
+    tiles = -(-int(np.prod(problem["grids"][0]["n"])) // 512)
+    wave = max(1, 148 // tiles)
+    want = {0, 1, wave - 1, wave, nx // 2 - 1, nx // 2, nx - 2, nx - 1}
+    want |= {int(v) for v in np.linspace(0, nx - 1, n)}
+    return sorted(c for c in want if 0 <= c < nx)
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 4])
+def test_fullsize_sampled_parity(cfg):
     import paper_2308_04869_b200 as rbg
     w = workloads.make(cfg)
     col = rbg.Collision(w["problem"])
     f = torch.from_numpy(w["f"]).cuda()
     C = col.collision(f, w["n_samples"], w["seed"])
     torch.cuda.synchronize()
+    cells = _sample_cells(w["problem"])
+    assert len(cells) >= 16
     _check_cells(w, C.cpu().numpy(), cells, False)
     # properties that hold at any size: finite everywhere, every spatial cell written
     assert bool(torch.isfinite(C).all())
@@ -50,7 +64,9 @@ def test_fullsize_config5_fused_update_fp32():
     torch.cuda.synchronize()
     got = out.cpu().numpy()
     orc = oracle.Oracle(w["problem"], use_float=True)
-    for ix in (0, 4095):
+    cells = _sample_cells(w["problem"])
+    assert len(cells) >= 16
+    for ix in cells:
         C_ref, mag = oracle_C_and_scale(orc, w["f"], w["n_samples"], w["seed"], ix_begin=ix, ix_end=ix + 1)
         for s in range(orc.n_species):
             sl = slice(orc.sp_off[s] + ix * orc.np[s], orc.sp_off[s] + (ix + 1) * orc.np[s])
@@ -117,14 +133,14 @@ def test_fullsize_config2_tchannel_sampler():
 
 def test_fullsize_config7_qgp_sampled_parity():
     """Workload 7 (the paper's quark-gluon-plasma scenario, 21^3 x 11^3, 70 roles) at full size: the oracle recomputes
-    two spatial cells; every cell is finite and written."""
+    16+ spatial cells; every cell is finite and written."""
     import paper_2308_04869_b200 as rbg
     w = workloads.make(7)
     col = rbg.Collision(w["problem"])
     C = col.collision(torch.from_numpy(w["f"]).cuda(), w["n_samples"], w["seed"])
     torch.cuda.synchronize()
     assert col.last_launch_count() == 70
-    _check_cells(w, C.cpu().numpy(), (0, 9260), False)
+    _check_cells(w, C.cpu().numpy(), _sample_cells(w["problem"]), False)
     assert bool(torch.isfinite(C).all())
 
 

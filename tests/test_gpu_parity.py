@@ -101,9 +101,16 @@ def test_result_independent_of_launch_geometry_and_gather_path():
     w = workloads.make(2, nx=2, np_side=12, n_samples=80)
     base, _ = gpu_C(w["problem"], w["f"], w["n_samples"], w["seed"])
     for opts in ([("warps_per_cta", 3), ("p1_per_cta", 5)], [("warps_per_cta", 8), ("p1_per_cta", 1000)],
-                 [("gather", 2)], [("gather", 2), ("warps_per_cta", 1), ("p1_per_cta", 1)]):
+                 [("gather", 2)], [("gather", 2), ("warps_per_cta", 1), ("p1_per_cta", 1)],
+                 [("samples_per_lane", 1)], [("warps_per_cta", 32)], [("samples_per_lane", 1), ("gather", 2), ("warps_per_cta", 5)]):
         other, _ = gpu_C(w["problem"], w["f"], w["n_samples"], w["seed"], options=opts)
         assert np.array_equal(base, other), opts
+    # more than two 32-sample blocks per lane, a ragged last block, fp32 kinematics: the lane sums must not depend on SPL
+    for fp32, N in ((False, 200), (True, 333)):
+        base, _ = gpu_C(w["problem"], w["f"], N, 9, fp32=fp32)
+        for opts in ([("samples_per_lane", 1)], [("warps_per_cta", 32)], [("samples_per_lane", 2), ("warps_per_cta", 7)]):
+            other, _ = gpu_C(w["problem"], w["f"], N, 9, fp32=fp32, options=opts)
+            assert np.array_equal(base, other), (fp32, N, opts)
 
 
 def test_spatial_sharding_reproduces_the_single_device_result():
@@ -121,6 +128,28 @@ def test_spatial_sharding_reproduces_the_single_device_result():
             parts_ref.append(full[offs[s]:offs[s] + 5 * npc].reshape(5, npc)[lo:hi].reshape(-1))
         shard, _ = gpu_C(prob, np.concatenate(parts_in), w["n_samples"], w["seed"], ix_offset=lo)
         assert np.array_equal(shard, np.concatenate(parts_ref))
+
+
+@pytest.mark.skipif(torch.cuda.device_count() < 2, reason="needs two CUDA devices")
+def test_two_device_shards_concatenate_to_the_single_device_result():
+    """What `bench.py --gpus 2` does, in one process: each device holds half of the spatial cells (workloads.make(cells=...)),
+    the handle is created on that device with the shard's global offset; the pieces concatenate bit-identically.  Also
+    exercises the device guard: the second handle is called while device 0 is current."""
+    rbg = _rbg()
+    from paper_2308_04869_b200 import sharding
+    w = workloads.make(2, nx=6, np_side=8, n_samples=48)
+    full, _ = gpu_C(w["problem"], w["f"], w["n_samples"], w["seed"])
+    pieces = []
+    for r in range(2):
+        ws = workloads.make(2, nx=6, np_side=8, n_samples=48, cells=sharding.cell_range(6, r, 2))
+        with torch.cuda.device(r):
+            col = rbg.Collision(ws["problem"], ix_offset=ws["ix_offset"])
+            ft = torch.from_numpy(ws["f"]).cuda()
+        torch.cuda.set_device(0)
+        C = col.collision(ft, ws["n_samples"], ws["seed"], stream=torch.cuda.current_stream(r))
+        torch.cuda.synchronize(r)
+        pieces.append(C.cpu().numpy())
+    assert np.array_equal(sharding.unshard(w["problem"], pieces), full)
 
 
 def test_fused_update_and_negativity_flag():
@@ -199,6 +228,35 @@ def test_edge_cases():
     C_ref, mag = oracle_C_and_scale(orc, w0["f"], 40, 5)
     C, _ = gpu_C(w0["problem"], w0["f"], 40, 5)
     assert_parity(C, C_ref, mag, TOL64, "massless")
+    assert np.all(np.isfinite(C))
+    # a massless species with a cell centre at p = 0 (odd grid, symmetric box): 1/p0 of Eq. 16 diverges -> refused, as the
+    # oracle refuses it; with a mass, or when the species takes part in no process, the same grid is accepted
+    w1 = workloads.make(3, nx=1, np_side=7, n_samples=8)
+    w1["problem"]["species"][3]["mass"] = 0.0
+    with pytest.raises(rbg.RbgError, match="zero energy"):
+        rbg.Collision(w1["problem"])
+    with pytest.raises(ValueError):
+        oracle.Oracle(w1["problem"])
+    idle = dict(w1["problem"], processes=[p for p in w1["problem"]["processes"] if 3 not in (p["a"], p["b"])])
+    assert rbg.Collision(idle).n_roles == oracle.Oracle(idle).n_roles
+    w1["problem"]["species"][3]["mass"] = 0.01
+    C, _ = gpu_C(w1["problem"], w1["f"], 8, 5)
+    assert np.all(np.isfinite(C))
+
+
+def test_hbar_enters_the_prefactor_squared_and_the_occupation_number():
+    """Eq. 16: hbar^2 c |M|^2 / (64 pi^2 ...); Eq. 18: nbar = (2 pi hbar)^3 f / g.  Parity at hbar != 1 for a
+    quantum problem, and C(hbar) = hbar^2 C(1) exactly (a power of two) for a classical one."""
+    w = workloads.make(3, nx=2, np_side=8, n_samples=64)
+    prob = dict(w["problem"], hbar=0.25)
+    orc = oracle.Oracle(prob)
+    C_ref, mag = oracle_C_and_scale(orc, w["f"], 64, 11)
+    C, _ = gpu_C(prob, w["f"], 64, 11)
+    assert_parity(C, C_ref, mag, TOL64, "hbar = 0.25, quantum")
+    w = workloads.make(1, nx=2, np_side=8, n_samples=64)
+    C1, _ = gpu_C(w["problem"], w["f"], 64, 11)
+    Ch, _ = gpu_C(dict(w["problem"], hbar=0.25), w["f"], 64, 11)
+    assert np.array_equal(Ch, 0.0625 * C1) and np.any(C1 != 0)
 
 
 def test_argument_errors():

@@ -86,13 +86,24 @@ def qgp_processes(par, n_flavours=3):
     return procs
 
 
+NOMINAL_NX = {1: 1, 2: 8 ** 3, 3: 4 ** 3, 4: 32 ** 3, 5: 16 ** 3, 6: 1, 7: 21 ** 3}
+
+
 def make(cfg: int, nx: int | None = None, n_samples: int | None = None, np_side: int | None = None,
-         sampler: int = 0):
-    """Return dict(name, problem, f, n_samples, seed, dt, fp32).  ``nx``/``n_samples``/``np_side``
+         sampler: int = 0, cells: tuple | None = None):
+    """Return dict(name, problem, f, n_samples, seed, dt, fp32, ix_offset, nx_global).  ``nx``/``n_samples``/``np_side``
     override the config's spatial cell count / sample count / momentum cells per axis (tests use
     reduced sizes; bench.py uses the defaults).  ``sampler`` = 1 asks for the t-channel importance
-    sampler on every process whose |M|^2 kind has the t-channel shape (configs 2, 3, 5)."""
+    sampler on every process whose |M|^2 kind has the t-channel shape (configs 2, 3, 5).
+    ``cells`` = (lo, hi) builds only spatial cells [lo, hi) of the workload (a rank's shard): the
+    per-cell random numbers are drawn for the whole domain and sliced, so the shards of any partition concatenate to
+    the unsharded f bit for bit; problem["nx"] is then hi - lo and ix_offset = lo."""
     rng = np.random.Generator(np.random.PCG64(INPUT_SEED_BASE + cfg))
+    nx_all = NOMINAL_NX[cfg] if nx is None else int(nx)
+    lo, hi = (0, nx_all) if cells is None else (int(cells[0]), int(cells[1]))
+    if not (0 <= lo < hi <= nx_all):
+        raise ValueError(f"cells {cells} outside [0, {nx_all})")
+    sl = slice(lo, hi)
     seed = MC_SEED_BASE + cfg
     dt, fp32 = 0.0, False
     if cfg == 1:
@@ -104,7 +115,7 @@ def make(cfg: int, nx: int | None = None, n_samples: int | None = None, np_side:
         procs = [_elastic(0, 0, KIND_CONST, [1.0])]
         P = cell_centres(grids[0])
         E = np.sqrt((P * P).sum(1) + 1.0)
-        f = np.exp(-E / 1.0)[None, :] * (1.0 + 0.1 * (2.0 * rng.random((nx, P.shape[0])) - 1.0))
+        f = np.exp(-E / 1.0)[None, :] * (1.0 + 0.1 * (2.0 * rng.random((nx, P.shape[0]))[sl] - 1.0))
         fs = [f]
         name = "cfg1: 1 classical species, const |M|^2, MJ T=1 + 10% noise"
     elif cfg in (2, 5):
@@ -120,7 +131,7 @@ def make(cfg: int, nx: int | None = None, n_samples: int | None = None, np_side:
         for s, g in zip(species, grids):
             P = cell_centres(g)
             E = np.sqrt((P * P).sum(1) + s["mass"] ** 2)
-            dens = 1.0 + 0.1 * (2.0 * rng.random(nx) - 1.0)          # seeded density perturbation n(x)
+            dens = 1.0 + 0.1 * (2.0 * rng.random(nx)[sl] - 1.0)      # seeded density perturbation n(x)
             fs.append(dens[:, None] * np.exp(-(E - s["mass"]) / 1.0)[None, :])   # rest mass subtracted
         name = "cfg2: e-/H+ screened Coulomb" if cfg == 2 else "cfg5: e-/H+ fused Euler update, fp32 kinematics"
         if cfg == 5:
@@ -143,7 +154,7 @@ def make(cfg: int, nx: int | None = None, n_samples: int | None = None, np_side:
             pabs = np.sqrt((P * P).sum(1))
             E = np.sqrt(pabs ** 2 + s["mass"] ** 2)
             nbar = equilibrium_nbar(E, 0.3, s["stat"])
-            aniso = 1.0 + 0.2 * (P[:, 2] / pabs)[None, :] * (2.0 * rng.random((nx, P.shape[0])) - 1.0)
+            aniso = 1.0 + 0.2 * (P[:, 2] / pabs)[None, :] * (2.0 * rng.random((nx, P.shape[0]))[sl] - 1.0)
             fs.append(nbar[None, :] / kappa * aniso)
         name = "cfg3: 3 fermions + 2 bosons, t-channel g^4 s^2/(t-mD^2)^2"
     elif cfg == 4:
@@ -158,7 +169,7 @@ def make(cfg: int, nx: int | None = None, n_samples: int | None = None, np_side:
             Q = P.copy(); Q[:, 2] -= shift
             return np.exp(-np.sqrt((Q * Q).sum(1) + 1.0) / 0.5)
         prof = 0.5 * (mj(2.0) + mj(-2.0))                    # two counter-streaming beams along z
-        dens = 1.0 + 0.1 * (2.0 * rng.random(nx) - 1.0)
+        dens = 1.0 + 0.1 * (2.0 * rng.random(nx)[sl] - 1.0)
         fs = [dens[:, None] * prof[None, :]]
         name = "cfg4: 1 classical species, two counter-streaming beams, const |M|^2"
     elif cfg == 6:
@@ -177,7 +188,7 @@ def make(cfg: int, nx: int | None = None, n_samples: int | None = None, np_side:
                  _elastic(0, 1, KIND_ISO_DSIGMA, [0.01])]
         P = cell_centres(grids[0])
         inside = ((P * P).sum(1) < 1.0).astype(np.float64)
-        fs = [np.tile(f0 * inside, (nx, 1)) for f0 in (0.2, 0.4)]
+        fs = [np.tile(f0 * inside, (hi - lo, 1)) for f0 in (0.2, 0.4)]
         dt = 0.0002 / 0.197
         name = "cfg6: paper's collision test (Eq. 46-48): 2 classical species m=0.3, const dsigma/dOmega 1/20/0.01"
     elif cfg == 7:
@@ -203,7 +214,7 @@ def make(cfg: int, nx: int | None = None, n_samples: int | None = None, np_side:
             E = np.sqrt((P * P).sum(1) + s["mass"] ** 2)
             kappa = (2.0 * np.pi) ** 3 / s["g"]
             nbar = equilibrium_nbar(E, 0.4, s["stat"]) * (0.5 if s["stat"] == 1 else 1.0)
-            aniso = 1.0 + 0.2 * (P[:, 2] / E)[None, :] * (2.0 * rng.random((nx, P.shape[0])) - 1.0)
+            aniso = 1.0 + 0.2 * (P[:, 2] / E)[None, :] * (2.0 * rng.random((nx, P.shape[0]))[sl] - 1.0)
             fs.append(nbar[None, :] / kappa * aniso)
         name = "cfg7: quark-gluon plasma, 7 species, all Table III processes (34 processes, 70 roles)"
     else:
@@ -213,10 +224,10 @@ def make(cfg: int, nx: int | None = None, n_samples: int | None = None, np_side:
             if p["kind"] in (KIND_COULOMB_SCREENED, KIND_TCHAN_S2):
                 p["sampler"] = int(sampler)
         name += " [t-channel importance sampler]"
-    problem = dict(nx=int(nx), species=species, grids=grids, processes=procs, hbar=1.0)
+    problem = dict(nx=int(hi - lo), species=species, grids=grids, processes=procs, hbar=1.0)
     f = np.concatenate([np.ascontiguousarray(a, dtype=np.float64).reshape(-1) for a in fs])
     return dict(cfg=cfg, name=name, problem=problem, f=f, n_samples=int(N if n_samples is None else n_samples),
-                seed=int(seed), dt=float(dt), fp32=bool(fp32))
+                seed=int(seed), dt=float(dt), fp32=bool(fp32), ix_offset=int(lo), nx_global=int(nx_all))
 
 
 def roles(problem):
