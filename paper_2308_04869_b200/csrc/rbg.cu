@@ -8,6 +8,9 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
+#include <set>
+#include <type_traits>
 #include <utility>
 #include <string>
 #include <vector>
@@ -137,53 +140,57 @@ rbg::RoleParams<R> make_role_params(const rbg_handle& H, const Role& r) {
     return k;
 }
 
-// Opt a kernel in to the device's largest dynamic shared-memory size once per (template instantiation, device) instead of
-// before every launch; the function-local static makes the cache per instantiation.
-constexpr int kMaxDevices = 64;
+// Opt a kernel in to the device's largest dynamic shared-memory size once per (kernel, device) instead of before every
+// launch.  Keyed by the kernel's address: kernels of one signature share a function-pointer type.
 template <typename K>
 cudaError_t ensure_max_smem(K kern, int device, int max_optin) {
-    static bool done[kMaxDevices] = {};
-    if (device >= 0 && device < kMaxDevices && done[device]) return cudaSuccess;
+    static std::mutex mu;
+    static std::set<std::pair<const void*, int>> done;
+    const std::pair<const void*, int> key(reinterpret_cast<const void*>(kern), device);
+    std::lock_guard<std::mutex> lock(mu);
+    if (done.count(key)) return cudaSuccess;
     const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, max_optin);
-    if (e == cudaSuccess && device >= 0 && device < kMaxDevices) done[device] = true;
+    if (e == cudaSuccess) done.insert(key);
     return e;
 }
 struct LaunchCtx { int device, max_optin; cudaStream_t st; };
 
-template <typename R, int KIND, bool Q, bool SMEM, int MAXT, int SPL, bool TCH, bool INEL>
+template <typename R, int KIND, bool Q, bool SMEM, int MAXT, int SPL, bool TCH, bool INEL, bool PIPE = false>
 cudaError_t launch_one(const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp, int grid, int threads, size_t smem,
                        const LaunchCtx& cx) {
-    auto kern = rbg::collision_role_kernel<R, KIND, Q, SMEM, MAXT, SPL, TCH, INEL>;
+    auto kern = rbg::collision_role_kernel<R, KIND, Q, SMEM, MAXT, SPL, TCH, INEL, PIPE>;
     const cudaError_t e = ensure_max_smem(kern, cx.device, cx.max_optin);
     if (e != cudaSuccess) return e;
     kern<<<grid, threads, smem, cx.st>>>(rp, lp);
     return cudaGetLastError();
 }
 
-// geometry variant: CTAs of up to 512 threads evaluate SPL = 1 or 2 samples per lane and iteration
-// (up to 128 registers per thread); CTAs of up to 1024 threads evaluate 1 (64 registers).
-template <typename R, int KIND, bool Q, bool SMEM, bool TCH>
+// Launch geometries: CTAs of up to 8 warps evaluate SPL = 4 samples per lane and loop iteration (up to 255 registers per
+// thread), up to 16 warps SPL = 2 (128 registers), up to 32 warps SPL = 1 (64 registers; elastic roles only).  All three
+// keep the whole register file of an SM busy with one CTA; results are bit-identical (fixed lane summation order).
+template <typename R, int KIND, bool Q, bool SMEM, bool TCH, bool INEL>
 cudaError_t launch_geo(int spl, const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp, int grid, int threads,
                        size_t smem, const LaunchCtx& st) {
-    if (threads > 512) return launch_one<R, KIND, Q, SMEM, 1024, 1, TCH, false>(rp, lp, grid, threads, smem, st);
-    if (spl == 2) return launch_one<R, KIND, Q, SMEM, 512, 2, TCH, false>(rp, lp, grid, threads, smem, st);
-    return launch_one<R, KIND, Q, SMEM, 512, 1, TCH, false>(rp, lp, grid, threads, smem, st);
+    if (spl == 4) return launch_one<R, KIND, Q, SMEM, 256, 4, TCH, INEL>(rp, lp, grid, threads, smem, st);
+    if constexpr (!INEL)
+        if (spl == 1) return launch_one<R, KIND, Q, SMEM, 1024, 1, TCH, INEL>(rp, lp, grid, threads, smem, st);
+    return launch_one<R, KIND, Q, SMEM, 512, 2, TCH, INEL>(rp, lp, grid, threads, smem, st);
 }
 
-// inel: general roles (species 3,4 differ from 1,2) run one geometry (up to 16 warps, 2 samples per lane), uniform sampler
+// inel: general roles (species 3,4 differ from 1,2), uniform sampler only
 template <typename R, int KIND, bool TCH>
 cudaError_t launch_kq(bool q, bool smem_path, bool inel, int spl, const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp,
                       int grid, int threads, size_t smem, const LaunchCtx& st) {
     if (inel) {
-        if (q) return smem_path ? launch_one<R, KIND, true, true, 512, 2, false, true>(rp, lp, grid, threads, smem, st)
-                                : launch_one<R, KIND, true, false, 512, 2, false, true>(rp, lp, grid, threads, smem, st);
-        return smem_path ? launch_one<R, KIND, false, true, 512, 2, false, true>(rp, lp, grid, threads, smem, st)
-                         : launch_one<R, KIND, false, false, 512, 2, false, true>(rp, lp, grid, threads, smem, st);
+        if (q) return smem_path ? launch_geo<R, KIND, true, true, false, true>(spl, rp, lp, grid, threads, smem, st)
+                                : launch_geo<R, KIND, true, false, false, true>(spl, rp, lp, grid, threads, smem, st);
+        return smem_path ? launch_geo<R, KIND, false, true, false, true>(spl, rp, lp, grid, threads, smem, st)
+                         : launch_geo<R, KIND, false, false, false, true>(spl, rp, lp, grid, threads, smem, st);
     }
-    if (q) return smem_path ? launch_geo<R, KIND, true, true, TCH>(spl, rp, lp, grid, threads, smem, st)
-                            : launch_geo<R, KIND, true, false, TCH>(spl, rp, lp, grid, threads, smem, st);
-    return smem_path ? launch_geo<R, KIND, false, true, TCH>(spl, rp, lp, grid, threads, smem, st)
-                     : launch_geo<R, KIND, false, false, TCH>(spl, rp, lp, grid, threads, smem, st);
+    if (q) return smem_path ? launch_geo<R, KIND, true, true, TCH, false>(spl, rp, lp, grid, threads, smem, st)
+                            : launch_geo<R, KIND, true, false, TCH, false>(spl, rp, lp, grid, threads, smem, st);
+    return smem_path ? launch_geo<R, KIND, false, true, TCH, false>(spl, rp, lp, grid, threads, smem, st)
+                     : launch_geo<R, KIND, false, false, TCH, false>(spl, rp, lp, grid, threads, smem, st);
 }
 
 template <typename R>
@@ -212,13 +219,41 @@ int run_roles(rbg_handle* h, const double* f, double* out, bool update, double d
         const Role& r = h->roles[ir];
         const rbg::RoleParams<R> rp = make_role_params<R>(*h, r);
         const bool inel = !r.elastic;
-        int warps = h->opt_warps > 0 ? h->opt_warps : 16;
-        if (inel && warps > 16) warps = 16;
-        const int spl = h->opt_spl > 0 ? h->opt_spl : 2;
+        // samples per lane: the option, else the default of the arithmetic type; CTAs wider than its geometry allows
+        // fall to the next one (8 / 16 / 32 warps for 4 / 2 / 1 samples per lane; general roles: at most 16 warps)
+        // default (measured, profiles/r2_collision.md): 4 for fp64 roles with large momentum grids staged in shared memory,
+        // 2 otherwise
         const int np1 = rp.np[0];
-        long work = (long)h->nx * np1;
-        int T = h->opt_p1_per_cta > 0 ? h->opt_p1_per_cta : (int)std::min<long>(512, std::max<long>(warps, work / ((long)h->sm_count * 8)));
-        T = std::min(T, np1);
+        int spl = h->opt_spl > 0 ? h->opt_spl
+                  : (sizeof(R) == 8 && np1 >= 4096 && r.kind < RBG_M2_QCD_Q1Q2 ? 4 : 2);
+        int warps = h->opt_warps > 0 ? h->opt_warps : 32 / spl;
+        if (inel && warps > 16) warps = 16;
+        if (warps > 16) spl = 1;
+        else if (warps > 8 && spl == 4) spl = 2;
+        if (inel && spl == 1) spl = 2;
+        // Tile size T (momentum cells per CTA; one CTA per SM at a time): a CTA stages its tables (about 2 us + bytes at
+        // 100 GB/s) and then takes ceil(T / warps) rounds of one p1 per warp (a round of n_samples samples per warp at
+        // about 5.7e8 samples/s per SM); the grid of nx * tiles CTAs runs in ceil(nx * tiles / SMs) waves.  Take the
+        // tiling with the smallest waves * (rounds + staging), preferring larger tiles on near-ties.  T <= 512.
+        int T = h->opt_p1_per_cta;
+        if (T <= 0) {
+            size_t tab_bytes = 0;
+            for (int i = 1; i < 4; ++i) {
+                bool first = true;
+                for (int j = 1; j < i; ++j) first = first && r.s[j] != r.s[i];
+                if (first) tab_bytes += (size_t)rp.np[i] * sizeof(R);
+            }
+            const double staging = (2e-6 + (double)tab_bytes / 1e11) * 5.7e8 / ((double)n_samples * warps);
+            double best_cost = -1.0;
+            const int t_lo = (np1 + 511) / 512, t_hi = std::max(t_lo, std::min(4096, (np1 + warps - 1) / warps));
+            for (int tiles = t_lo; tiles <= t_hi; ++tiles) {
+                const int Tt = (np1 + tiles - 1) / tiles;
+                const long ctas = (long)h->nx * ((np1 + Tt - 1) / Tt);
+                const double cost = (double)((ctas + h->sm_count - 1) / h->sm_count) * ((double)((Tt + warps - 1) / warps) + staging);
+                if (best_cost < 0.0 || cost < 0.995 * best_cost) { best_cost = cost; T = Tt; }
+            }
+        }
+        T = std::max(1, std::min(T, np1));
         // shared memory: [16 B mbarrier][T doubles][one f table per distinct species among slots 2, 3, 4, 16-B aligned]
         rbg::LaunchParams lp;
         std::memset(&lp, 0, sizeof lp);
@@ -589,7 +624,7 @@ int rbg_set_option(rbg_handle* h, const char* key, int value) {
     if (!h || !key) return fail(h, RBG_E_INVALID_ARG, "null argument");
     const std::string k(key);
     if (k == "warps_per_cta") { if (value < 0 || value > 32) return fail(h, RBG_E_INVALID_ARG, "warps_per_cta must be 0 (auto) or 1..32"); h->opt_warps = value; }
-    else if (k == "samples_per_lane") { if (value < 0 || value > 2) return fail(h, RBG_E_INVALID_ARG, "samples_per_lane must be 0 (auto), 1 or 2"); h->opt_spl = value; }
+    else if (k == "samples_per_lane") { if (value != 0 && value != 1 && value != 2 && value != 4) return fail(h, RBG_E_INVALID_ARG, "samples_per_lane must be 0 (auto), 1, 2 or 4"); h->opt_spl = value; }
     else if (k == "p1_per_cta") { if (value < 0) return fail(h, RBG_E_INVALID_ARG, "p1_per_cta must be >= 0 (0 = auto)"); h->opt_p1_per_cta = value; }
     else if (k == "gather") { if (value < 0 || value > 2) return fail(h, RBG_E_INVALID_ARG, "gather must be 0, 1 or 2"); h->opt_gather = value; }
     else return fail(h, RBG_E_INVALID_ARG, "unknown option " + k);
@@ -680,7 +715,7 @@ int rbg_moments(rbg_handle* h, const double* f_dev, double* M_dev, double* total
         }
         const bool one_team = g.team == rbg::MOM_THREADS && g.n_stages * g.group <= rbg::MOM_RED;
         auto launch = [&](auto kern) -> cudaError_t {
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem);
+            const cudaError_t e = ensure_max_smem(kern, h->device, h->max_smem_optin);
             if (e != cudaSuccess) return e;
             kern<<<g.ctas, rbg::MOM_THREADS, g.smem, st>>>(fs, tb, h->nx, Ms, g.group, g.n_stages, g.team, g.lead);
             return cudaSuccess;
@@ -796,10 +831,10 @@ int rbg_vlasov_step(rbg_handle* h, const double* f_dev, double* f_out_dev, doubl
             continue;
         }
         if (g.team >= nyz) {
-            RBG_CUDA(h, cudaFuncSetAttribute(rbg::vlasov_upfd_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
+            RBG_CUDA(h, ensure_max_smem(rbg::vlasov_upfd_kernel<1>, h->device, h->max_smem_optin));
             rbg::vlasov_upfd_kernel<1><<<g.ctas, rbg::MOM_THREADS, g.smem, st>>>(fs, os, tb, vp, g.group, g.n_stages, g.team, g.lead);
         } else {
-            RBG_CUDA(h, cudaFuncSetAttribute(rbg::vlasov_upfd_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
+            RBG_CUDA(h, ensure_max_smem(rbg::vlasov_upfd_kernel<4>, h->device, h->max_smem_optin));
             rbg::vlasov_upfd_kernel<4><<<g.ctas, rbg::MOM_THREADS, g.smem, st>>>(fs, os, tb, vp, g.group, g.n_stages, g.team, g.lead);
         }
         RBG_CUDA(h, cudaGetLastError());

@@ -240,8 +240,12 @@ def test_edge_cases():
     idle = dict(w1["problem"], processes=[p for p in w1["problem"]["processes"] if 3 not in (p["a"], p["b"])])
     assert rbg.Collision(idle).n_roles == oracle.Oracle(idle).n_roles
     w1["problem"]["species"][3]["mass"] = 0.01
-    C, _ = gpu_C(w1["problem"], w1["f"], 8, 5)
+    f1 = np.nan_to_num(w1["f"], nan=0.1)             # the generator's anisotropy factor p_z/|p| is 0/0 at the centre cell
+    orc = oracle.Oracle(w1["problem"])
+    C_ref, mag = oracle_C_and_scale(orc, f1, 8, 5)
+    C, _ = gpu_C(w1["problem"], f1, 8, 5)
     assert np.all(np.isfinite(C))
+    assert_parity(C, C_ref, mag, TOL64, "odd grid, light species")
 
 
 def test_hbar_enters_the_prefactor_squared_and_the_occupation_number():
