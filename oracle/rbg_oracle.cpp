@@ -188,18 +188,36 @@ template <> struct OctantPoly<float> {
 // O6: unit vector, uniform on the sphere, from one word for cos(theta) and 24 bits for phi.
 //   nz = usym(x3 | odd), odd = lowest bit that usym keeps (so |nz| < 1 and the lattice is symmetric);
 //   sin(theta) = sqrt(1 - nz^2);
-//   phi = (k + 1/2) 2 pi / 2^24, k = 24-bit integer: quadrant q = k >> 22, second-half flag b = bit 21,
-//   in-octant index r = k & (2^21 - 1), folded r' = b ? 2^21 - 1 - r : r, a = (r' + 1/2)(pi/4)/2^21,
-//   (cos, sin) of the angle inside the quadrant = b ? (sin a, cos a) : (cos a, sin a), then the
-//   exact rotation by q * pi/2.
+//   azimuth from the 24-bit integer k: quadrant q = k >> 22, second-half flag b = bit 21, in-octant index
+//   r = k & (2^21 - 1), folded r' = b ? 2^21 - 1 - r : r; (cos, sin) of the angle a in (0, pi/4) inside the octant (below);
+//   (cos, sin) of the angle inside the quadrant = b ? (sin a, cos a) : (cos a, sin a), then the exact rotation by q * pi/2.
+// float chain:  a = (r' + 1/2)(pi/4)/2^21, cos a and sin a from the octant polynomials.
+// double chain (chain v3): the lattice keeps the top 19 bits of r', r19 = r' >> 2 = 2^10 hi + lo, and the angle is split
+//   a = alpha + beta,  alpha = (2^10 hi) A1,  beta = (lo + 1/2) A1,  A1 = (pi/4) / 2^19  (beta = fma(lo, A1, A1/2)),
+//   cos a = cos(alpha) cos(beta) - sin(alpha) sin(beta),  sin a = sin(alpha) cos(beta) + cos(alpha) sin(beta),
+//   each written as one fma of a product, with cos / sin of alpha and of beta from the octant polynomials (both angles
+//   lie in [0, pi/4)).  alpha takes 512 values and beta 1024, so an implementation may tabulate the four factors.
+template <typename R> inline void octant_angle(uint32_t rf21, R& ca, R& sa);
+template <> inline void octant_angle<float>(uint32_t rf21, float& ca, float& sa) {
+    const float A1 = (float)0x1.921fb54442d18p-22;       // (pi/4) / 2^21
+    const float A0 = (float)0x1.921fb54442d18p-23;       // half a step
+    OctantPoly<float>::eval(rfma<float>((float)rf21, A1, A0), ca, sa);
+}
+template <> inline void octant_angle<double>(uint32_t rf21, double& ca, double& sa) {
+    const double A1 = 0x1.921fb54442d18p-20;             // (pi/4) / 2^19
+    const double A0 = 0x1.921fb54442d18p-21;             // half a step
+    const uint32_t r19 = rf21 >> 2, hi = r19 >> 10, lo = r19 & 1023u;
+    double cA, sA, cB, sB;
+    OctantPoly<double>::eval((double)(hi << 10) * A1, cA, sA);
+    OctantPoly<double>::eval(std::fma((double)lo, A1, A0), cB, sB);
+    ca = std::fma(cA, cB, -(sA * sB));
+    sa = std::fma(sA, cB, cA * sB);
+}
 template <typename R> inline void azimuth(uint32_t k24, R& cphi, R& sphi) {
     const uint32_t q = k24 >> 22, b = (k24 >> 21) & 1u, r = k24 & 0x1FFFFFu;
     const uint32_t rf = b ? 0x1FFFFFu - r : r;
-    const R A1 = (R)0x1.921fb54442d18p-22;       // (pi/4) / 2^21
-    const R A0 = (R)0x1.921fb54442d18p-23;       // half a step
-    const R a = rfma<R>((R)rf, A1, A0);
     R ca, sa;
-    OctantPoly<R>::eval(a, ca, sa);
+    octant_angle<R>(rf, ca, sa);
     const R c1 = b ? sa : ca, s1 = b ? ca : sa;  // angle in (0, pi/2)
     switch (q) {
         case 0:  cphi = c1;  sphi = s1;  break;

@@ -139,7 +139,8 @@ def test_threshold_and_degenerate_samples_contribute_zero():
 def test_direction_against_library_trigonometry():
     """O6: the polynomial, libm-free direction equals
     (sin(theta) cos(phi), sin(theta) sin(phi), cos(theta)) with mpmath's cos/sin (40 digits), for
-    cos(theta) = (x3|1) 2^-31 - 1 (odd lattice: never 0 or +-1) and phi = (k + 1/2) 2 pi / 2^24, k from the low bytes of x0..x2:
+    cos(theta) = (x3|1) 2^-31 - 1 (odd lattice: never 0 or +-1) and phi = (k + 1/2) 2 pi / 2^24, k from the low bytes of x0..x2
+    (float chain), phi = ((k >> 2) + 1/2) 2 pi / 2^22 (double chain v3: the lattice keeps the top 22 bits of k):
     to 4e-16 in double and 3e-7 in float; exactly unit length to rounding; every octant, both ends
     of every octant and the symmetric partner (k -> 2^24 - 1 - k mirrors phi -> -phi exactly)."""
     rng = np.random.default_rng(7)
@@ -149,9 +150,10 @@ def test_direction_against_library_trigonometry():
         for x3 in [0, 1, 2 ** 31, 2 ** 32 - 1] + [int(v) for v in rng.integers(0, 2 ** 32, 3)]:
             hi = [int(v) << 8 for v in rng.integers(0, 2 ** 24, 3)]          # p2 bits: must not matter
             words = [hi[0] | (k >> 16), hi[1] | ((k >> 8) & 255), hi[2] | (k & 255), x3]
-            phi = (mpmath.mpf(k) + 0.5) * 2 * mpmath.pi / 2 ** 24        # 40 digits: no rounding of the angle
-            cphi, sphi = float(mpmath.cos(phi)), float(mpmath.sin(phi))
             for use_float, tol in ((False, 4e-16), (True, 3e-7)):
+                # 40 digits: no rounding of the angle
+                phi = (mpmath.mpf(k) + 0.5) * 2 * mpmath.pi / 2 ** 24 if use_float else (mpmath.mpf(k >> 2) + 0.5) * 2 * mpmath.pi / 2 ** 22
+                cphi, sphi = float(mpmath.cos(phi)), float(mpmath.sin(phi))
                 ct = ((x3 >> 8) | 1) * 2.0 ** -23 - 1.0 if use_float else (x3 | 1) * 2.0 ** -31 - 1.0
                 assert 0.0 < abs(ct) < 1.0
                 st = math.sqrt(float(1 - Fraction(ct) ** 2))              # 1 - ct^2 exactly, one rounding
