@@ -57,6 +57,7 @@ struct rbg_handle {
     // per-species device tables for the moment / drift / Vlasov kernels: 1/E_p and v = p/E_p per momentum cell
     std::vector<double*> tab_iE, tab_v;
     double* charges_dev = nullptr;
+    double2* dir_tab = nullptr;          // direction table of the double chain (rbg::kDirTabEntries entries)
     // scratch for the host entry point
     double *scratch_f = nullptr, *scratch_c = nullptr;
     size_t scratch_elems = 0;
@@ -155,10 +156,10 @@ cudaError_t ensure_max_smem(K kern, int device, int max_optin) {
 }
 struct LaunchCtx { int device, max_optin; cudaStream_t st; };
 
-template <typename R, int KIND, bool Q, bool SMEM, int MAXT, int SPL, bool TCH, bool INEL, bool PIPE = false>
+template <typename R, int KIND, bool Q, bool SMEM, int MAXT, int SPL, bool TCH, bool INEL>
 cudaError_t launch_one(const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp, int grid, int threads, size_t smem,
                        const LaunchCtx& cx) {
-    auto kern = rbg::collision_role_kernel<R, KIND, Q, SMEM, MAXT, SPL, TCH, INEL, PIPE>;
+    auto kern = rbg::collision_role_kernel<R, KIND, Q, SMEM, MAXT, SPL, TCH, INEL>;
     const cudaError_t e = ensure_max_smem(kern, cx.device, cx.max_optin);
     if (e != cudaSuccess) return e;
     kern<<<grid, threads, smem, cx.st>>>(rp, lp);
@@ -257,7 +258,7 @@ int run_roles(rbg_handle* h, const double* f, double* out, bool update, double d
         // shared memory: [16 B mbarrier][T doubles][one f table per distinct species among slots 2, 3, 4, 16-B aligned]
         rbg::LaunchParams lp;
         std::memset(&lp, 0, sizeof lp);
-        const size_t head = 16 + (((size_t)T * 8 + 15) & ~(size_t)15);
+        const size_t head = 16 + (sizeof(R) == 8 ? (size_t)rbg::kDirTabBytes : 0) + (((size_t)T * 8 + 15) & ~(size_t)15);
         size_t tabs = 0;
         for (int i = 1; i < 4; ++i) {
             int owner = i;
@@ -276,6 +277,7 @@ int run_roles(rbg_handle* h, const double* f, double* out, bool update, double d
         for (int i = 0; i < 4; ++i) lp.fb[i] = f + h->sp_off[r.s[i]];
         lp.out_base = out + h->sp_off[r.s[0]];
         lp.nx_local = h->nx; lp.ix_offset = h->ix_offset; lp.n_samples = n_samples;
+        lp.dir_tab = h->dir_tab;
         lp.key0 = (uint32_t)seed; lp.key1 = (uint32_t)(seed >> 32);
         for (int rr = 0; rr < 10; ++rr) {
             lp.rk[2 * rr] = lp.key0 + (uint32_t)rr * 0x9E3779B9u;
@@ -477,6 +479,10 @@ int rbg_create(rbg_handle** out, const rbg_spatial_grid* grid, int n_species, co
         }
         h->tab_iE.push_back(d_iE); h->tab_v.push_back(d_v);
     }
+    // direction table of the double chain (O6): evaluated once on the device
+    if (cudaMalloc(&h->dir_tab, rbg::kDirTabBytes) != cudaSuccess) { rbg_destroy(h); return fail(nullptr, RBG_E_CUDA, "allocating the direction table failed"); }
+    rbg::dir_table_kernel<<<(rbg::kDirTabEntries + 255) / 256, 256>>>(h->dir_tab);
+    if (cudaGetLastError() != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess) { rbg_destroy(h); return fail(nullptr, RBG_E_CUDA, "building the direction table failed"); }
     if (cudaMalloc(&h->charges_dev, n_species * sizeof(double)) != cudaSuccess ||
         cudaMemcpy(h->charges_dev, charges.data(), n_species * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess) {
         rbg_destroy(h);
@@ -535,9 +541,10 @@ int rbg_collision_symmetric(rbg_handle* h, const double* f_dev, double* C_dev, i
             if (owner == i) { sp.ctab_own[i] = 1; sp.ctab_off[i] = (int)tabs; tabs += ((size_t)rp.np[i] * 8 + 15) & ~(size_t)15; }
             else { sp.ctab_own[i] = 0; sp.ctab_off[i] = sp.ctab_off[owner]; }
         }
-        const bool csmem = tabs <= (size_t)h->max_smem_optin;
+        const bool csmem = rbg::kDirTabBytes + tabs <= (size_t)h->max_smem_optin;
         rbg::LaunchParams lp;
         std::memset(&lp, 0, sizeof lp);
+        lp.dir_tab = h->dir_tab;
         for (int i = 0; i < 4; ++i) lp.fb[i] = f_dev + h->sp_off[r.s[i]];
         lp.nx_local = h->nx; lp.ix_offset = h->ix_offset; lp.n_samples = n_samples;
         lp.key0 = (uint32_t)seed; lp.key1 = (uint32_t)(seed >> 32);
@@ -555,7 +562,7 @@ int rbg_collision_symmetric(rbg_handle* h, const double* f_dev, double* C_dev, i
         if (grid > 0x7fffffffL) return fail(h, RBG_E_UNSUPPORTED, "grid too large");
         bool q = false;
         for (int i = 0; i < 4; ++i) q = q || h->species[r.s[i]].stat != 0;
-        const size_t smem = csmem ? tabs : 0;
+        const size_t smem = rbg::kDirTabBytes + (csmem ? tabs : 0);
         cudaError_t e;
         switch (r.kind) {
             case RBG_M2_CONST: e = launch_sym<rbg::KIND_CONST>(q, !r.elastic, csmem, rp, lp, sp, (int)grid, smem, st); break;
@@ -639,6 +646,7 @@ void rbg_destroy(rbg_handle* h) {
     for (double* p : h->tab_iE) cudaFree(p);
     for (double* p : h->tab_v) cudaFree(p);
     cudaFree(h->charges_dev);
+    cudaFree(h->dir_tab);
     delete h;
 }
 
