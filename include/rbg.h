@@ -225,8 +225,7 @@ uint64_t rbg_sample_evals(const rbg_handle* h, int n_samples);
 int rbg_last_launch_count(const rbg_handle* h);
 /* Launch geometry / gather path knobs (results do not depend on them; 0 = automatic).  key:
  * "warps_per_cta" (1..32), "p1_per_cta" (momentum cells per CTA, >= 1), "samples_per_lane"
- * (1, 2 or 4: samples a lane evaluates per loop iteration; CTAs of more than 8 warps use at most 2, of more than 16
- * warps 1),
+ * (1 or 2: samples a lane evaluates per loop iteration; CTAs of more than 16 warps use 1),
  * "gather" (1 shared memory, 2 global/L2).  Returns RBG_E_INVALID_ARG for an unknown key or value. */
 int rbg_set_option(rbg_handle* h, const char* key, int value);
 /* Text of the last error on this handle (or of the last failed rbg_create if h is NULL). */
@@ -237,6 +236,16 @@ void rbg_destroy(rbg_handle* h);
  * the achieved rate.  what: 0 = fp64 FMA, 1 = fp32 FMA, 2 = int32 multiply-add.  *ops_per_s counts
  * one FMA as one operation.  Used by bench.py for the live roofline denominator. */
 int rbg_probe_alu_peak(int what, int iters, double* ops_per_s, void* cuda_stream);
+
+/* Diagnostic of the CHECKED build (librbg_checked.so, `python -m paper_2308_04869_b200.build --checked`, -DRBG_CHECKED): the
+ * kernels then verify every index into a shared-memory or global table, the shared-memory layout of every CTA and, in the
+ * persistent moments / Vlasov kernels, that a ring slot still holds the unit a warp believes it is consuming when it starts
+ * and when it finishes reading it.  counts[0..7] receive the failures seen since the library was loaded, by class: f-table
+ * index, tile index, direction-table index, output index, shared-memory layout, ring-slot contents, stencil / moment
+ * index, conservative-estimator index; all must be 0.  Synchronises the device.  In the normal build the checks are
+ * compiled out and the call returns RBG_E_UNSUPPORTED with all counts 0. */
+#define RBG_SELFCHECK_CLASSES 8
+int rbg_selfcheck_failures(uint64_t* counts /* [RBG_SELFCHECK_CLASSES], host */);
 
 /* Diagnostic: compares the kernels' own fp64 and fp32 divide / reciprocal / square-root sequences
  * (the round-to-nearest fast paths without range checks) bit for bit with the

@@ -77,11 +77,21 @@ _SIGNATURES = {
     "rbg_destroy": (None, [C.c_void_p]),
     "rbg_probe_alu_peak": (C.c_int, [C.c_int, C.c_int, C.POINTER(C.c_double), C.c_void_p]),
     "rbg_selftest_math": (C.c_int, [C.c_uint64, C.c_uint32, C.POINTER(C.c_uint64)]),
+    "rbg_selfcheck_failures": (C.c_int, [C.POINTER(C.c_uint64)]),
 }
 
 
 def exported_symbols():
     return sorted(_SIGNATURES)
+
+
+def use_checked_build():
+    """Select librbg_checked.so (device-side index / layout / ring-slot checks, rbg_selfcheck_failures) for this process.
+    Must be called before the first load_library()."""
+    global _LIB_PATH
+    if _lib is not None:
+        raise RbgError("the library is already loaded")
+    _LIB_PATH = _PKG / "librbg_checked.so"
 
 
 def load_library():
@@ -110,6 +120,13 @@ def probe_alu_peak(what: int, iters: int = 1 << 16, stream=None) -> float:
     out = C.c_double()
     _check(load_library().rbg_probe_alu_peak(what, iters, C.byref(out), _stream_ptr(stream)))
     return out.value
+
+
+def selfcheck_failures():
+    """rbg_selfcheck_failures: the eight failure counters of the checked build (raises in the normal build)."""
+    out = (C.c_uint64 * 8)()
+    _check(load_library().rbg_selfcheck_failures(out))
+    return [int(v) for v in out]
 
 
 def selftest_math(n_operands: int, seed: int = 1) -> int:

@@ -30,22 +30,26 @@ def _digest() -> str:
     return h.hexdigest()
 
 
-def build(force: bool = False, verbose: bool = False) -> Path:
-    tag = PKG / ".librbg.tag"
+def build(force: bool = False, verbose: bool = False, checked: bool = False) -> Path:
+    """checked = True builds librbg_checked.so with -DRBG_CHECKED (device-side index / layout / ring-slot checks, include/rbg.h
+    rbg_selfcheck_failures) next to the normal library."""
+    lib = PKG / "librbg_checked.so" if checked else LIB
+    tag = PKG / (".librbg_checked.tag" if checked else ".librbg.tag")
     dig = _digest()
-    if not force and LIB.exists() and tag.exists() and tag.read_text() == dig:
-        return LIB
-    cmd = ["nvcc", *NVCC_FLAGS, "-o", str(LIB), *map(str, SOURCES)]
+    if not force and lib.exists() and tag.exists() and tag.read_text() == dig:
+        return lib
+    cmd = ["nvcc", *NVCC_FLAGS, *(["-DRBG_CHECKED"] if checked else []), "-o", str(lib), *map(str, SOURCES)]
     res = subprocess.run(cmd, capture_output=True, text=True)
-    (PKG / "ptxas.log").write_text(res.stderr)
+    if not checked:
+        (PKG / "ptxas.log").write_text(res.stderr)
     if res.returncode != 0:
         sys.stderr.write(res.stderr)
         raise RuntimeError("nvcc failed building librbg.so")
     if verbose:
         sys.stderr.write(res.stderr)
     tag.write_text(dig)
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose=True))
+    print(build(force="--force" in sys.argv, verbose=True, checked="--checked" in sys.argv))

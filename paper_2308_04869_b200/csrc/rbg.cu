@@ -166,13 +166,13 @@ cudaError_t launch_one(const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp
     return cudaGetLastError();
 }
 
-// Launch geometries: CTAs of up to 8 warps evaluate SPL = 4 samples per lane and loop iteration (up to 255 registers per
-// thread), up to 16 warps SPL = 2 (128 registers), up to 32 warps SPL = 1 (64 registers; elastic roles only).  All three
-// keep the whole register file of an SM busy with one CTA; results are bit-identical (fixed lane summation order).
+// Launch geometries: CTAs of up to 16 warps evaluate SPL = 2 samples per lane and loop iteration (128 registers per
+// thread), up to 32 warps SPL = 1 (64 registers; elastic roles only).  Both keep the whole register file of an SM busy
+// with one CTA; results are bit-identical (fixed lane summation order).  Measured (profiles/r2_collision.md): 4 samples
+// per lane at 8 warps and 255 registers is 2-5 % slower than SPL = 2 once the azimuth comes from shared memory.
 template <typename R, int KIND, bool Q, bool SMEM, bool TCH, bool INEL>
 cudaError_t launch_geo(int spl, const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp, int grid, int threads,
                        size_t smem, const LaunchCtx& st) {
-    if (spl == 4) return launch_one<R, KIND, Q, SMEM, 256, 4, TCH, INEL>(rp, lp, grid, threads, smem, st);
     if constexpr (!INEL)
         if (spl == 1) return launch_one<R, KIND, Q, SMEM, 1024, 1, TCH, INEL>(rp, lp, grid, threads, smem, st);
     return launch_one<R, KIND, Q, SMEM, 512, 2, TCH, INEL>(rp, lp, grid, threads, smem, st);
@@ -220,18 +220,13 @@ int run_roles(rbg_handle* h, const double* f, double* out, bool update, double d
         const Role& r = h->roles[ir];
         const rbg::RoleParams<R> rp = make_role_params<R>(*h, r);
         const bool inel = !r.elastic;
-        // samples per lane: the option, else the default of the arithmetic type; CTAs wider than its geometry allows
-        // fall to the next one (8 / 16 / 32 warps for 4 / 2 / 1 samples per lane; general roles: at most 16 warps)
-        // default (measured, profiles/r2_collision.md): 4 for fp64 roles with large momentum grids staged in shared memory,
-        // 2 otherwise
+        // samples per lane: 2 (at most 16 warps) unless the option or a wider CTA asks for 1 (elastic roles only)
         const int np1 = rp.np[0];
-        int spl = h->opt_spl > 0 ? h->opt_spl
-                  : (sizeof(R) == 8 && np1 >= 4096 && r.kind < RBG_M2_QCD_Q1Q2 ? 4 : 2);
+        int spl = h->opt_spl > 0 ? h->opt_spl : 2;
         int warps = h->opt_warps > 0 ? h->opt_warps : 32 / spl;
         if (inel && warps > 16) warps = 16;
         if (warps > 16) spl = 1;
-        else if (warps > 8 && spl == 4) spl = 2;
-        if (inel && spl == 1) spl = 2;
+        if (inel) spl = 2;
         // Tile size T (momentum cells per CTA; one CTA per SM at a time): a CTA stages its tables (about 2 us + bytes at
         // 100 GB/s) and then takes ceil(T / warps) rounds of one p1 per warp (a round of n_samples samples per warp at
         // about 5.7e8 samples/s per SM); the grid of nx * tiles CTAs runs in ceil(nx * tiles / SMs) waves.  Take the
@@ -631,8 +626,16 @@ int rbg_set_option(rbg_handle* h, const char* key, int value) {
     if (!h || !key) return fail(h, RBG_E_INVALID_ARG, "null argument");
     const std::string k(key);
     if (k == "warps_per_cta") { if (value < 0 || value > 32) return fail(h, RBG_E_INVALID_ARG, "warps_per_cta must be 0 (auto) or 1..32"); h->opt_warps = value; }
-    else if (k == "samples_per_lane") { if (value != 0 && value != 1 && value != 2 && value != 4) return fail(h, RBG_E_INVALID_ARG, "samples_per_lane must be 0 (auto), 1, 2 or 4"); h->opt_spl = value; }
+    else if (k == "samples_per_lane") { if (value < 0 || value > 2) return fail(h, RBG_E_INVALID_ARG, "samples_per_lane must be 0 (auto), 1 or 2"); h->opt_spl = value; }
     else if (k == "p1_per_cta") { if (value < 0) return fail(h, RBG_E_INVALID_ARG, "p1_per_cta must be >= 0 (0 = auto)"); h->opt_p1_per_cta = value; }
+#ifdef RBG_CHECKED
+    else if (k == "selfcheck_probe") {             // checked build only: `value` threads fail one check of every class
+        if (value < 0 || value > 1024) return fail(h, RBG_E_INVALID_ARG, "selfcheck_probe must be 0..1024");
+        DeviceGuard guard(h->device);
+        rbg::selfcheck_probe_kernel<<<1, 1024>>>(value);
+        RBG_CUDA(h, cudaDeviceSynchronize());
+    }
+#endif
     else if (k == "gather") { if (value < 0 || value > 2) return fail(h, RBG_E_INVALID_ARG, "gather must be 0, 1 or 2"); h->opt_gather = value; }
     else return fail(h, RBG_E_INVALID_ARG, "unknown option " + k);
     return RBG_OK;
@@ -910,6 +913,20 @@ int rbg_be_step(rbg_handle* h, double* f_dev, double* scratch_dev, const rbg_be_
     if (cur != f_dev) RBG_CUDA(h, cudaMemcpyAsync(f_dev, cur, bytes, cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
     h->last_launches = launches;
     return RBG_OK;
+}
+
+int rbg_selfcheck_failures(uint64_t* counts) {
+    if (!counts) return fail(nullptr, RBG_E_INVALID_ARG, "null argument");
+#ifdef RBG_CHECKED
+    unsigned long long h[rbg::CHK_CLASSES];
+    RBG_CUDA(nullptr, cudaDeviceSynchronize());
+    RBG_CUDA(nullptr, cudaMemcpyFromSymbol(h, rbg::g_check_failures, sizeof h));
+    for (int i = 0; i < rbg::CHK_CLASSES; ++i) counts[i] = h[i];
+    return RBG_OK;
+#else
+    for (int i = 0; i < rbg::CHK_CLASSES; ++i) counts[i] = 0;
+    return fail(nullptr, RBG_E_UNSUPPORTED, "not a checked build (python -m paper_2308_04869_b200.build --checked)");
+#endif
 }
 
 int rbg_selftest_math(uint64_t n_operands, uint32_t seed, uint64_t* mismatches) {

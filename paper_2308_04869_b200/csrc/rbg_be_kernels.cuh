@@ -13,6 +13,20 @@
 
 namespace rbg {
 
+// Checked build: a warp that consumes a ring slot verifies, before its first and after its last read, that the slot still
+// holds the unit it believes it is consuming (first and last value against global memory, bit for bit): a refill that
+// overtakes a reader, or a wait on the wrong mbarrier phase, changes them.
+#ifdef RBG_CHECKED
+#define RBG_CHECK_STAGE(fs, src, n)                                                                                        \
+    do {                                                                                                                     \
+        if ((threadIdx.x & 31) == 0)                                                                                         \
+            RBG_CHECK(__double_as_longlong((fs)[0]) == __double_as_longlong(__ldg(src)) &&                                   \
+                      __double_as_longlong((fs)[(n) - 1]) == __double_as_longlong(__ldg((src) + (n) - 1)), CHK_STAGE_CONTENT); \
+    } while (0)
+#else
+#define RBG_CHECK_STAGE(fs, src, n) ((void)0)
+#endif
+
 enum { N_MOMENTS = 14 };   // n, jx, jy, jz, T00, T01, T02, T03, T11, T12, T13, T22, T23, T33
 
 struct SpeciesTables {
@@ -130,6 +144,8 @@ moments_kernel(const double* __restrict__ f_species, SpeciesTables tb, int nx_ce
             for (size_t j = threadIdx.x; j < (size_t)cells * np; j += MOM_THREADS) fs[j] = __ldcs(src + j);
             __syncthreads();
         }
+        RBG_CHECK_STAGE(fs, f_species + (size_t)first * np, (size_t)cells * np);
+        RBG_CHECK(first + cells <= nx_cells && (size_t)(slot + 1) * stage_bytes + head + tab_bytes <= dynamic_smem_size(), CHK_BE_INDEX);
         for (int cell0 = 0; cell0 < cells; cell0 += n_teams) {           // one round: every team reduces one cell
             const int cell = cell0 + my_team;
             const bool active = cell < cells;
@@ -229,6 +245,7 @@ moments_kernel(const double* __restrict__ f_species, SpeciesTables tb, int nx_ce
                 flip ^= 1;                                     // the next round writes the other buffer: one barrier per round
             }
         }
+        RBG_CHECK_STAGE(fs, f_species + (size_t)first * np, (size_t)cells * np);
         if (ONE_TEAM) {
             // the warp that finishes last with this stage refills it (its reads of the stage and of the reduction
             // buffers are complete: their values were consumed above)
@@ -345,6 +362,13 @@ drift_upfd_kernel(const double* __restrict__ f_species, double* __restrict__ out
             const double* __restrict__ row = f_species + (row0 + z) * np;
             ptrdiff_t offz;
             upwind(2, z, offz, csz[k]);
+#ifdef RBG_CHECKED
+            {   // every address of the stencil lies inside the species block
+                const ptrdiff_t total = (ptrdiff_t)dp.nxyz[0] * dp.nxyz[1] * dp.nxyz[2] * np, base = (ptrdiff_t)(row0 + z) * np;
+                RBG_CHECK(base + ip >= 0 && base + ip < total && base + offx >= 0 && base + offx < total && base + offy >= 0 &&
+                          base + offy < total && base + offz >= 0 && base + offz < total, CHK_BE_INDEX);
+            }
+#endif
             self[k] = __ldg(row + ip);
             ux[k] = __ldg(row + offx);
             uy[k] = __ldg(row + offy);
@@ -502,6 +526,8 @@ vlasov_upfd_kernel(const double* __restrict__ f_species, double* __restrict__ ou
             for (size_t j = threadIdx.x; j < (size_t)cells * np; j += MOM_THREADS) fs[j] = __ldcs(src + j);
             __syncthreads();
         }
+        RBG_CHECK_STAGE(fs, f_species + (size_t)first * np, (size_t)cells * np);
+        RBG_CHECK(first + cells <= vp.nx_cells, CHK_BE_INDEX);
         for (int cell = my_team; cell < cells; cell += n_teams) {
             const double* __restrict__ fc = fs + (size_t)cell * np;
             double* __restrict__ oc = out_species + ((size_t)first + cell) * np;
@@ -543,6 +569,7 @@ vlasov_upfd_kernel(const double* __restrict__ f_species, double* __restrict__ ou
                 }
             }
         }
+        RBG_CHECK_STAGE(fs, f_species + (size_t)first * np, (size_t)cells * np);
         // no CTA barrier: a warp that is done moves on to the next stage; the last warp to finish with this one (its
         // shared-memory reads have completed: their values were consumed by the stores above) refills it
         __syncwarp();

@@ -5,6 +5,11 @@
     compute-sanitizer --tool synccheck python tests/sanitizer_cases.py
     compute-sanitizer --tool initcheck python tests/sanitizer_cases.py
 
+and, where compute-sanitizer is not available (it is closed on the pool this repo is developed on, profiles/r2_sanitizers.md),
+with the library's own device-side checks:
+
+    python tests/sanitizer_cases.py --checked      # librbg_checked.so; prints the eight failure counters, all must be 0
+
 Not a pytest module (correctness against the oracle is tests/test_gpu_*.py); it only drives the CUDA path through the C ABI
 so that the tool sees every staging / synchronisation pattern: TMA bulk copy + mbarrier, cooperative staging, global (L2)
 gathers, the fused update, shared-memory and global atomics of the conservative estimator with its CTA-end flush, the
@@ -99,8 +104,21 @@ def be_step_cases():
 
 
 if __name__ == "__main__":
+    checked = "--checked" in sys.argv
+    if checked:
+        from paper_2308_04869_b200.build import build
+        build(checked=True)
+        rbg.use_checked_build()
     torch.cuda.set_device(0)
     collision_cases()
     symmetric_cases()
     be_step_cases()
     print("all sanitizer cases ran")
+    if checked:
+        counts = rbg.selfcheck_failures()
+        names = ("f-table index", "tile index", "direction-table index", "output index", "shared-memory layout",
+                 "ring-slot contents", "stencil / moment index", "conservative-estimator index")
+        for n, c in zip(names, counts):
+            print(f"checked build: {n}: {c} failures")
+        assert not any(counts), counts
+        print("CHECKED BUILD SUMMARY: 0 failures")

@@ -9,3 +9,30 @@ def test_custom_fp64_ops_are_correctly_rounded():
     import paper_2308_04869_b200 as rbg
     for seed in (1, 2, 3):
         assert rbg.selftest_math(200_000_000, seed) == 0
+
+
+def test_checked_build_finds_no_bad_index_layout_or_ring_slot():
+    """compute-sanitizer is closed on the development pool (profiles/r2_sanitizers.md); the library's checked build verifies
+    every table index, the shared-memory layout and the ring-slot contents on the device while tests/sanitizer_cases.py drives
+    every kernel family.  Runs in a subprocess: the checked library must be the one loaded."""
+    import subprocess
+    import sys
+    from pathlib import Path
+    root = Path(__file__).resolve().parent.parent
+    res = subprocess.run([sys.executable, str(root / "tests" / "sanitizer_cases.py"), "--checked"], capture_output=True, text=True,
+                         timeout=1500)
+    assert res.returncode == 0, res.stdout[-3000:] + res.stderr[-3000:]
+    assert "CHECKED BUILD SUMMARY: 0 failures" in res.stdout
+    assert res.stdout.count("\nok  ") + res.stdout.startswith("ok  ") >= 35
+    # the counters do count: the probe fails one check of every class for each of 5 threads
+    code = ("import sys; sys.path.insert(0, %r); import paper_2308_04869_b200 as rbg, workloads; rbg.use_checked_build(); "
+            "col = rbg.Collision(workloads.make(1, np_side=4)['problem']); col.set_option('selfcheck_probe', 5); "
+            "print(rbg.selfcheck_failures())" % str(root))
+    res = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=600)
+    assert res.returncode == 0 and res.stdout.strip().endswith("[5, 5, 5, 5, 5, 5, 5, 5]"), res.stdout + res.stderr
+
+
+def test_normal_build_has_no_checks_compiled_in():
+    import paper_2308_04869_b200 as rbg
+    with pytest.raises(rbg.RbgError, match="not a checked build"):
+        rbg.selfcheck_failures()
