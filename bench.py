@@ -451,13 +451,16 @@ def roofline_of(rbg, torch, res, args, local, probe_cache):
     if what not in probe_cache:
         probe_cache[what] = rbg.probe_alu_peak(what, 1 << 17) * 2 / 1e12
     probe = probe_cache[what]
+    if "ctx" not in probe_cache:        # operand-pattern context (profiles/r2_collision.md): instructions/s per SM sub-partition-cycle
+        probe_cache["ctx"] = {"dfma_3_distinct_operands_tflops": rbg.probe_alu_peak(3, 1 << 16) * 2 / 1e12,
+                              "widemul_u32_gops": rbg.probe_alu_peak(4, 1 << 16) / 1e9}
     sym = args.estimator == "symmetric"
     traffic = NCU_TRAFFIC_BYTES_PER_LAUNCH.get(w["cfg"]) if (args.nx is None and not args.sampler and not sym and not args.opt) else None
     return {"bound": "alu", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s", "frac": achieved / peak_nominal,
             "traffic": traffic[0] if traffic else None,
             "traffic_unit": f"bytes per launch (dram read + write, {traffic[1]})" if traffic else None,
             "peak_source": f"{sms} SM x {lanes} FMA/clk x 2 x {max_mhz:.0f} MHz ({'FP32' if w['fp32'] else 'FP64'} FMA pipe; DESIGN.md section 8)",
-            "peak_probe_tflops": probe, "frac_of_probe": achieved / probe,
+            "peak_probe_tflops": probe, "frac_of_probe": achieved / probe, "probe_context": probe_cache["ctx"],
             "kernel": "rbg::collision_symmetric_kernel" if sym else "rbg::collision_role_kernel", "launch_ms": t_launch * 1e3,
             "flops_per_sample": res["fl_rank"] / res["n_evals_rank"]}
 

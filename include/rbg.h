@@ -233,8 +233,10 @@ const char* rbg_last_error(const rbg_handle* h);
 void rbg_destroy(rbg_handle* h);
 
 /* Measurement helper: runs a register-resident chain of independent FMAs on every SM and reports
- * the achieved rate.  what: 0 = fp64 FMA, 1 = fp32 FMA, 2 = int32 multiply-add.  *ops_per_s counts
- * one FMA as one operation.  Used by bench.py for the live roofline denominator. */
+ * the achieved rate.  what: 0 = fp64 FMA, 1 = fp32 FMA, 2 = int32 multiply-add (each re-using two of its three
+ * operands), 3 = fp64 FMA naming three distinct register pairs per instruction (register-file read bandwidth, not
+ * the FP64 lanes, limits it), 4 = the 32 x 32 -> 64-bit multiply of a Philox round.  *ops_per_s counts one FMA /
+ * multiply as one operation.  Used by bench.py for the live roofline denominator and its context. */
 int rbg_probe_alu_peak(int what, int iters, double* ops_per_s, void* cuda_stream);
 
 /* Diagnostic of the CHECKED build (librbg_checked.so, `python -m paper_2308_04869_b200.build --checked`, -DRBG_CHECKED): the

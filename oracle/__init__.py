@@ -30,18 +30,26 @@ def _cpu_has_fma() -> bool:
 
 
 def build(force: bool = False) -> Path:
-    """Compile the oracle with g++ (no CUDA).  -ffp-contract=off: every rounding is explicit."""
-    tag = _HERE / ".build_tag"
+    """Compile the oracle with g++ (no CUDA).  -ffp-contract=off: every rounding is explicit.
+
+    RBG_ORACLE_SANITIZE=1 in the environment builds and loads librbg_oracle_san.so instead, compiled with
+    -fsanitize=address,undefined (run the CPU pins under it with LD_PRELOAD=$(gcc -print-file-name=libasan.so);
+    profiles/r2_sanitizers.md has the command and its result)."""
+    san = os.environ.get("RBG_ORACLE_SANITIZE", "") not in ("", "0")
+    lib_path = _HERE / "librbg_oracle_san.so" if san else _LIB
+    tag = _HERE / (".build_tag_san" if san else ".build_tag")
     want = f"fma={int(_cpu_has_fma())} mtime={_SRC.stat().st_mtime_ns}"
-    if not force and _LIB.exists() and tag.exists() and tag.read_text() == want:
-        return _LIB
+    if not force and lib_path.exists() and tag.exists() and tag.read_text() == want:
+        return lib_path
     cmd = ["g++", "-O2", "-std=c++17", "-fopenmp", "-ffp-contract=off", "-fPIC", "-shared",
-           "-o", str(_LIB), str(_SRC)]
+           "-o", str(lib_path), str(_SRC)]
+    if san:
+        cmd[1:1] = ["-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"]
     if _cpu_has_fma():
         cmd.insert(1, "-mfma")          # std::fma -> one vfmadd instruction instead of a libm call
     subprocess.run(cmd, check=True)
     tag.write_text(want)
-    return _LIB
+    return lib_path
 
 
 class _Species(C.Structure):

@@ -116,7 +116,8 @@ def _check(rc, handle=None):
 
 
 def probe_alu_peak(what: int, iters: int = 1 << 16, stream=None) -> float:
-    """FMA/s (one FMA = one op) of a register-resident chain: 0 fp64, 1 fp32, 2 int32."""
+    """Operations/s (one FMA or multiply = one op) of a register-resident chain: 0 fp64, 1 fp32, 2 int32 (two of three
+    operands re-used), 3 fp64 with three distinct register operands per FMA, 4 the 32 x 32 -> 64-bit multiply of Philox."""
     out = C.c_double()
     _check(load_library().rbg_probe_alu_peak(what, iters, C.byref(out), _stream_ptr(stream)))
     return out.value

@@ -947,7 +947,7 @@ int rbg_selftest_math(uint64_t n_operands, uint32_t seed, uint64_t* mismatches) 
 }
 
 int rbg_probe_alu_peak(int what, int iters, double* ops_per_s, void* cuda_stream) {
-    if (!ops_per_s || iters <= 0 || what < 0 || what > 2) return fail(nullptr, RBG_E_INVALID_ARG, "bad probe arguments");
+    if (!ops_per_s || iters <= 0 || what < 0 || what > 4) return fail(nullptr, RBG_E_INVALID_ARG, "bad probe arguments");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int dev = 0, sms = 0;
     RBG_CUDA(nullptr, cudaGetDevice(&dev));
@@ -962,7 +962,9 @@ int rbg_probe_alu_peak(int what, int iters, double* ops_per_s, void* cuda_stream
         cudaEventRecord(e0, st);
         if (what == 0) rbg::alu_probe_kernel<double><<<ctas, threads, 0, st>>>((double*)buf, 1.0000001, 1e-9, iters);
         else if (what == 1) rbg::alu_probe_kernel<float><<<ctas, threads, 0, st>>>((float*)buf, 1.0000001f, 1e-9f, iters);
-        else rbg::alu_probe_kernel<unsigned><<<ctas, threads, 0, st>>>((unsigned*)buf, 2654435761u, 12345u, iters);
+        else if (what == 2) rbg::alu_probe_kernel<unsigned><<<ctas, threads, 0, st>>>((unsigned*)buf, 2654435761u, 12345u, iters);
+        else if (what == 3) rbg::dfma3_probe_kernel<<<ctas, threads, 0, st>>>((double*)buf, iters);
+        else rbg::widemul_probe_kernel<<<ctas, threads, 0, st>>>((unsigned*)buf, iters);
         cudaEventRecord(e1, st);
         cudaError_t e = cudaEventSynchronize(e1);
         if (e != cudaSuccess) { cudaFree(buf); return fail(nullptr, RBG_E_CUDA, cudaGetErrorString(e)); }
