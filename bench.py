@@ -48,20 +48,25 @@ FLOPS_PER_SAMPLE = {0: 141.0, 1: 155.0, 2: 157.0, 3: 142.0,
                     # rational function (5 / 14 / 14 / 5 / 12 / 12 / 16; a reciprocal = 1)
                     4: 164.0, 5: 173.0, 6: 173.0, 7: 164.0, 8: 171.0, 9: 171.0, 10: 175.0}
 QUANTUM_EXTRA_FLOPS = 10.0
+# Chain v3 (double chain only, O6): the azimuth is two tabulated angles and the addition theorem
+# (2 multiplies + 2 FMAs = 6 flops) instead of two polynomial evaluations (29 flops): 23 flops fewer per sample.  The count
+# is that of the tabulated form -- what an implementation has to compute -- not of the oracle's per-sample polynomials.
+DOUBLE_CHAIN_V3_SAVING = 23.0
 # the same count for the t-channel importance sampler (steps S1-S7), kinds 1 and 2
 FLOPS_PER_SAMPLE_TCHANNEL = {1: 185.0, 2: 187.0}
 FP64_LANES_PER_SM = 64          # FMA/clk/SM; confirmed by the live probe
 # dram__bytes_read.sum + dram__bytes_write.sum of one role launch at full size, from the committed `ncu --set full`
 # captures (file named beside each); null for workloads without a capture.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {2: (35.02e6, "profiles/r1c_chain_v2_cfg2.md")}
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {2: (32.93e6 + 2.78e6, "profiles/r2_collision.md, capture C"),
+                                4: (2184746496.0 + 2083488256.0, "profiles/r2_collision.md, capture D")}
 
 
-def flops_per_sweep(problem, n_samples):
+def flops_per_sweep(problem, n_samples, fp32=False):
     tot = 0.0
     for r, p in zip(wl.roles(problem), wl.role_processes(problem)):
         q = any(problem["species"][s]["stat"] != 0 for s in r)
         table = FLOPS_PER_SAMPLE_TCHANNEL if p.get("sampler", 0) == 1 else FLOPS_PER_SAMPLE
-        per = table[p["kind"]] + (QUANTUM_EXTRA_FLOPS if q else 0.0)
+        per = table[p["kind"]] + (QUANTUM_EXTRA_FLOPS if q else 0.0) - (0.0 if fp32 else DOUBLE_CHAIN_V3_SAVING)
         tot += per * problem["nx"] * int(np.prod(problem["grids"][r[0]]["n"])) * n_samples
     return tot
 
@@ -402,7 +407,7 @@ def time_config(rbg, torch, cfg, args, steps, warmup, rank, world, local, e2e=Tr
         dist.all_reduce(t, op=dist.ReduceOp.SUM)
         total_evals = int(t.item())
     res = {"w": w, "t_step": t_step, "n_evals_total": total_evals, "n_evals_rank": n_evals, "launches_per_step": launches_per_step,
-           "clocks": clocks, "times_ms": times_ms, "fl_rank": flops_per_sweep(prob, w["n_samples"])}
+           "clocks": clocks, "times_ms": times_ms, "fl_rank": flops_per_sweep(prob, w["n_samples"], w["fp32"])}
 
     if e2e:
         # the same sweep through the C ABI with HOST buffers (pinned): copies inside the timed region
@@ -461,6 +466,9 @@ def roofline_of(rbg, torch, res, args, local, probe_cache):
             "traffic_unit": f"bytes per launch (dram read + write, {traffic[1]})" if traffic else None,
             "peak_source": f"{sms} SM x {lanes} FMA/clk x 2 x {max_mhz:.0f} MHz ({'FP32' if w['fp32'] else 'FP64'} FMA pipe; DESIGN.md section 8)",
             "peak_probe_tflops": probe, "frac_of_probe": achieved / probe, "probe_context": probe_cache["ctx"],
+            # FP64 chain: a DFMA whose three operands are distinct registers is limited by register-file operand bandwidth
+            # to 2/3 of the lane peak; the fraction of THAT rate is context, `frac` stays the headline
+            "frac_of_3_operand_dfma_rate": None if w["fp32"] else achieved / probe_cache["ctx"]["dfma_3_distinct_operands_tflops"],
             "kernel": "rbg::collision_symmetric_kernel" if sym else "rbg::collision_role_kernel", "launch_ms": t_launch * 1e3,
             "flops_per_sample": res["fl_rank"] / res["n_evals_rank"]}
 

@@ -161,8 +161,11 @@ int rbg_collision_symmetric(rbg_handle* h, const double* f_dev, double* C_dev, i
                             void* cuda_stream);
 
 /* Same as rbg_collision with HOST buffers: copies f_host to the device (handle-owned scratch),
- * runs the kernels, copies C back, synchronises.  Pinned host memory makes the copies faster but
- * is not required. */
+ * runs the kernels, copies C back, synchronises.  Spatial cells are independent, so large problems are pipelined over
+ * up to 16 chunks of cells on three handle-owned streams (copy-in of chunk k+1 and copy-out of chunk k-1 beside the
+ * kernels of chunk k); the result is bit-identical to rbg_collision (the sample stream is keyed by the global cell).
+ * Pinned host memory lets the copies overlap the kernels; pageable memory works but serialises them.  f_host and
+ * C_host must not overlap. */
 int rbg_collision_host(rbg_handle* h, const double* f_host, double* C_host, int n_samples, uint64_t seed);
 
 /* ---- The steps either side of the collision term ---------------------------------

@@ -61,6 +61,9 @@ struct rbg_handle {
     // scratch for the host entry point
     double *scratch_f = nullptr, *scratch_c = nullptr;
     size_t scratch_elems = 0;
+    enum { HOST_CHUNKS_MAX = 16 };
+    cudaStream_t host_streams[3] = {nullptr, nullptr, nullptr};      // copy-in, kernels, copy-out of rbg_collision_host
+    cudaEvent_t host_events[2 * HOST_CHUNKS_MAX] = {};
     mutable std::string err;
 };
 
@@ -196,9 +199,12 @@ cudaError_t launch_kq(bool q, bool smem_path, bool inel, int spl, const rbg::Rol
 
 template <typename R>
 int run_roles(rbg_handle* h, const double* f, double* out, bool update, double dt, int* neg_flag, int n_samples,
-              uint64_t seed, cudaStream_t stream) {
+              uint64_t seed, cudaStream_t stream, int cell_begin = 0, int cell_count = -1) {
+    // [cell_begin, cell_begin + cell_count) = the local spatial cells this call sweeps (default: all of them); the stream
+    // key is the global cell index, so sweeping the cells in several calls gives the same result as one call
     const LaunchCtx st{h->device, h->max_smem_optin, stream};
-    h->last_launches = 0;
+    const int ncell = cell_count < 0 ? h->nx : cell_count;
+    if (cell_begin == 0) h->last_launches = 0;
     // last role per species (update mode counts negatives there); species with no role: C = 0 / f_out = f
     std::vector<int> first_role(h->n_species, -1), last_role(h->n_species, -1);
     for (size_t i = 0; i < h->roles.size(); ++i) {
@@ -207,13 +213,13 @@ int run_roles(rbg_handle* h, const double* f, double* out, bool update, double d
     }
     for (int s = 0; s < h->n_species; ++s) {
         if (first_role[s] >= 0) continue;
-        const size_t n = (size_t)h->nx * h->np[s];
+        const size_t n = (size_t)ncell * h->np[s], o = h->sp_off[s] + (size_t)cell_begin * h->np[s];
         if (update) {
-            rbg::copy_count_kernel<<<h->sm_count * 4, 256, 0, stream>>>(f + h->sp_off[s], out + h->sp_off[s], n, neg_flag);
+            rbg::copy_count_kernel<<<h->sm_count * 4, 256, 0, stream>>>(f + o, out + o, n, neg_flag);
             RBG_CUDA(h, cudaGetLastError());
             ++h->last_launches;
         } else {
-            RBG_CUDA(h, cudaMemsetAsync(out + h->sp_off[s], 0, n * sizeof(double), stream));
+            RBG_CUDA(h, cudaMemsetAsync(out + o, 0, n * sizeof(double), stream));
         }
     }
     for (size_t ir = 0; ir < h->roles.size(); ++ir) {
@@ -244,7 +250,7 @@ int run_roles(rbg_handle* h, const double* f, double* out, bool update, double d
             const int t_lo = (np1 + 511) / 512, t_hi = std::max(t_lo, std::min(4096, (np1 + warps - 1) / warps));
             for (int tiles = t_lo; tiles <= t_hi; ++tiles) {
                 const int Tt = (np1 + tiles - 1) / tiles;
-                const long ctas = (long)h->nx * ((np1 + Tt - 1) / Tt);
+                const long ctas = (long)ncell * ((np1 + Tt - 1) / Tt);
                 const double cost = (double)((ctas + h->sm_count - 1) / h->sm_count) * ((double)((Tt + warps - 1) / warps) + staging);
                 if (best_cost < 0.0 || cost < 0.995 * best_cost) { best_cost = cost; T = Tt; }
             }
@@ -269,9 +275,9 @@ int run_roles(rbg_handle* h, const double* f, double* out, bool update, double d
         if (h->opt_gather == 1 && !smem_path) return fail(h, RBG_E_UNSUPPORTED, "gather=1 (shared memory) requested but the f tables do not fit");
         if (h->opt_gather == 2) smem_path = false;
         const size_t smem = head + (smem_path ? tabs : 0);
-        for (int i = 0; i < 4; ++i) lp.fb[i] = f + h->sp_off[r.s[i]];
-        lp.out_base = out + h->sp_off[r.s[0]];
-        lp.nx_local = h->nx; lp.ix_offset = h->ix_offset; lp.n_samples = n_samples;
+        for (int i = 0; i < 4; ++i) lp.fb[i] = f + h->sp_off[r.s[i]] + (size_t)cell_begin * h->np[r.s[i]];
+        lp.out_base = out + h->sp_off[r.s[0]] + (size_t)cell_begin * h->np[r.s[0]];
+        lp.nx_local = ncell; lp.ix_offset = h->ix_offset + cell_begin; lp.n_samples = n_samples;
         lp.dir_tab = h->dir_tab;
         lp.key0 = (uint32_t)seed; lp.key1 = (uint32_t)(seed >> 32);
         for (int rr = 0; rr < 10; ++rr) {
@@ -282,7 +288,7 @@ int run_roles(rbg_handle* h, const double* f, double* out, bool update, double d
         lp.accumulate = first_role[r.s[0]] != (int)ir;
         lp.update = update; lp.dt = dt; lp.neg_flag = neg_flag;
         lp.count_negative = update && last_role[r.s[0]] == (int)ir;
-        const long grid = (long)lp.tiles * h->nx;
+        const long grid = (long)lp.tiles * ncell;
         if (grid > 0x7fffffffL) return fail(h, RBG_E_UNSUPPORTED, "grid too large; raise p1_per_cta");
         bool q = false;
         for (int i = 0; i < 4; ++i) q = q || h->species[r.s[i]].stat != 0;
@@ -597,6 +603,7 @@ int rbg_collision_evolve(rbg_handle* h, double* f_dev, double* scratch_dev, doub
 int rbg_collision_host(rbg_handle* h, const double* f_host, double* C_host, int n_samples, uint64_t seed) {
     if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
     if (!f_host || !C_host) return fail(h, RBG_E_INVALID_ARG, "null buffer");
+    if (n_samples <= 0) return fail(h, RBG_E_INVALID_ARG, "n_samples must be positive");
     DeviceGuard guard(h->device);
     if (h->scratch_elems < h->f_elems) {
         cudaFree(h->scratch_f); cudaFree(h->scratch_c); h->scratch_f = h->scratch_c = nullptr; h->scratch_elems = 0;
@@ -604,11 +611,39 @@ int rbg_collision_host(rbg_handle* h, const double* f_host, double* C_host, int 
         RBG_CUDA(h, cudaMalloc(&h->scratch_c, h->f_elems * sizeof(double)));
         h->scratch_elems = h->f_elems;
     }
-    RBG_CUDA(h, cudaMemcpyAsync(h->scratch_f, f_host, h->f_elems * sizeof(double), cudaMemcpyHostToDevice, 0));
-    int rc = run(h, h->scratch_f, h->scratch_c, false, 0.0, nullptr, n_samples, seed, nullptr);
-    if (rc != RBG_OK) return rc;
-    RBG_CUDA(h, cudaMemcpyAsync(C_host, h->scratch_c, h->f_elems * sizeof(double), cudaMemcpyDeviceToHost, 0));
-    RBG_CUDA(h, cudaStreamSynchronize(0));
+    if (!h->host_streams[0]) {
+        for (int i = 0; i < 3; ++i) RBG_CUDA(h, cudaStreamCreateWithFlags(&h->host_streams[i], cudaStreamNonBlocking));
+        for (int i = 0; i < 2 * rbg_handle::HOST_CHUNKS_MAX; ++i) RBG_CUDA(h, cudaEventCreateWithFlags(&h->host_events[i], cudaEventDisableTiming));
+    }
+    // Spatial cells are independent (Eq. 16 couples only momenta at one x), so the sweep is pipelined over chunks of cells:
+    // copy-in of chunk k+1 and copy-out of chunk k-1 run beside the kernels of chunk k (three streams).  The chunk count
+    // keeps a chunk at 64 MB or more; small problems take one chunk.  Results do not depend on it (global-cell stream key).
+    const size_t bytes = h->f_elems * sizeof(double);
+    int chunks = (int)std::min<size_t>(rbg_handle::HOST_CHUNKS_MAX, std::max<size_t>(1, bytes / ((size_t)64 << 20)));
+    chunks = std::min(chunks, h->nx);
+    cudaStream_t s_in = h->host_streams[0], s_k = h->host_streams[1], s_out = h->host_streams[2];
+    const bool fp32 = (h->flags & RBG_FP32_KINEMATICS) != 0;
+    for (int c = 0; c < chunks; ++c) {
+        const int x0 = (int)((long)h->nx * c / chunks), x1 = (int)((long)h->nx * (c + 1) / chunks);
+        for (int s = 0; s < h->n_species; ++s) {
+            const size_t o = h->sp_off[s] + (size_t)x0 * h->np[s], n = (size_t)(x1 - x0) * h->np[s];
+            RBG_CUDA(h, cudaMemcpyAsync(h->scratch_f + o, f_host + o, n * sizeof(double), cudaMemcpyHostToDevice, s_in));
+        }
+        RBG_CUDA(h, cudaEventRecord(h->host_events[2 * c], s_in));
+        RBG_CUDA(h, cudaStreamWaitEvent(s_k, h->host_events[2 * c], 0));
+        const int rc = fp32 ? run_roles<float>(h, h->scratch_f, h->scratch_c, false, 0.0, nullptr, n_samples, seed, s_k, x0, x1 - x0)
+                            : run_roles<double>(h, h->scratch_f, h->scratch_c, false, 0.0, nullptr, n_samples, seed, s_k, x0, x1 - x0);
+        if (rc != RBG_OK) { cudaDeviceSynchronize(); return rc; }
+        RBG_CUDA(h, cudaEventRecord(h->host_events[2 * c + 1], s_k));
+        RBG_CUDA(h, cudaStreamWaitEvent(s_out, h->host_events[2 * c + 1], 0));
+        for (int s = 0; s < h->n_species; ++s) {
+            const size_t o = h->sp_off[s] + (size_t)x0 * h->np[s], n = (size_t)(x1 - x0) * h->np[s];
+            RBG_CUDA(h, cudaMemcpyAsync(C_host + o, h->scratch_c + o, n * sizeof(double), cudaMemcpyDeviceToHost, s_out));
+        }
+    }
+    RBG_CUDA(h, cudaStreamSynchronize(s_out));
+    RBG_CUDA(h, cudaStreamSynchronize(s_k));
+    RBG_CUDA(h, cudaStreamSynchronize(s_in));
     return RBG_OK;
 }
 
@@ -645,7 +680,10 @@ const char* rbg_last_error(const rbg_handle* h) { return h ? h->err.c_str() : g_
 
 void rbg_destroy(rbg_handle* h) {
     if (!h) return;
+    DeviceGuard guard(h->device);
     cudaFree(h->scratch_f); cudaFree(h->scratch_c);
+    for (cudaStream_t st : h->host_streams) if (st) cudaStreamDestroy(st);
+    for (cudaEvent_t ev : h->host_events) if (ev) cudaEventDestroy(ev);
     for (double* p : h->tab_iE) cudaFree(p);
     for (double* p : h->tab_v) cudaFree(p);
     cudaFree(h->charges_dev);

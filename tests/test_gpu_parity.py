@@ -191,6 +191,20 @@ def test_host_entry_point_matches_device_entry_point():
     assert np.array_equal(col.collision_host(pinned, w["n_samples"], w["seed"]).numpy(), C_dev)
 
 
+def test_host_entry_point_pipelined_over_cell_chunks_is_bit_identical():
+    """rbg_collision_host pipelines copy-in / kernels / copy-out over chunks of spatial cells once f exceeds 128 MB
+    (include/rbg.h); two species so that every chunk is two H2D copies, an odd cell count so that the chunks are unequal.
+    The sample stream is keyed by the global cell index, so the result must equal the one-launch device path bit for bit."""
+    w = workloads.make(2, nx=1201, np_side=20, n_samples=8)           # 2 x 1201 x 8000 doubles = 154 MB -> 2 chunks
+    assert w["f"].nbytes > (128 << 20)
+    C_dev, col = gpu_C(w["problem"], w["f"], w["n_samples"], w["seed"])
+    n_device_launches = col.last_launch_count()
+    pinned = torch.from_numpy(w["f"]).pin_memory()
+    C_host = col.collision_host(pinned, w["n_samples"], w["seed"]).numpy()
+    assert col.last_launch_count() == 2 * n_device_launches            # two chunks, every role in each
+    assert np.array_equal(C_host, C_dev)
+
+
 def test_edge_cases():
     rbg = _rbg()
     # single sample; fewer samples than lanes; one momentum cell; a species that takes part in no process
