@@ -52,7 +52,7 @@ struct rbg_handle {
     int sm_count = 148;
     int max_smem_optin = 0;
     // options
-    int opt_warps = 0, opt_p1_per_cta = 0, opt_gather = 0, opt_spl = 0;
+    int opt_warps = 0, opt_p1_per_cta = 0, opt_gather = 0, opt_spl = 0, opt_moments_path = 0;
     int last_launches = 0;
     // per-species device tables for the moment / drift / Vlasov kernels: 1/E_p and v = p/E_p per momentum cell
     std::vector<double*> tab_iE, tab_v;
@@ -671,6 +671,7 @@ int rbg_set_option(rbg_handle* h, const char* key, int value) {
         RBG_CUDA(h, cudaDeviceSynchronize());
     }
 #endif
+    else if (k == "moments_path") { if (value < 0 || value > 1) return fail(h, RBG_E_INVALID_ARG, "moments_path must be 0 (auto) or 1 (general staged kernel)"); h->opt_moments_path = value; }
     else if (k == "gather") { if (value < 0 || value > 2) return fail(h, RBG_E_INVALID_ARG, "gather must be 0, 1 or 2"); h->opt_gather = value; }
     else return fail(h, RBG_E_INVALID_ARG, "unknown option " + k);
     return RBG_OK;
@@ -750,6 +751,26 @@ int rbg_moments(rbg_handle* h, const double* f_dev, double* M_dev, double* total
         const int nyz = tb.n[1] * tb.n[2];
         // head: mbarriers, counters, MOM_RED reduction buffers, p_x table
         const size_t head = (128 + ((size_t)rbg::MOM_RED * (rbg::MOM_THREADS / 32) * 16 + (size_t)tb.n[0]) * 8 + 127) & ~(size_t)127;
+        // Momentum grid symmetric about 0 in every direction, at most 512 (p_y, p_z) columns, a cell of whole 16-byte units
+        // that fits three times next to the octant table: moments_sym_kernel (rbg_be_kernels.cuh)
+        {
+            bool sym = h->opt_moments_path != 1 && nyz <= rbg::MS_TEAM * rbg::MS_MAXC && (tb.np * 8) % 16 == 0 &&
+                       reinterpret_cast<uintptr_t>(fs) % 16 == 0;
+            for (int d = 0; d < 3; ++d) {
+                const rbg_momentum_grid& G = h->grids[s];
+                sym = sym && std::fabs(G.pmin[d] + G.pmax[d]) <= 1e-12 * (G.pmax[d] - G.pmin[d]);
+            }
+            const int c0 = tb.n[0] / 2, n0h = (tb.n[0] + 1) / 2, n1h = (tb.n[1] + 1) / 2, n2h = (tb.n[2] + 1) / 2;
+            const size_t head_sym = (128 + ((size_t)rbg::MS_STAGES * (rbg::MS_TEAM / 32) * 16 + 2 * (size_t)c0 + (size_t)n0h * n1h * n2h) * 8 + 127) & ~(size_t)127;
+            const size_t smem_sym = head_sym + (size_t)rbg::MS_STAGES * (((size_t)tb.np * 8 + 127) & ~(size_t)127);
+            if (sym && smem_sym <= (size_t)h->max_smem_optin) {
+                RBG_CUDA(h, ensure_max_smem(rbg::moments_sym_kernel, h->device, h->max_smem_optin));
+                rbg::moments_sym_kernel<<<std::max(1, std::min(h->sm_count, h->nx)), rbg::MS_THREADS, smem_sym, st>>>(fs, tb, h->nx, Ms);
+                RBG_CUDA(h, cudaGetLastError());
+                ++h->last_launches;
+                continue;
+            }
+        }
         // the 1/E table lives in shared memory when it fits next to two stages (measured: reading it through L1 and
         // spending its shared memory on a third stage is slower, 0.73 vs 0.58 ms on config 4: the kernel is bound by the
         // CTA's own instruction latency, the two-stage ring alone streams at 6.2 TB/s); otherwise it is read through L1

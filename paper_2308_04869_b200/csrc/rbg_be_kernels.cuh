@@ -265,6 +265,166 @@ moments_kernel(const double* __restrict__ f_species, SpeciesTables tb, int nx_ce
     (void)warp_in_team;
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Moments on a momentum grid that is symmetric about p = 0 in all three directions (every workload of the paper), one
+// spatial cell per stage.  Same sums as moments_kernel; what the symmetry buys:
+//   * 1/E_p depends on |p_x|, |p_y|, |p_z| only, so its table shrinks to one octant (8 KB instead of 64 KB at 20^3) and the
+//     ring gets a third stage;
+//   * the planes +p_x and -p_x of a column share 1/E: with s = a_+ + a_-, d = a_+ - a_- the five running sums of a column
+//     take X0 += s, X1 += p_x d, G0 += e s, G1 += p_x (e d), G2 += p_x^2 (e s): 9 FP64 instructions per pair of cells
+//     instead of 14, 3 shared-memory loads instead of 6;
+//   * a thread always owns the same (at most MS_MAXC) columns, so p_y, p_z, p_y^2 + p_z^2 + m^2 and the table offset
+//     are computed once per kernel, not once per cell.
+// The CTA is two teams of 8 warps; a team takes every other unit of the CTA, so two cells are reduced at a time (each
+// lane carries up to two columns: the 16-value butterfly and the cross-warp sum are paid by 8 warps per cell instead
+// of 16) while the third stage is in flight.  No CTA barrier after the prologue: the last warp of a team to finish a
+// stage re-arms it (mbarrier + bulk copy) for the unit three further on, which the other team will consume.
+// ---------------------------------------------------------------------------------------------------------------
+enum { MS_THREADS = 512, MS_TEAM = 256, MS_STAGES = 3, MS_MAXC = 2 };
+
+__global__ void __launch_bounds__(MS_THREADS, 1)
+moments_sym_kernel(const double* __restrict__ f_species, SpeciesTables tb, int nx_cells, double* __restrict__ M_species) {
+    extern __shared__ __align__(128) unsigned char mom_smem[];
+    uint64_t* bars = reinterpret_cast<uint64_t*>(mom_smem);                             // 2 MS_STAGES mbarriers: [slot][fill & 1]
+    int* done = reinterpret_cast<int*>(mom_smem + 64);                                  // [MS_STAGES] warps done with the stage
+    int* cnt = done + MS_STAGES;                                                        // [MS_STAGES] warps whose partial sums are in
+    double* red = reinterpret_cast<double*>(mom_smem + 128);                            // [MS_STAGES][8 warps][16]
+    const int c0 = tb.n[0] >> 1, odd0 = tb.n[0] & 1, c1 = tb.n[1] >> 1, odd1 = tb.n[1] & 1, c2 = tb.n[2] >> 1, odd2 = tb.n[2] & 1;
+    const int n0h = c0 + odd0, n1h = c1 + odd1, n2h = c2 + odd2, nyzh = n1h * n2h;
+    double* pxs = red + MS_STAGES * (MS_TEAM / 32) * 16;                                // [c0] p_x of the planes above the centre
+    double* px2s = pxs + c0;                                                            // [c0] their squares
+    double* iEc = px2s + c0;                                                            // [n0h][n1h][n2h] 1/E of one octant
+    const size_t np = (size_t)tb.np;
+    const size_t head = (128 + ((size_t)MS_STAGES * (MS_TEAM / 32) * 16 + 2 * (size_t)c0 + (size_t)n0h * nyzh) * 8 + 127) & ~(size_t)127;
+    const size_t stage_bytes = (np * 8 + 127) & ~(size_t)127;
+    unsigned char* ring = mom_smem + head;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int team = warp >> 3, wt = warp & 7;                                          // team 0 / 1, warp within the team
+    const int nyz = tb.n[1] * tb.n[2];
+    const int n_units = (nx_cells - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // units k = 0.. of this CTA: cell blockIdx.x + k gridDim.x
+    // Fill number m = k / 3 of slot k % 3 completes on mbarrier [slot][m & 1].  The fills of a slot alternate between the
+    // teams, so each barrier belongs to one team: its previous fill (m - 2) was waited on by the same team and its next one
+    // (m + 2) cannot be armed before that team has consumed fill m -- the barrier is either in phase m >> 1 (in flight) or
+    // one past it (landed), which the parity wait tells apart.  (One barrier per slot would not do: a team about to wait for
+    // fill m could find it in phase m - 1, m or m + 1.)
+    auto arm = [&](int slot, int k) {
+        if (k < n_units) {
+            uint64_t* bar = &bars[2 * slot + ((k / MS_STAGES) & 1)];
+            mbar_expect_tx(bar, (uint32_t)(np * 8));
+            tma_bulk_g2s(ring + (size_t)slot * stage_bytes, f_species + ((size_t)blockIdx.x + (size_t)k * gridDim.x) * np, (uint32_t)(np * 8), bar);
+        }
+    };
+    if (threadIdx.x == 0) {
+        for (int k = 0; k < MS_STAGES; ++k) { mbar_init(&bars[2 * k], 1); mbar_init(&bars[2 * k + 1], 1); done[k] = 0; cnt[k] = 0; }
+        fence_mbar_init();
+        for (int k = 0; k < MS_STAGES; ++k) arm(k, k);
+    }
+    // rows 0 .. c0-1 of the octant table: the planes above the centre (pair j = planes c0 + odd0 + j and c0 - 1 - j);
+    // row c0 (odd n only): the centre plane p_x = 0.  Likewise in y and z.
+    for (int i = threadIdx.x; i < c0; i += MS_THREADS) {
+        const double px = fma((double)(c0 + odd0 + i) + 0.5, tb.delta[0], tb.pmin[0]);
+        pxs[i] = px; px2s[i] = px * px;
+    }
+    for (int i = threadIdx.x; i < n0h * nyzh; i += MS_THREADS) {
+        const int j0 = i / nyzh, r = i - j0 * nyzh, j1 = r / n2h, j2 = r - j1 * n2h;
+        const int i0 = j0 < c0 ? c0 + odd0 + j0 : c0, i1 = j1 < c1 ? c1 + odd1 + j1 : c1, i2 = j2 < c2 ? c2 + odd2 + j2 : c2;
+        iEc[i] = __ldg(tb.iE + ((size_t)i0 * tb.n[1] + i1) * tb.n[2] + i2);
+    }
+    // this thread's columns (fixed for the whole kernel) and everything that depends on the column only
+    int col[MS_MAXC], cm[MS_MAXC];
+    bool valid[MS_MAXC];
+    double py[MS_MAXC], pz[MS_MAXC], rr[MS_MAXC];
+    const double msq = tb.mass * tb.mass;
+#pragma unroll
+    for (int q = 0; q < MS_MAXC; ++q) {
+        const int c = wt * 32 + lane + q * MS_TEAM;
+        valid[q] = c < nyz;
+        col[q] = valid[q] ? c : nyz - 1;                                  // an idle slot reads a valid column and is discarded
+        const int iy = col[q] / tb.n[2], iz = col[q] - iy * tb.n[2];
+        py[q] = fma((double)iy + 0.5, tb.delta[1], tb.pmin[1]);
+        pz[q] = fma((double)iz + 0.5, tb.delta[2], tb.pmin[2]);
+        rr[q] = fma(py[q], py[q], fma(pz[q], pz[q], msq));               // E^2 - p_x^2
+        const int m1 = iy >= c1 + odd1 ? iy - c1 - odd1 : (iy < c1 ? c1 - 1 - iy : c1);
+        const int m2 = iz >= c2 + odd2 ? iz - c2 - odd2 : (iz < c2 ? c2 - 1 - iz : c2);
+        cm[q] = m1 * n2h + m2;
+    }
+    const bool second = __any_sync(0xffffffffu, valid[1]);               // warp-uniform: does any lane carry a second column
+    const double dp3 = tb.delta[0] * tb.delta[1] * tb.delta[2];
+    __syncthreads();
+    for (int k = team; k < n_units; k += 2) {
+        const int slot = k % MS_STAGES;
+        const size_t cell = (size_t)blockIdx.x + (size_t)k * gridDim.x;
+        const double* __restrict__ fc = reinterpret_cast<const double*>(ring + (size_t)slot * stage_bytes);
+        mbar_wait(&bars[2 * slot + ((k / MS_STAGES) & 1)], (uint32_t)(k / (2 * MS_STAGES)) & 1u);
+        RBG_CHECK_STAGE(fc, f_species + cell * np, np);
+        RBG_CHECK(cell < (size_t)nx_cells && (size_t)(slot + 1) * stage_bytes + head <= dynamic_smem_size(), CHK_BE_INDEX);
+        double acc[16];
+#pragma unroll
+        for (int m = 0; m < 16; ++m) acc[m] = 0.0;
+#pragma unroll
+        for (int q = 0; q < MS_MAXC; ++q) {
+            if (q == 1 && !second) break;
+            const double* __restrict__ pf = fc + col[q];
+            const double* __restrict__ pe = iEc + cm[q];
+            double x0 = 0.0, x1 = 0.0, g0 = 0.0, g1 = 0.0, g2 = 0.0;
+            if (odd0) {                                                  // centre plane: p_x = 0
+                const double a = pf[(size_t)c0 * nyz];
+                x0 = a; g0 = a * pe[(size_t)c0 * nyzh];
+            }
+#pragma unroll 5
+            for (int j = 0; j < c0; ++j) {
+                const double ap = pf[(size_t)(c0 + odd0 + j) * nyz], am = pf[(size_t)(c0 - 1 - j) * nyz];
+                const double e = pe[(size_t)j * nyzh], px = pxs[j], px2 = px2s[j];
+                const double sm = ap + am, df = ap - am;
+                const double es = e * sm, ed = e * df;
+                x0 += sm;
+                x1 = fma(px, df, x1);
+                g0 += es;
+                g1 = fma(px, ed, g1);
+                g2 = fma(px2, es, g2);
+            }
+            if (!valid[q]) { x0 = x1 = g0 = g1 = g2 = 0.0; }
+            const double yG0 = py[q] * g0, zG0 = pz[q] * g0;
+            acc[0] += x0;                                                                     // n
+            acc[1] += g1; acc[2] += yG0; acc[3] += zG0;                                       // j
+            acc[4] += fma(rr[q], g0, g2);                                                     // T00 = S (px^2 + r) g
+            acc[5] += x1; acc[6] = fma(py[q], x0, acc[6]); acc[7] = fma(pz[q], x0, acc[7]);   // T0k
+            acc[8] += g2; acc[9] = fma(py[q], g1, acc[9]); acc[10] = fma(pz[q], g1, acc[10]); // Txx Txy Txz
+            acc[11] = fma(py[q], yG0, acc[11]); acc[12] = fma(py[q], zG0, acc[12]); acc[13] = fma(pz[q], zG0, acc[13]);
+        }
+        RBG_CHECK_STAGE(fc, f_species + cell * np, np);
+        const double tot = warp_reduce16(acc, lane);
+        double* rb = red + (size_t)slot * (MS_TEAM / 32) * 16;
+        if (lane < 16) rb[wt * 16 + mom_slot(lane)] = tot;
+        __syncwarp();
+        int last = 0;
+        if (lane == 0) {
+            __threadfence_block();
+            last = atomicAdd(&cnt[slot], 1) == MS_TEAM / 32 - 1;
+            if (last) cnt[slot] = 0;
+        }
+        last = __shfl_sync(0xffffffffu, last, 0);
+        if (last) {                                                      // the partial sums of all 8 warps of the team are in rb
+            __threadfence_block();
+            if (lane < N_MOMENTS) {
+                double v = 0.0;
+#pragma unroll
+                for (int w = 0; w < MS_TEAM / 32; ++w) v += rb[w * 16 + lane];
+                M_species[cell * N_MOMENTS + lane] = v * dp3;
+            }
+        }
+        // the warp that finishes last with this stage (its reads of the stage and of rb are complete) refills it
+        __syncwarp();
+        if (lane == 0) {
+            __threadfence_block();
+            if (atomicAdd(&done[slot], 1) == MS_TEAM / 32 - 1) {
+                done[slot] = 0;
+                arm(slot, k + MS_STAGES);
+            }
+        }
+    }
+}
+
 // total[ix][m] = Sum_a M[a][ix][m] (Eq. 7, 9); em[ix][0..3] = Sum_a Q_a (n_a, j_a) (Eq. 15).  Either may be null.
 __global__ void totals_kernel(const double* __restrict__ M, const double* __restrict__ charges, int n_species, int nx_cells,
                               double* __restrict__ total, double* __restrict__ em) {

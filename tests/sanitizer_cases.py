@@ -83,6 +83,11 @@ def be_step_cases():
         f = torch.from_numpy(w["f"]).cuda()
         M, tot, em = col.moments(f)
         _finite(M, what + " [moments]")
+        # the general staged kernel as well where the symmetric-grid kernel (three stages, two teams) was taken above
+        col.set_option("moments_path", 1)
+        M, tot, em = col.moments(f)
+        _finite(M, what + " [moments, general staged kernel]")
+        col.set_option("moments_path", 0)
         E = torch.from_numpy(rng.normal(size=(nx, 3))).cuda()
         B = torch.from_numpy(rng.normal(size=(nx, 3))).cuda()
         _finite(col.vlasov_step(f, 0.01, E, B), what + " [vlasov]")

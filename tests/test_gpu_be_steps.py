@@ -29,8 +29,10 @@ CASES = [(2, dict(np_side=20), (3, 2, 2)),          # two species, 8000-cell gri
          (1, dict(np_side=16), (1, 1, 1))]
 
 
-@pytest.mark.parametrize("cfg,kw,nxyz", CASES)
-def test_moments_parity(cfg, kw, nxyz):
+@pytest.mark.parametrize("path", [0, 1])             # 0: symmetric-grid kernel where it applies, 1: general staged kernel
+@pytest.mark.parametrize("cfg,kw,nxyz", CASES + [(4, dict(np_side=20), (1, 1, 7)),     # one species, odd number of units
+                                                 (1, dict(np_side=7), (2, 1, 1))])    # odd np: the symmetric kernel does not apply
+def test_moments_parity(cfg, kw, nxyz, path):
     rbg = _rbg()
     w = workloads.make(cfg, nx=int(np.prod(nxyz)), **kw)
     prob = w["problem"]
@@ -40,6 +42,7 @@ def test_moments_parity(cfg, kw, nxyz):
     Mabs, totabs, _ = bs.moments(prob, np.abs(w["f"]))
     # scale of a term sum: moments of |f| with |weights| are bounded by E-weighted ones; use n and T00 of |f|
     col = rbg.Collision(_with_grid(prob, nxyz))
+    col.set_option("moments_path", path)
     M, tot, em = col.moments(torch.from_numpy(w["f"]).cuda())
     torch.cuda.synchronize()
     M, tot, em = M.cpu().numpy(), tot.cpu().numpy(), em.cpu().numpy()
@@ -181,7 +184,8 @@ def test_be_step_is_drift_then_vlasov_then_collision_with_3dt():
 @pytest.mark.parametrize("cfg,kw,nx", [(2, dict(np_side=20), 1300),      # one cell per stage, two stages: every CTA reuses its slots 4-5 times
                                        (7, dict(np_side=11), 2500),      # four cells per stage, odd np: leading cell, cooperative tails
                                        (1, dict(np_side=16), 1000)])     # two cells per stage (4096-cell grid)
-def test_staged_kernels_are_race_free_under_ring_reuse(cfg, kw, nx):
+@pytest.mark.parametrize("path", [0, 1])
+def test_staged_kernels_are_race_free_under_ring_reuse(cfg, kw, nx, path):
     """The persistent moments / Vlasov kernels recycle their shared-memory stages through mbarrier phases and warp
     arrival counters.  Many units per CTA, repeated runs: every run must equal the oracle and, bit for bit, every
     other run (both kernels add in a fixed order)."""
@@ -195,6 +199,7 @@ def test_staged_kernels_are_race_free_under_ring_reuse(cfg, kw, nx):
     M_ref, _, _ = bs.moments(prob, w["f"])
     V_ref = bs.vlasov_upfd(prob, w["f"], 0.02, E, B)
     col = rbg.Collision(prob)
+    col.set_option("moments_path", path)       # 0: the symmetric-grid moments kernel (three stages, two teams) for cfg 2 and 1
     f = torch.from_numpy(w["f"]).cuda()
     Ed, Bd = torch.from_numpy(E).cuda(), torch.from_numpy(B).cuda()
     first = None
