@@ -52,7 +52,7 @@ struct rbg_handle {
     int sm_count = 148;
     int max_smem_optin = 0;
     // options
-    int opt_warps = 0, opt_p1_per_cta = 0, opt_gather = 0, opt_spl = 0, opt_moments_path = 0;
+    int opt_warps = 0, opt_p1_per_cta = 0, opt_gather = 0, opt_spl = 0, opt_moments_path = 0, opt_vlasov_path = 0;
     int last_launches = 0;
     // per-species device tables for the moment / drift / Vlasov kernels: 1/E_p and v = p/E_p per momentum cell
     std::vector<double*> tab_iE, tab_v;
@@ -671,6 +671,7 @@ int rbg_set_option(rbg_handle* h, const char* key, int value) {
         RBG_CUDA(h, cudaDeviceSynchronize());
     }
 #endif
+    else if (k == "vlasov_path") { if (value < 0 || value > 1) return fail(h, RBG_E_INVALID_ARG, "vlasov_path must be 0 (auto) or 1 (general staged kernel)"); h->opt_vlasov_path = value; }
     else if (k == "moments_path") { if (value < 0 || value > 1) return fail(h, RBG_E_INVALID_ARG, "moments_path must be 0 (auto) or 1 (general staged kernel)"); h->opt_moments_path = value; }
     else if (k == "gather") { if (value < 0 || value > 2) return fail(h, RBG_E_INVALID_ARG, "gather must be 0, 1 or 2"); h->opt_gather = value; }
     else return fail(h, RBG_E_INVALID_ARG, "unknown option " + k);
@@ -890,6 +891,32 @@ int rbg_vlasov_step(rbg_handle* h, const double* f_dev, double* f_out_dev, doubl
         const double* fs = f_dev + h->sp_off[s];
         double* os = f_out_dev + h->sp_off[s];
         const int nyz = tb.n[1] * tb.n[2];
+        // Momentum grid symmetric about 0 in every direction, at most 800 (p_y, p_z) columns, a cell of whole 16-byte units
+        // that fits three times next to the octant table: vlasov_sym_kernel (rbg_be_kernels.cuh)
+        {
+            bool sym = h->opt_vlasov_path != 1 && nyz <= rbg::VS_MAX_THREADS && nyz % 2 == 0 &&          // planes of whole 16-byte units
+                       reinterpret_cast<uintptr_t>(fs) % 16 == 0;
+            for (int d = 0; d < 3; ++d) {
+                const rbg_momentum_grid& G = h->grids[s];
+                sym = sym && std::fabs(G.pmin[d] + G.pmax[d]) <= 1e-12 * (G.pmax[d] - G.pmin[d]);
+            }
+            const int n0h = (tb.n[0] + 1) / 2, n1h = (tb.n[1] + 1) / 2, n2h = (tb.n[2] + 1) / 2;
+            const size_t head_sym = (128 + (size_t)tb.n[0] * 16 + (size_t)n0h * n1h * n2h * 8 + 127) & ~(size_t)127;
+            // a stage holds the cell plus one halo plane on either side (the periodic p_x neighbours)
+            const size_t smem_sym = head_sym + (size_t)rbg::VS_STAGES * (((size_t)tb.np * 8 + 2 * (size_t)nyz * 8 + 127) & ~(size_t)127);
+            if (sym && smem_sym <= (size_t)h->max_smem_optin) {
+                // segments per column: as many as fit in 800 threads, each of ceil(n0 / segs) planes
+                int segs = std::max(1, std::min(tb.n[0], rbg::VS_MAX_THREADS / nyz));
+                const int seg_len = (tb.n[0] + segs - 1) / segs;
+                segs = (tb.n[0] + seg_len - 1) / seg_len;
+                const int threads = ((segs * nyz + 31) / 32) * 32;
+                RBG_CUDA(h, ensure_max_smem(rbg::vlasov_sym_kernel, h->device, h->max_smem_optin));
+                rbg::vlasov_sym_kernel<<<std::max(1, std::min(h->sm_count, h->nx)), threads, smem_sym, st>>>(fs, os, tb, vp, segs, seg_len);
+                RBG_CUDA(h, cudaGetLastError());
+                ++h->last_launches;
+                continue;
+            }
+        }
         const size_t head = (128 + (size_t)tb.n[0] * 8 + 127) & ~(size_t)127;
         const StagedGeometry g = staged_geometry(h, s, fs, head, true);
         if (!g.ok) {                                   // the block does not fit twice next to the table: direct kernel

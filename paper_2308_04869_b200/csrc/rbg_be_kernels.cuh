@@ -744,6 +744,143 @@ vlasov_upfd_kernel(const double* __restrict__ f_species, double* __restrict__ ou
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// Vlasov step on a momentum grid symmetric about p = 0 (every workload of the paper), one spatial cell per stage.
+// Same update as vlasov_upfd_kernel; differences:
+//   * octant 1/E table (8 KB instead of 64 KB at 20^3): the ring has three stages;
+//   * a column (ipy, ipz) is split into VS segments along ipx, one thread per (segment, column): 800 threads = 25 warps
+//     at 20^3 where the column-per-thread kernel keeps 12.5 of its 16 warps busy (the kernel is latency-bound: 47 % issue
+//     utilisation in round 1), at <= 80 registers;
+//   * a thread always owns the same column and segment, so everything that depends on the momentum cell's (ipy, ipz) is
+//     computed once per kernel; per spatial cell the force is built from pre-scaled fields,
+//       c_x = dt |F_x| / dp_x = | e Ax + Ex' |,  Ax = k0 Q (p_y B_z - p_z B_y),  Ex' = k0 Q E_x,  e = 1 / E_p,
+//       c_y = | e (Ay - p_x Bz') + Ey' |,  c_z = | e (p_x By' - Az) + Ez' |     (k_d = dt / dp_d folded into the constants),
+//     5 FMAs per cell instead of 3 multiplies, 6 FMAs and 3 scalings.
+// Every warp consumes every unit; the last warp to finish with a stage re-arms it (as in vlasov_upfd_kernel).
+// ---------------------------------------------------------------------------------------------------------------
+enum { VS_MAX_THREADS = 800, VS_STAGES = 3 };
+struct __align__(16) VsPlane { double px; int erow; int pad; };   // per ipx: p_x and the byte offset of its row in the octant table
+
+__global__ void __launch_bounds__(VS_MAX_THREADS, 1)
+vlasov_sym_kernel(const double* __restrict__ f_species, double* __restrict__ out_species, SpeciesTables tb, VlasovParams vp,
+                  int segs, int seg_len) {
+    extern __shared__ __align__(128) unsigned char mom_smem[];
+    uint64_t* bars = reinterpret_cast<uint64_t*>(mom_smem);                             // VS_STAGES mbarriers
+    int* done = reinterpret_cast<int*>(mom_smem + 64);                                  // [VS_STAGES] warps done with the stage
+    VsPlane* xtab = reinterpret_cast<VsPlane*>(mom_smem + 128);                         // [n0]
+    const int n0 = tb.n[0], n1 = tb.n[1], n2 = tb.n[2], nyz = n1 * n2;
+    const int c0 = n0 >> 1, odd0 = n0 & 1, c1 = n1 >> 1, odd1 = n1 & 1, c2 = n2 >> 1, odd2 = n2 & 1;
+    const int n0h = c0 + odd0, n1h = c1 + odd1, n2h = c2 + odd2, nyzh = n1h * n2h;
+    double* iEc = reinterpret_cast<double*>(xtab + n0);                                 // [n0h][n1h][n2h] 1/E of one octant
+    const size_t np = (size_t)tb.np;
+    const size_t head = (128 + (size_t)n0 * 16 + (size_t)n0h * nyzh * 8 + 127) & ~(size_t)127;
+    // a stage = [plane n0-1][the cell's n0 planes][plane 0]: the periodic p_x neighbours of the first and the
+    // last plane are read like any other, without index wrapping in the loop
+    const uint32_t plane_bytes = (uint32_t)nyz * 8u;
+    const size_t stage_bytes = (np * 8 + 2 * (size_t)plane_bytes + 127) & ~(size_t)127;
+    unsigned char* ring = mom_smem + head;
+    const int lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
+    const int n_units = (vp.nx_cells - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    auto arm = [&](int slot, int k) {
+        if (k < n_units) {
+            const double* src = f_species + ((size_t)blockIdx.x + (size_t)k * gridDim.x) * np;
+            unsigned char* dst = ring + (size_t)slot * stage_bytes;
+            mbar_expect_tx(&bars[slot], (uint32_t)(np * 8) + 2u * plane_bytes);
+            tma_bulk_g2s(dst + plane_bytes, src, (uint32_t)(np * 8), &bars[slot]);
+            tma_bulk_g2s(dst, src + (np - (size_t)nyz), plane_bytes, &bars[slot]);
+            tma_bulk_g2s(dst + plane_bytes + np * 8, src, plane_bytes, &bars[slot]);
+        }
+    };
+    if (threadIdx.x == 0) {
+        for (int k = 0; k < VS_STAGES; ++k) { mbar_init(&bars[k], 1); done[k] = 0; }
+        fence_mbar_init();
+        for (int k = 0; k < VS_STAGES; ++k) arm(k, k);
+    }
+    // rows 0 .. c0-1 of the octant table: the planes above the centre; row c0 (odd n only): the centre plane; likewise in
+    // y and z (as in moments_sym_kernel)
+    for (int i = threadIdx.x; i < n0; i += blockDim.x) {
+        const int mi = i >= c0 + odd0 ? i - c0 - odd0 : (i < c0 ? c0 - 1 - i : c0);
+        xtab[i].px = fma((double)i + 0.5, tb.delta[0], tb.pmin[0]);
+        xtab[i].erow = mi * nyzh * 8;
+        xtab[i].pad = 0;
+    }
+    for (int i = threadIdx.x; i < n0h * nyzh; i += blockDim.x) {
+        const int j0 = i / nyzh, r = i - j0 * nyzh, j1 = r / n2h, j2 = r - j1 * n2h;
+        const int i0 = j0 < c0 ? c0 + odd0 + j0 : c0, i1 = j1 < c1 ? c1 + odd1 + j1 : c1, i2 = j2 < c2 ? c2 + odd2 + j2 : c2;
+        iEc[i] = __ldg(tb.iE + ((size_t)i0 * n1 + i1) * n2 + i2);
+    }
+    // this thread's (segment, column): fixed for the whole kernel
+    const int seg = (int)threadIdx.x / nyz, c = (int)threadIdx.x - seg * nyz;
+    const bool active = seg < segs;
+    const int i_lo = min(seg * seg_len, n0), i_hi = active ? min(i_lo + seg_len, n0) : i_lo;
+    const int iy = c / n2, iz = c - iy * n2;
+    const double py = fma((double)iy + 0.5, tb.delta[1], tb.pmin[1]);
+    const double pz = fma((double)iz + 0.5, tb.delta[2], tb.pmin[2]);
+    // byte offsets of the periodic p_y, p_z neighbours relative to the cell itself (the same in every plane)
+    const int dym = (iy > 0 ? -n2 : (n1 - 1) * n2) * 8, dyp = (iy < n1 - 1 ? n2 : -(n1 - 1) * n2) * 8;
+    const int dzm = (iz > 0 ? -1 : n2 - 1) * 8, dzp = (iz < n2 - 1 ? 1 : -(n2 - 1)) * 8;
+    const int m1 = iy >= c1 + odd1 ? iy - c1 - odd1 : (iy < c1 ? c1 - 1 - iy : c1);
+    const int m2 = iz >= c2 + odd2 ? iz - c2 - odd2 : (iz < c2 ? c2 - 1 - iz : c2);
+    const unsigned char* __restrict__ pe = reinterpret_cast<const unsigned char*>(iEc + m1 * n2h + m2);
+    const double k0 = vp.dt / tb.delta[0], k1 = vp.dt / tb.delta[1], k2 = vp.dt / tb.delta[2];
+    const double Q = tb.charge;
+    const double third = 1.0 / 3.0;
+    const size_t j_lo = (size_t)i_lo * nyz + c;
+    __syncthreads();
+    uint32_t phases = 0;
+    for (int k = 0; k < n_units; ++k) {
+        const int slot = k % VS_STAGES;
+        const size_t cell = (size_t)blockIdx.x + (size_t)k * gridDim.x;
+        const unsigned char* __restrict__ fcb = ring + (size_t)slot * stage_bytes + plane_bytes;    // plane 0 of the cell
+        // F = Q (E + v x B); Q and dt / dp_d folded into the fields of this spatial cell
+        const double* __restrict__ Ev = vp.E + cell * 3;
+        const double* __restrict__ Bv = vp.B + cell * 3;
+        const double QBx = Q * __ldg(Bv), QBy = Q * __ldg(Bv + 1), QBz = Q * __ldg(Bv + 2);
+        const double Ex = k0 * (Q * __ldg(Ev)), Ey = k1 * (Q * __ldg(Ev + 1)), Ez = k2 * (Q * __ldg(Ev + 2));
+        const double Ax = k0 * fma(py, QBz, -(pz * QBy));               // k0 Q E_p (v x B)_x
+        const double Ay = k1 * (pz * QBx), Bz1 = k1 * QBz;              // k1 Q E_p (v x B)_y = Ay - p_x Bz1
+        const double Az = k2 * (py * QBx), By2 = k2 * QBy;              // k2 Q E_p (v x B)_z = p_x By2 - Az
+        mbar_wait(&bars[slot], (phases >> slot) & 1u);
+        phases ^= 1u << slot;
+        RBG_CHECK_STAGE(reinterpret_cast<const double*>(fcb), f_species + cell * np, np);
+        RBG_CHECK(cell < (size_t)vp.nx_cells && (size_t)(slot + 1) * stage_bytes + head <= dynamic_smem_size(), CHK_BE_INDEX);
+        // walk up the segment with the p_x neighbours in registers: one load brings the next plane's value
+        const unsigned char* __restrict__ a = fcb + j_lo * 8;
+        double* __restrict__ op = out_species + cell * np + j_lo;
+        double prev = *reinterpret_cast<const double*>(a - plane_bytes);
+        double cur = active ? *reinterpret_cast<const double*>(a) : 0.0;
+#pragma unroll 2
+        for (int i = i_lo; i < i_hi; ++i) {
+            const double next = *reinterpret_cast<const double*>(a + plane_bytes);
+            const VsPlane xp = xtab[i];
+            const double e = *reinterpret_cast<const double*>(pe + xp.erow);
+            const double Fx = fma(e, Ax, Ex);
+            const double Fy = fma(e, fma(-xp.px, Bz1, Ay), Ey);
+            const double Fz = fma(e, fma(xp.px, By2, -Az), Ez);
+            const double u0 = Fx > 0.0 ? prev : next;
+            const double u1 = *reinterpret_cast<const double*>(a + (Fy > 0.0 ? dym : dyp));
+            const double u2 = *reinterpret_cast<const double*>(a + (Fz > 0.0 ? dzm : dzp));
+            const double cxd = fabs(Fx), cyd = fabs(Fy), czd = fabs(Fz);
+            const double num = fma(czd, u2, fma(cyd, u1, fma(cxd, u0, cur * third)));
+            const double den = ((third + cxd) + cyd) + czd;
+            __stcs(op, num * rcp_fast(den));                             // den >= 1/3: no range checks; ~1 ulp
+            prev = cur; cur = next;
+            a += plane_bytes; op += nyz;
+        }
+        RBG_CHECK_STAGE(reinterpret_cast<const double*>(fcb), f_species + cell * np, np);
+        // the last warp to finish with this stage (its shared-memory reads have completed: their values were consumed by
+        // the stores above) refills it
+        __syncwarp();
+        if (lane == 0) {
+            __threadfence_block();
+            if (atomicAdd(&done[slot], 1) == nwarps - 1) {
+                done[slot] = 0;
+                arm(slot, k + VS_STAGES);
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // Direct (unstaged) variants for momentum grids whose block of one spatial cell does not fit in shared memory twice
 // (e.g. the paper's 35^3 test grid, 343 KB): same arithmetic, f read straight from global memory / L2.
 // ---------------------------------------------------------------------------------------------------------------

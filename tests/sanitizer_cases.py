@@ -91,6 +91,9 @@ def be_step_cases():
         E = torch.from_numpy(rng.normal(size=(nx, 3))).cuda()
         B = torch.from_numpy(rng.normal(size=(nx, 3))).cuda()
         _finite(col.vlasov_step(f, 0.01, E, B), what + " [vlasov]")
+        col.set_option("vlasov_path", 1)
+        _finite(col.vlasov_step(f, 0.01, E, B), what + " [vlasov, general staged kernel]")
+        col.set_option("vlasov_path", 0)
     for what, cfg, kw, nxyz, bc, zeta in (("drift: periodic", 2, dict(np_side=8), (5, 4, 3), (1, 1, 1), 0.0),
                                           ("drift: reflecting and absorbing walls", 7, dict(np_side=5), (3, 6, 4), (0, 1, 0), 0.6)):
         nx = int(np.prod(nxyz))

@@ -78,9 +78,13 @@ def test_drift_step_parity(cfg, kw, nxyz, bc, zeta):
     assert np.allclose(out, w["f"], rtol=1e-13) == (int(np.prod(nxyz)) == 1)
 
 
+@pytest.mark.parametrize("path", [0, 1])             # 0: symmetric-grid kernel where it applies, 1: general staged kernel
 @pytest.mark.parametrize("cfg,kw,nx", [(2, dict(np_side=8), 7), (7, dict(np_side=5), 20), (2, dict(np_side=20), 3),
-                                       (3, dict(np_side=6), 17)])
-def test_vlasov_step_parity(cfg, kw, nx):
+                                       (3, dict(np_side=6), 17),
+                                       (4, dict(np_side=20), 301),    # several units per CTA: every ring slot is re-armed
+                                       (1, dict(np_side=10), 5),      # 100 columns: 5 segments of 2 planes per column
+                                       (1, dict(np_side=28), 2)])     # 784 columns: one segment, 800 threads
+def test_vlasov_step_parity(cfg, kw, nx, path):
     rbg = _rbg()
     w = workloads.make(cfg, nx=nx, **kw)
     prob = w["problem"]
@@ -93,6 +97,7 @@ def test_vlasov_step_parity(cfg, kw, nx):
     dt = 0.02
     ref = bs.vlasov_upfd(prob, w["f"], dt, E, B)
     col = rbg.Collision(prob)
+    col.set_option("vlasov_path", path)
     out = col.vlasov_step(torch.from_numpy(w["f"]).cuda(), dt, torch.from_numpy(E).cuda(), torch.from_numpy(B).cuda())
     torch.cuda.synchronize()
     out = out.cpu().numpy()
@@ -200,6 +205,7 @@ def test_staged_kernels_are_race_free_under_ring_reuse(cfg, kw, nx, path):
     V_ref = bs.vlasov_upfd(prob, w["f"], 0.02, E, B)
     col = rbg.Collision(prob)
     col.set_option("moments_path", path)       # 0: the symmetric-grid moments kernel (three stages, two teams) for cfg 2 and 1
+    col.set_option("vlasov_path", path)        # 0: the symmetric-grid Vlasov kernel (three stages, 800 / 768 threads)
     f = torch.from_numpy(w["f"]).cuda()
     Ed, Bd = torch.from_numpy(E).cuda(), torch.from_numpy(B).cuda()
     first = None
