@@ -832,8 +832,8 @@ int rbg_drift_step(rbg_handle* h, const double* f_dev, double* f_out_dev, const 
     cudaStream_t st = (cudaStream_t)cuda_stream;
     DeviceGuard guard(h->device);
     h->last_launches = 0;
-    dp.zseg = std::min(16, h->nxyz[2]);
-    dp.tile_y = std::min(8, h->nxyz[1]);
+    dp.zseg = std::min(16, h->nxyz[2]);                 // measured on config 4: segments of 8 or 32 cells are slower
+    dp.tile_y = std::min(8, h->nxyz[1]);                // measured on config 4: tiles of 2, 4 or 16 rows are slower
     const long nzseg = (h->nxyz[2] + dp.zseg - 1) / dp.zseg, nyt = (h->nxyz[1] + dp.tile_y - 1) / dp.tile_y;
     for (int s = 0; s < h->n_species; ++s) {
         const long nchunks = ((long)h->np[s] + 255) / 256;

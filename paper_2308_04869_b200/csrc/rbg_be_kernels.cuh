@@ -460,7 +460,7 @@ struct DriftParams {
     int tile_y;              // rows per y tile (CTA order: y tile, i_x, row in tile, z segment, momentum chunk)
 };
 
-enum { STENCIL_BATCH = 4 };  // spatial cells whose loads are issued together
+enum { STENCIL_BATCH = 4 };  // spatial cells whose loads are issued together (measured on config 4: 3, 6, 8 are slower)
 
 // CTA = (momentum chunk of 256 cells) x (segment of a z row).  CTAs are ordered so that consecutive CTAs walk along x
 // inside a tile of tile_y rows: the x neighbour of a cell was read tile_y * nz spatial cells earlier and is still in
@@ -514,33 +514,53 @@ drift_upfd_kernel(const double* __restrict__ f_species, double* __restrict__ out
     upwind(0, ixx, offx, csx);
     upwind(1, iy, offy, csy);
     const size_t row0 = ((size_t)ixx * dp.nxyz[1] + iy) * dp.nxyz[2];
-    for (int zb = z0; zb < z1; zb += STENCIL_BATCH) {
-        double self[STENCIL_BATCH], ux[STENCIL_BATCH], uy[STENCIL_BATCH], uz[STENCIL_BATCH], csz[STENCIL_BATCH];
+    // Walk the z segment in the direction of v_z, so that the upwind z neighbour of a cell is the cell visited just before
+    // it: three loads per cell (itself, the x and the y neighbour) instead of four, and only the first cell of the walk needs
+    // the general neighbour rule (interior / periodic / wall ghost).  Lanes with v_z < 0 walk down while the others walk up;
+    // each still reads and writes runs of consecutive momentum cells.
+    const int len = z1 - z0, zstart = sgn[2] > 0 ? z0 : z1 - 1;
+    const ptrdiff_t step = sgn[2] > 0 ? np : -np;
+    const double* __restrict__ ps = f_species + (row0 + zstart) * np;            // momentum block of the cell being visited
+    double* __restrict__ po = out_species + (row0 + zstart) * np + ip;
+    ptrdiff_t offz;
+    double cz;
+    upwind(2, zstart, offz, cz);
+#ifdef RBG_CHECKED
+    const ptrdiff_t total = (ptrdiff_t)dp.nxyz[0] * dp.nxyz[1] * dp.nxyz[2] * np;
+    {
+        const ptrdiff_t base = (ptrdiff_t)(row0 + zstart) * np;
+        RBG_CHECK(base + offz >= 0 && base + offz < total, CHK_BE_INDEX);
+    }
+#endif
+    double prev = __ldg(ps + offz);                                             // upwind z neighbour (or wall ghost) of the first cell
+    const double third = 1.0 / 3.0;
+    for (int t = 0; t < len; t += STENCIL_BATCH) {
+        double self[STENCIL_BATCH], ux[STENCIL_BATCH], uy[STENCIL_BATCH];
 #pragma unroll
         for (int k = 0; k < STENCIL_BATCH; ++k) {
-            const int z = min(zb + k, z1 - 1);                       // the tail repeats the last cell (not stored)
-            const double* __restrict__ row = f_species + (row0 + z) * np;
-            ptrdiff_t offz;
-            upwind(2, z, offz, csz[k]);
+            const double* __restrict__ row = ps + (ptrdiff_t)min(k, len - 1 - t) * step;    // the tail repeats the last cell (not stored)
 #ifdef RBG_CHECKED
             {   // every address of the stencil lies inside the species block
-                const ptrdiff_t total = (ptrdiff_t)dp.nxyz[0] * dp.nxyz[1] * dp.nxyz[2] * np, base = (ptrdiff_t)(row0 + z) * np;
+                const ptrdiff_t base = row - f_species;
                 RBG_CHECK(base + ip >= 0 && base + ip < total && base + offx >= 0 && base + offx < total && base + offy >= 0 &&
-                          base + offy < total && base + offz >= 0 && base + offz < total, CHK_BE_INDEX);
+                          base + offy < total, CHK_BE_INDEX);
             }
 #endif
             self[k] = __ldg(row + ip);
             ux[k] = __ldg(row + offx);
             uy[k] = __ldg(row + offy);
-            uz[k] = __ldg(row + offz);
         }
 #pragma unroll
         for (int k = 0; k < STENCIL_BATCH; ++k) {
-            if (zb + k < z1) {
-                const double num = fma(csz[k], uz[k], fma(csy, uy[k], fma(csx, ux[k], self[k] * (1.0 / 3.0))));
-                __stcs(out_species + (row0 + zb + k) * np + ip, num * rden);
+            if (t + k < len) {
+                const double num = fma(cz, prev, fma(csy, uy[k], fma(csx, ux[k], self[k] * third)));
+                __stcs(po + (ptrdiff_t)k * step, num * rden);
+                prev = self[k];
+                cz = c[2];                                                       // every later cell has an interior neighbour
             }
         }
+        ps += (ptrdiff_t)STENCIL_BATCH * step;
+        po += (ptrdiff_t)STENCIL_BATCH * step;
     }
 }
 
