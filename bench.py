@@ -171,8 +171,8 @@ def config_block(w, args, world):
 
 # ---- the NEXT-4 kernels -----------------------------------------------------------------------------------------
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the NEXT-4 kernels on config 4 at full size, from the committed
-# `ncu --set full` captures (profiles/r1d_be_steps_and_qgp.md, captures D and F); null for other workloads.
-NCU_TRAFFIC_BE_CFG4 = {"moments": 2.097e9 + 7.1e6, "drift": 2.460e9 + 2.087e9, "vlasov": 2.099e9 + 2.042e9,
+# `ncu --set full` captures (profiles/r2_be_steps.md; drift_pfl: profiles/r1d_be_steps_and_qgp.md, capture F); null otherwise.
+NCU_TRAFFIC_BE_CFG4 = {"moments": 2.097e9 + 7.4e6, "drift": 2.495e9 + 2.071e9, "vlasov": 2.099e9 + 2.042e9,
                        "drift_pfl": 5.233e9 + 2.083e9}
 
 
@@ -240,7 +240,7 @@ def run_be_steps(args):
             ms = sum(ts) / len(ts)
             gbs = bytes_per_cell * cells / (ms * 1e-3) / 1e9
             res[name] = {"ms": ms, "algorithmic_bytes_per_cell": bytes_per_cell, "achieved_gbs": gbs, "frac": gbs / peak,
-                         "traffic": NCU_TRAFFIC_BE_CFG4.get(name) if (args.config == 4 and args.nx is None) else None}
+                         "traffic": NCU_TRAFFIC_BE_CFG4.get(name) if (args.config == 4 and args.nx is None and not args.opt) else None}
     clocks = cs.summary()
     t_step = sum(r["ms"] for k, r in res.items() if k != "drift_pfl") * 1e-3
     # e2e: host buffers in, host buffers out, for the three calls of one step
@@ -255,6 +255,7 @@ def run_be_steps(args):
     torch.cuda.synchronize()
     t_e2e = time.perf_counter() - t0
     dom = max(("drift", "vlasov"), key=lambda k: res[k]["ms"])
+    kern_name = {"drift": "rbg::drift_upfd_kernel", "vlasov": "rbg::vlasov_sym_kernel / rbg::vlasov_upfd_kernel"}[dom]
     line = {"metric": "be_step_phase_space_cells_per_s", "value": cells / t_step, "unit": "cells/s", "n_gpus": 1, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": t_step * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -264,7 +265,7 @@ def run_be_steps(args):
             "e2e": {"value": cells / t_e2e, "unit": "cells/s", "h2d_bytes_per_step": int(w["f"].nbytes),
                     "d2h_bytes_per_step": int(w["f"].nbytes) + int(em.numel() * 8), "ms_per_step": t_e2e * 1e3},
             "roofline": {"bound": "hbm", "achieved": res[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s", "frac": res[dom]["frac"],
-                         "traffic": res[dom]["traffic"], "kernel": f"rbg::{dom}_upfd_kernel", "peak_source": peak_src},
+                         "traffic": res[dom]["traffic"], "kernel": kern_name, "peak_source": peak_src},
             "kernels": res}
     if not args.no_cpu_baseline:
         from oracle import be_steps as bs
