@@ -113,7 +113,15 @@ class ClockSampler:
                 if v.strip().lower() == "active":
                     reasons.add(name)
         if not sm:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+            # the timed region was shorter than one sampling period (configs 1 and 6): one sample right after it instead
+            try:
+                r = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i", str(self.gpu)],
+                                   capture_output=True, text=True, timeout=20).stdout.strip().split(",")
+                reasons = sorted(n for n, v in zip(names, r[5:9]) if v.strip().lower() == "active")
+                return {"sm_mhz": float(r[1]), "sm_max_mhz": float(r[2]), "reasons": reasons, "samples": 0,
+                        "note": "timed region shorter than the 100 ms sampling period: one sample taken right after it"}
+            except (OSError, ValueError, IndexError, subprocess.TimeoutExpired):
+                return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
 
 
@@ -547,7 +555,8 @@ def main():
                                else "pinned host -> device copy, device entry point, device -> pinned host copy"},
                 "roofline": roofline_of(rbg, torch, res, args, local, probe_cache)}
         # ---- every other BASELINE config in the same record (N = 1 only) -------------------------------------------
-        if world == 1 and not args.no_config_block and args.config == HEADLINE_CONFIG and args.nx is None and not args.opt:
+        if (world == 1 and not args.no_config_block and args.config == HEADLINE_CONFIG and args.nx is None and not args.opt
+                and args.estimator == "standard" and not args.sampler):
             block = {}
             for cfg in BLOCK_CONFIGS:
                 r = time_config(rbg, torch, cfg, args, args.block_steps, 3, 0, 1, local, e2e=False)
