@@ -223,18 +223,28 @@ def test_staged_kernels_are_race_free_under_ring_reuse(cfg, kw, nx, path):
             assert torch.equal(M, first[0]) and torch.equal(V, first[1]), rep
 
 
-def _tiny_problem(n, nx):
+def _tiny_problem(n, nx, asym=False):
+    """asym: the first species' box is not symmetric about p_x = 0 (the symmetric-grid kernels must not be taken for it)."""
     return dict(nx=nx, species=[dict(mass=0.4, charge=-1.0, stat=0, g=1.0), dict(mass=0.0, charge=2.0, stat=0, g=1.0)],
-                grids=[dict(n=list(n), pmin=[-1.0, -2.0, -1.5], pmax=[1.0, 2.0, 1.5]), dict(n=list(n[::-1]), pmin=[-2.0] * 3, pmax=[2.0] * 3)],
+                grids=[dict(n=list(n), pmin=[-1.0, -2.0, -1.5], pmax=[1.75 if asym else 1.0, 2.0, 1.5]),
+                       dict(n=list(n[::-1]), pmin=[-2.0] * 3, pmax=[2.0] * 3)],
                 processes=[], hbar=1.0)
 
 
-@pytest.mark.parametrize("n,nx", [((1, 1, 1), 1), ((1, 1, 1), 37), ((2, 1, 3), 5), ((3, 7, 1), 64), ((1, 40, 33), 3)])
-def test_be_steps_on_degenerate_momentum_grids(n, nx):
+@pytest.mark.parametrize("n,nx,asym", [((1, 1, 1), 1, False), ((1, 1, 1), 37, False), ((2, 1, 3), 5, False), ((3, 7, 1), 64, False),
+                                       ((1, 40, 33), 3, False),
+                                       # even cell counts with odd extents: the symmetric-grid kernels with a centre plane / row
+                                       ((3, 2, 2), 40, False), ((1, 2, 2), 7, False), ((7, 6, 2), 9, False),
+                                       ((5, 4, 6), 700, False),      # five units per CTA: every ring slot re-armed, centre plane
+                                       ((2, 24, 32), 5, False),      # 768 columns: Vlasov one segment per column, moments general kernel
+                                       ((20, 3, 1), 11, False),      # three columns: twenty one-plane segments per column
+                                       ((4, 4, 4), 300, True)])      # box not symmetric about p_x = 0: general kernels
+def test_be_steps_on_degenerate_momentum_grids(n, nx, asym):
     """Edge cases: one momentum cell (its own periodic neighbour), extents of 1 along some axes, a (ipy, ipz) plane wider
-    than a team (1 x 40 x 33), a massless species with a cell at p = 0, no processes at all."""
+    than a team (1 x 40 x 33), odd extents in the symmetric-grid kernels, a box that is not symmetric, a massless species
+    with a cell at p = 0, no processes at all."""
     rbg = _rbg()
-    prob = _tiny_problem(n, nx)
+    prob = _tiny_problem(n, nx, asym)
     rng = np.random.default_rng(21)
     npc = int(np.prod(n))
     f = rng.random(2 * nx * npc) + 0.05
