@@ -169,16 +169,21 @@ cudaError_t launch_one(const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp
     return cudaGetLastError();
 }
 
-// Launch geometries: CTAs of up to 16 warps evaluate SPL = 2 samples per lane and loop iteration (128 registers per
-// thread), up to 32 warps SPL = 1 (64 registers; elastic roles only).  Both keep the whole register file of an SM busy
-// with one CTA; results are bit-identical (fixed lane summation order).  Measured (profiles/r2_collision.md): 4 samples
-// per lane at 8 warps and 255 registers is 2-5 % slower than SPL = 2 once the azimuth comes from shared memory.
+// Launch geometries.  SPL = 2 samples per lane and loop iteration: the double chain in CTAs of up to 12 warps (384 threads,
+// up to 168 registers per thread: 159 used, no spills, no constant re-loads in the loop), its Table III kinds and the float
+// chain in CTAs of up to 16 warps (128 registers).  Wider CTAs (up to 32 warps, 64 registers) evaluate SPL = 1 (elastic roles only).  Results are
+// bit-identical (fixed lane summation order).  Measured on config 4 / config 2 (profiles/r2_collision.md): 12 warps
+// 9.66e10 / 9.18e10 samples/s, 16 warps at 128 registers 9.33e10 / 8.88e10, 8 / 10 / 11 / 13 warps 8.98 / 8.10 / 8.85 /
+// 7.54e10 (warp counts that do not divide over the four schedulers lose); 4 samples per lane at 8 warps is 2-5 % slower
+// than SPL = 2; the float chain gains nothing from 20-24 warps.
+// (the Table III kinds need 130-143 registers and run 7 % faster on config 7 with 16 warps at 128 than with 12 warps)
+template <typename R, int KIND> constexpr int kSpl2Threads = (sizeof(R) == 8 && KIND != rbg::KIND_QCD) ? 384 : 512;
 template <typename R, int KIND, bool Q, bool SMEM, bool TCH, bool INEL>
 cudaError_t launch_geo(int spl, const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp, int grid, int threads,
                        size_t smem, const LaunchCtx& st) {
     if constexpr (!INEL)
         if (spl == 1) return launch_one<R, KIND, Q, SMEM, 1024, 1, TCH, INEL>(rp, lp, grid, threads, smem, st);
-    return launch_one<R, KIND, Q, SMEM, 512, 2, TCH, INEL>(rp, lp, grid, threads, smem, st);
+    return launch_one<R, KIND, Q, SMEM, kSpl2Threads<R, KIND>, 2, TCH, INEL>(rp, lp, grid, threads, smem, st);
 }
 
 // inel: general roles (species 3,4 differ from 1,2), uniform sampler only
@@ -226,12 +231,15 @@ int run_roles(rbg_handle* h, const double* f, double* out, bool update, double d
         const Role& r = h->roles[ir];
         const rbg::RoleParams<R> rp = make_role_params<R>(*h, r);
         const bool inel = !r.elastic;
-        // samples per lane: 2 (at most 16 warps) unless the option or a wider CTA asks for 1 (elastic roles only)
+        // samples per lane: 2 (at most 12 / 16 warps, double / float chain) unless the option or a wider CTA asks for 1
+        // (elastic roles only)
         const int np1 = rp.np[0];
+        // widest CTA of the two-samples-per-lane kernels of this chain and kind
+        const int kW2 = (r.kind >= RBG_M2_QCD_Q1Q2 ? kSpl2Threads<R, rbg::KIND_QCD> : kSpl2Threads<R, rbg::KIND_CONST>) / 32;
         int spl = h->opt_spl > 0 ? h->opt_spl : 2;
-        int warps = h->opt_warps > 0 ? h->opt_warps : 32 / spl;
-        if (inel && warps > 16) warps = 16;
-        if (warps > 16) spl = 1;
+        int warps = h->opt_warps > 0 ? h->opt_warps : (spl == 2 ? kW2 : 32);
+        if (inel && warps > kW2) warps = kW2;
+        if (warps > kW2) spl = 1;
         if (inel) spl = 2;
         // Tile size T (momentum cells per CTA; one CTA per SM at a time): a CTA stages its tables (about 2 us + bytes at
         // 100 GB/s) and then takes ceil(T / warps) rounds of one p1 per warp (a round of n_samples samples per warp at
