@@ -57,8 +57,8 @@ FLOPS_PER_SAMPLE_TCHANNEL = {1: 185.0, 2: 187.0}
 FP64_LANES_PER_SM = 64          # FMA/clk/SM; confirmed by the live probe
 # dram__bytes_read.sum + dram__bytes_write.sum of one role launch at full size, from the committed `ncu --set full`
 # captures (file named beside each); null for workloads without a capture.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {2: (32.93e6 + 2.78e6, "profiles/r2_collision.md, capture C"),
-                                4: (2184746496.0 + 2083488256.0, "profiles/r2_collision.md, capture D")}
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {2: (32.91e6 + 2.41e6, "profiles/r2_collision.md, capture C"),
+                                4: (2183821056.0 + 2080522496.0, "profiles/r2_collision.md, capture D")}
 
 
 def flops_per_sweep(problem, n_samples, fp32=False):
