@@ -230,7 +230,8 @@ int rbg_last_launch_count(const rbg_handle* h);
  * "warps_per_cta" (1..32), "p1_per_cta" (momentum cells per CTA, >= 1), "samples_per_lane"
  * (1 or 2: samples a lane evaluates per loop iteration; CTAs of more than 12 warps -- 16 with RBG_FP32_KINEMATICS or a Table III kind -- use 1),
  * "gather" (1 shared memory, 2 global/L2), "moments_path" / "vlasov_path" (1: rbg_moments / rbg_vlasov_step use their general staged
- * kernel even where the symmetric-grid kernel applies).  Returns RBG_E_INVALID_ARG for an unknown key or value. */
+ * kernel even where the symmetric-grid kernel applies), "sym_tables" (1: rbg_collision_symmetric accumulates the deposits of a
+ * CTA in shared-memory tables and flushes them at its end, instead of one global atomic per deposit).  Returns RBG_E_INVALID_ARG for an unknown key or value. */
 int rbg_set_option(rbg_handle* h, const char* key, int value);
 /* Text of the last error on this handle (or of the last failed rbg_create if h is NULL). */
 const char* rbg_last_error(const rbg_handle* h);

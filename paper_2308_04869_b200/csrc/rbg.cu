@@ -52,7 +52,7 @@ struct rbg_handle {
     int sm_count = 148;
     int max_smem_optin = 0;
     // options
-    int opt_warps = 0, opt_p1_per_cta = 0, opt_gather = 0, opt_spl = 0, opt_moments_path = 0, opt_vlasov_path = 0;
+    int opt_warps = 0, opt_p1_per_cta = 0, opt_gather = 0, opt_spl = 0, opt_moments_path = 0, opt_vlasov_path = 0, opt_sym_tables = 0;
     int last_launches = 0;
     // per-species device tables for the moment / drift / Vlasov kernels: 1/E_p and v = p/E_p per momentum cell
     std::vector<double*> tab_iE, tab_v;
@@ -550,7 +550,10 @@ int rbg_collision_symmetric(rbg_handle* h, const double* f_dev, double* C_dev, i
             if (owner == i) { sp.ctab_own[i] = 1; sp.ctab_off[i] = (int)tabs; tabs += ((size_t)rp.np[i] * 8 + 15) & ~(size_t)15; }
             else { sp.ctab_own[i] = 0; sp.ctab_off[i] = sp.ctab_off[owner]; }
         }
-        const bool csmem = rbg::kDirTabBytes + tabs <= (size_t)h->max_smem_optin;
+        // Deposits go straight to C with red.global.add.f64 (one L2 atomic each) unless the option asks for per-CTA
+        // shared-memory tables: sm_100 has no fp64 shared-memory atomic add (red.shared.add.f64 compiles to a compare-and-swap
+        // loop), and the tables run 9-17 % slower (configs 4 / 7 / 2, profiles/r2_collision.md)
+        const bool csmem = h->opt_sym_tables == 1 && rbg::kDirTabBytes + tabs <= (size_t)h->max_smem_optin;
         rbg::LaunchParams lp;
         std::memset(&lp, 0, sizeof lp);
         lp.dir_tab = h->dir_tab;
@@ -679,6 +682,7 @@ int rbg_set_option(rbg_handle* h, const char* key, int value) {
         RBG_CUDA(h, cudaDeviceSynchronize());
     }
 #endif
+    else if (k == "sym_tables") { if (value < 0 || value > 1) return fail(h, RBG_E_INVALID_ARG, "sym_tables must be 0 (global atomics) or 1 (shared-memory accumulator tables)"); h->opt_sym_tables = value; }
     else if (k == "vlasov_path") { if (value < 0 || value > 1) return fail(h, RBG_E_INVALID_ARG, "vlasov_path must be 0 (auto) or 1 (general staged kernel)"); h->opt_vlasov_path = value; }
     else if (k == "moments_path") { if (value < 0 || value > 1) return fail(h, RBG_E_INVALID_ARG, "moments_path must be 0 (auto) or 1 (general staged kernel)"); h->opt_moments_path = value; }
     else if (k == "gather") { if (value < 0 || value > 2) return fail(h, RBG_E_INVALID_ARG, "gather must be 0, 1 or 2"); h->opt_gather = value; }

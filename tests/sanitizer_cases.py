@@ -57,11 +57,15 @@ def collision_cases():
 
 
 def symmetric_cases():
-    for what, cfg, kw in (("conservative estimator: shared-memory accumulators (red.shared + CTA-end flush)", 2, dict(nx=2, np_side=8, n_samples=40)),
-                          ("conservative estimator: inelastic roles", 7, dict(nx=2, np_side=4, n_samples=16)),
-                          ("conservative estimator: global accumulators (31^3 tables do not fit)", 6, dict(nx=1, np_side=31, n_samples=2))):
+    for what, cfg, kw, tables in (
+            ("conservative estimator: global atomics (default)", 2, dict(nx=2, np_side=8, n_samples=40), 0),
+            ("conservative estimator: shared-memory accumulators (red.shared + CTA-end flush)", 2, dict(nx=2, np_side=8, n_samples=40), 1),
+            ("conservative estimator: inelastic roles", 7, dict(nx=2, np_side=4, n_samples=16), 0),
+            ("conservative estimator: inelastic roles, shared-memory accumulators", 7, dict(nx=2, np_side=4, n_samples=16), 1),
+            ("conservative estimator: 31^3 tables do not fit, global atomics although tables were asked for", 6, dict(nx=1, np_side=31, n_samples=2), 1)):
         w = workloads.make(cfg, **kw)
         col = rbg.Collision(w["problem"])
+        col.set_option("sym_tables", tables)
         _finite(col.collision_symmetric(torch.from_numpy(w["f"]).cuda(), w["n_samples"], w["seed"]), what)
 
 

@@ -18,8 +18,10 @@ def _rbg():
     return rbg
 
 
-def _run(prob, f, n, seed):
+def _run(prob, f, n, seed, tables=0):
+    """tables = 1: deposits through per-CTA shared-memory tables (option "sym_tables") instead of global atomics."""
     col = _rbg().Collision(prob)
+    col.set_option("sym_tables", tables)
     C = col.collision_symmetric(torch.from_numpy(np.ascontiguousarray(f)).cuda(), n, seed)
     torch.cuda.synchronize()
     return C.cpu().numpy(), col
@@ -28,11 +30,12 @@ def _run(prob, f, n, seed):
 @pytest.mark.parametrize("cfg,kw", [(1, dict(nx=3, np_side=8, n_samples=100)), (2, dict(nx=3, np_side=10, n_samples=64)),
                                     (3, dict(nx=2, np_side=8, n_samples=48)), (7, dict(nx=2, np_side=6, n_samples=32)),
                                     (6, dict(nx=2, np_side=9, n_samples=64)), (1, dict())])
-def test_symmetric_parity(cfg, kw):
+@pytest.mark.parametrize("tables", [0, 1])
+def test_symmetric_parity(cfg, kw, tables):
     w = workloads.make(cfg, **kw)
     orc = oracle.Oracle(w["problem"])
     C_ref, mag = orc.collision_symmetric(w["f"], w["n_samples"], w["seed"])
-    C, col = _run(w["problem"], w["f"], w["n_samples"], w["seed"])
+    C, col = _run(w["problem"], w["f"], w["n_samples"], w["seed"], tables)
     err = np.abs(C - C_ref)
     assert np.all(err <= TOL * mag + 1e-300), float(np.max(err / np.maximum(mag, 1e-300)))
     assert np.any(C_ref != 0) and col.last_launch_count() == orc.n_roles
@@ -51,13 +54,14 @@ def test_symmetric_four_species_inelastic_and_global_accumulators():
     orc = oracle.Oracle(prob)
     f = np.random.default_rng(77).random(orc.f_elems) * 0.2
     C_ref, mag = orc.collision_symmetric(f, 80, 4321)
-    C, _ = _run(prob, f, 80, 4321)
-    assert np.all(np.abs(C - C_ref) <= TOL * mag + 1e-300)
-    # 35^3 tables (343 KB each) do not fit in shared memory: the deposits go to global memory
+    for tables in (0, 1):
+        C, _ = _run(prob, f, 80, 4321, tables)
+        assert np.all(np.abs(C - C_ref) <= TOL * mag + 1e-300)
+    # 35^3 tables (343 KB each) do not fit in shared memory: the deposits go to global memory whatever the option says
     w = workloads.make(6, n_samples=8)
     orc = oracle.Oracle(w["problem"])
     C_ref, mag = orc.collision_symmetric(w["f"], 8, 3)
-    C, _ = _run(w["problem"], w["f"], 8, 3)
+    C, _ = _run(w["problem"], w["f"], 8, 3, tables=1)
     assert np.all(np.abs(C - C_ref) <= TOL * mag + 1e-300)
 
 
