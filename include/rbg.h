@@ -228,7 +228,7 @@ uint64_t rbg_sample_evals(const rbg_handle* h, int n_samples);
 int rbg_last_launch_count(const rbg_handle* h);
 /* Launch geometry / gather path knobs (results do not depend on them; 0 = automatic).  key:
  * "warps_per_cta" (1..32), "p1_per_cta" (momentum cells per CTA, >= 1), "samples_per_lane"
- * (1 or 2: samples a lane evaluates per loop iteration; CTAs of more than 12 warps -- 16 with RBG_FP32_KINEMATICS or a Table III kind -- use 1),
+ * (1 or 2: samples a lane evaluates per loop iteration; CTAs of more than 12 warps -- 16 with RBG_FP32_KINEMATICS -- use 1),
  * "gather" (1 shared memory, 2 global/L2), "moments_path" / "vlasov_path" (1: rbg_moments / rbg_vlasov_step use their general staged
  * kernel even where the symmetric-grid kernel applies), "sym_tables" (1: rbg_collision_symmetric accumulates the deposits of a
  * CTA in shared-memory tables and flushes them at its end, instead of one global atomic per deposit).  Returns RBG_E_INVALID_ARG for an unknown key or value. */

@@ -170,14 +170,15 @@ cudaError_t launch_one(const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp
 }
 
 // Launch geometries.  SPL = 2 samples per lane and loop iteration: the double chain in CTAs of up to 12 warps (384 threads,
-// up to 168 registers per thread: 159 used, no spills, no constant re-loads in the loop), its Table III kinds and the float
-// chain in CTAs of up to 16 warps (128 registers).  Wider CTAs (up to 32 warps, 64 registers) evaluate SPL = 1 (elastic roles only).  Results are
+// up to 168 registers per thread: 159 used, no spills, no constant re-loads in the loop), the float chain in CTAs of up to
+// 16 warps (128 registers).  Wider CTAs (up to 32 warps, 64 registers) evaluate SPL = 1 (elastic roles only).  Results are
 // bit-identical (fixed lane summation order).  Measured on config 4 / config 2 (profiles/r2_collision.md): 12 warps
 // 9.66e10 / 9.18e10 samples/s, 16 warps at 128 registers 9.33e10 / 8.88e10, 8 / 10 / 11 / 13 warps 8.98 / 8.10 / 8.85 /
 // 7.54e10 (warp counts that do not divide over the four schedulers lose); 4 samples per lane at 8 warps is 2-5 % slower
 // than SPL = 2; the float chain gains nothing from 20-24 warps.
-// (the Table III kinds need 130-143 registers and run 7 % faster on config 7 with 16 warps at 128 than with 12 warps)
-template <typename R, int KIND> constexpr int kSpl2Threads = (sizeof(R) == 8 && KIND != rbg::KIND_QCD) ? 384 : 512;
+// (Table III kinds, row as a compile-time constant inside the kernel: config 7 runs 7.65e10 samples/s with 12 warps at 160
+// registers, 7.50e10 with 16 at 128; with the row as a run-time switch in the sample loop it was 7.2e10 / 6.7e10)
+template <typename R, int KIND> constexpr int kSpl2Threads = sizeof(R) == 8 ? 384 : 512;
 template <typename R, int KIND, bool Q, bool SMEM, bool TCH, bool INEL>
 cudaError_t launch_geo(int spl, const rbg::RoleParams<R>& rp, const rbg::LaunchParams& lp, int grid, int threads,
                        size_t smem, const LaunchCtx& st) {
