@@ -506,6 +506,8 @@ def main():
     ap.add_argument("--estimator", default="standard", choices=["standard", "symmetric"], help="symmetric: the conservative "
                     "estimator rbg_collision_symmetric (NEXT-3); the JSON line then names it")
     ap.add_argument("--opt", action="append", default=[], help="librbg option key=value (launch geometry)")
+    ap.add_argument("--evolve-steps", type=int, default=0, help="also time rbg_collision_evolve over this many explicit Euler steps "
+                    "in place (the paper's collision test, config 6: 25 000 steps, PAPER.md:469-506) and add an `evolve` object")
     ap.add_argument("--launch-check", action="store_true", help="launcher / rank plumbing only (gloo, no GPU work)")
     args = ap.parse_args()
     if args.gpus < 1:
@@ -569,6 +571,21 @@ def main():
                                                                      "flops_per_sample", "launch_ms", "traffic")},
                                    "clocks": r["clocks"]}
             line["configs"] = block
+        if args.evolve_steps > 0 and world == 1:
+            # the paper's collision-dominated run: n Euler steps f <- f + dt C[f] in place, every step a full sweep with its
+            # own seed (rbg_collision_evolve); wall clock around the call, device synchronised on both sides
+            col = rbg.Collision(w["problem"], fp32_kinematics=w["fp32"])
+            fe = torch.from_numpy(w["f"]).cuda()
+            dt_e = w["dt"] if w["dt"] > 0 else 1e-3
+            col.collision_evolve(fe, dt_e, 3, w["n_samples"], w["seed"])             # warm-up
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            _, negf = col.collision_evolve(fe, dt_e, args.evolve_steps, w["n_samples"], w["seed"])
+            torch.cuda.synchronize()
+            t_ev = time.perf_counter() - t0
+            line["evolve"] = {"steps": args.evolve_steps, "seconds": t_ev, "ms_per_step": 1e3 * t_ev / args.evolve_steps, "dt": dt_e,
+                              "samples_per_s": res["n_evals_total"] * args.evolve_steps / t_ev,
+                              "negative_cells_counted": int(negf.item()), "f_finite": bool(torch.isfinite(fe).all())}
         if not args.no_cpu_baseline and world == 1:          # rank 0 at N = 1 only
             cb = oracle_leg(w, args.cpu_seconds)
             cb.pop("seconds")
