@@ -168,8 +168,8 @@ class Oracle:
             self.roles.append(dict(s=tuple(s4), kind=kind.value, sym=sym.value, process=proc.value))
 
     def __del__(self):
-        if getattr(self, "_h", None):
-            lib().orc_destroy(self._h)
+        if getattr(self, "_h", None) and _lib is not None:      # at interpreter shutdown the module globals may be gone
+            _lib.orc_destroy(self._h)
             self._h = None
 
     def _cb(self, fcb):
