@@ -27,6 +27,12 @@ namespace rbg {
 #define RBG_CHECK_STAGE(fs, src, n) ((void)0)
 #endif
 
+// Momentum of a cell centre exactly as the host tables (1/E_p, v = p / E_p: rbg.cu) and the oracle compute it,
+// pmin + (i + 1/2) delta in two roundings (this file is compiled with -fmad=false).  A fused form differs by an ulp, which
+// is harmless everywhere except at a centre that is zero up to rounding: there a massless species has E_p ~ 1e-16 and
+// v = p / E_p depends on that ulp, so the kernels must use the very p that went into the tables.
+__device__ __forceinline__ double cell_centre(int i, double delta, double pmin) { return pmin + ((double)i + 0.5) * delta; }
+
 enum { N_MOMENTS = 14 };   // n, jx, jy, jz, T00, T01, T02, T03, T11, T12, T13, T22, T23, T33
 
 struct SpeciesTables {
@@ -119,7 +125,7 @@ moments_kernel(const double* __restrict__ f_species, SpeciesTables tb, int nx_ce
         fence_mbar_init();
         for (int k = 0; k < n_stages; ++k) arm(k, blockIdx.x + k * gridDim.x);          // prologue: fill the ring
     }
-    for (int i = threadIdx.x; i < tb.n[0]; i += MOM_THREADS) px_tab[i] = fma((double)i + 0.5, tb.delta[0], tb.pmin[0]);
+    for (int i = threadIdx.x; i < tb.n[0]; i += MOM_THREADS) px_tab[i] = cell_centre(i, tb.delta[0], tb.pmin[0]);
     if (IE_SMEM) {
         double* dst = reinterpret_cast<double*>(mom_smem + head);
         for (size_t j = threadIdx.x; j < np; j += MOM_THREADS) dst[j] = __ldg(tb.iE + j);
@@ -198,8 +204,8 @@ moments_kernel(const double* __restrict__ f_species, SpeciesTables tb, int nx_ce
                     const int c = c0 + q * team;
                     if (c < nyz) {
                         const int iy = c / tb.n[2], iz = c - iy * tb.n[2];
-                        const double py = fma((double)iy + 0.5, tb.delta[1], tb.pmin[1]);
-                        const double pz = fma((double)iz + 0.5, tb.delta[2], tb.pmin[2]);
+                        const double py = cell_centre(iy, tb.delta[1], tb.pmin[1]);
+                        const double pz = cell_centre(iz, tb.delta[2], tb.pmin[2]);
                         const double r = fma(py, py, fma(pz, pz, msq));                   // q - px^2
                         const double yG0 = py * G0[q], zG0 = pz * G0[q];
                         acc[0] += X0[q];                                                  // n
@@ -322,7 +328,7 @@ moments_sym_kernel(const double* __restrict__ f_species, SpeciesTables tb, int n
     // rows 0 .. c0-1 of the octant table: the planes above the centre (pair j = planes c0 + odd0 + j and c0 - 1 - j);
     // row c0 (odd n only): the centre plane p_x = 0.  Likewise in y and z.
     for (int i = threadIdx.x; i < c0; i += MS_THREADS) {
-        const double px = fma((double)(c0 + odd0 + i) + 0.5, tb.delta[0], tb.pmin[0]);
+        const double px = cell_centre((c0 + odd0 + i), tb.delta[0], tb.pmin[0]);
         pxs[i] = px; px2s[i] = px * px;
     }
     for (int i = threadIdx.x; i < n0h * nyzh; i += MS_THREADS) {
@@ -341,8 +347,8 @@ moments_sym_kernel(const double* __restrict__ f_species, SpeciesTables tb, int n
         valid[q] = c < nyz;
         col[q] = valid[q] ? c : nyz - 1;                                  // an idle slot reads a valid column and is discarded
         const int iy = col[q] / tb.n[2], iz = col[q] - iy * tb.n[2];
-        py[q] = fma((double)iy + 0.5, tb.delta[1], tb.pmin[1]);
-        pz[q] = fma((double)iz + 0.5, tb.delta[2], tb.pmin[2]);
+        py[q] = cell_centre(iy, tb.delta[1], tb.pmin[1]);
+        pz[q] = cell_centre(iz, tb.delta[2], tb.pmin[2]);
         rr[q] = fma(py[q], py[q], fma(pz[q], pz[q], msq));               // E^2 - p_x^2
         const int m1 = iy >= c1 + odd1 ? iy - c1 - odd1 : (iy < c1 ? c1 - 1 - iy : c1);
         const int m2 = iz >= c2 + odd2 ? iz - c2 - odd2 : (iz < c2 ? c2 - 1 - iz : c2);
@@ -685,7 +691,7 @@ vlasov_upfd_kernel(const double* __restrict__ f_species, double* __restrict__ ou
         fence_mbar_init();
         for (int k = 0; k < n_stages; ++k) arm(k, blockIdx.x + k * gridDim.x);
     }
-    for (int i = threadIdx.x; i < n0; i += MOM_THREADS) px_tab[i] = fma((double)i + 0.5, tb.delta[0], tb.pmin[0]);
+    for (int i = threadIdx.x; i < n0; i += MOM_THREADS) px_tab[i] = cell_centre(i, tb.delta[0], tb.pmin[0]);
     for (size_t j = threadIdx.x; j < np; j += MOM_THREADS) iEs[j] = __ldg(tb.iE + j);
     __syncthreads();
     const double k0 = vp.dt / tb.delta[0], k1 = vp.dt / tb.delta[1], k2 = vp.dt / tb.delta[2];
@@ -722,8 +728,8 @@ vlasov_upfd_kernel(const double* __restrict__ f_species, double* __restrict__ ou
                     const int c = c0 + q * team;
                     if (c < nyz) {
                         const int iy = c / n2, iz = c - iy * n2;
-                        const double py = fma((double)iy + 0.5, tb.delta[1], tb.pmin[1]);
-                        const double pz = fma((double)iz + 0.5, tb.delta[2], tb.pmin[2]);
+                        const double py = cell_centre(iy, tb.delta[1], tb.pmin[1]);
+                        const double pz = cell_centre(iz, tb.delta[2], tb.pmin[2]);
                         // periodic momentum neighbours of the column
                         const int cym = iy > 0 ? c - n2 : c + (n1 - 1) * n2, cyp = iy < n1 - 1 ? c + n2 : c - (n1 - 1) * n2;
                         const int czm = iz > 0 ? c - 1 : c + n2 - 1, czp = iz < n2 - 1 ? c + 1 : c - (n2 - 1);
@@ -819,7 +825,7 @@ vlasov_sym_kernel(const double* __restrict__ f_species, double* __restrict__ out
     // y and z (as in moments_sym_kernel)
     for (int i = threadIdx.x; i < n0; i += blockDim.x) {
         const int mi = i >= c0 + odd0 ? i - c0 - odd0 : (i < c0 ? c0 - 1 - i : c0);
-        xtab[i].px = fma((double)i + 0.5, tb.delta[0], tb.pmin[0]);
+        xtab[i].px = cell_centre(i, tb.delta[0], tb.pmin[0]);
         xtab[i].erow = mi * nyzh * 8;
         xtab[i].pad = 0;
     }
@@ -833,8 +839,8 @@ vlasov_sym_kernel(const double* __restrict__ f_species, double* __restrict__ out
     const bool active = seg < segs;
     const int i_lo = min(seg * seg_len, n0), i_hi = active ? min(i_lo + seg_len, n0) : i_lo;
     const int iy = c / n2, iz = c - iy * n2;
-    const double py = fma((double)iy + 0.5, tb.delta[1], tb.pmin[1]);
-    const double pz = fma((double)iz + 0.5, tb.delta[2], tb.pmin[2]);
+    const double py = cell_centre(iy, tb.delta[1], tb.pmin[1]);
+    const double pz = cell_centre(iz, tb.delta[2], tb.pmin[2]);
     // byte offsets of the periodic p_y, p_z neighbours relative to the cell itself (the same in every plane)
     const int dym = (iy > 0 ? -n2 : (n1 - 1) * n2) * 8, dyp = (iy < n1 - 1 ? n2 : -(n1 - 1) * n2) * 8;
     const int dzm = (iz > 0 ? -1 : n2 - 1) * 8, dzp = (iz < n2 - 1 ? 1 : -(n2 - 1)) * 8;
@@ -918,12 +924,12 @@ moments_direct_kernel(const double* __restrict__ f_species, SpeciesTables tb, in
     for (int m = 0; m < N_MOMENTS; ++m) acc[m] = 0.0;
     for (int c = warp * 32 + lane; c < nyz; c += nwarps * 32) {
         const int iy = c / tb.n[2], iz = c - iy * tb.n[2];
-        const double py = fma((double)iy + 0.5, tb.delta[1], tb.pmin[1]);
-        const double pz = fma((double)iz + 0.5, tb.delta[2], tb.pmin[2]);
+        const double py = cell_centre(iy, tb.delta[1], tb.pmin[1]);
+        const double pz = cell_centre(iz, tb.delta[2], tb.pmin[2]);
         double X0 = 0.0, X1 = 0.0, G0 = 0.0, G1 = 0.0, G2 = 0.0;
 #pragma unroll 4
         for (int i = 0; i < tb.n[0]; ++i) {
-            const double px = fma((double)i + 0.5, tb.delta[0], tb.pmin[0]);
+            const double px = cell_centre(i, tb.delta[0], tb.pmin[0]);
             const size_t j = (size_t)i * nyz + c;
             const double a = __ldcs(f + j);
             const double g = a * __ldg(iE + j);
@@ -974,9 +980,9 @@ vlasov_direct_kernel(const double* __restrict__ f_species, double* __restrict__ 
     const int z_m = ip + (i2 > 0 ? -1 : tb.n[2] - 1), z_p = ip + (i2 < tb.n[2] - 1 ? 1 : -(tb.n[2] - 1));
     // the same v = p * (1/E) as the staged kernel
     const double iE = __ldg(tb.iE + ip);
-    const double vx = fma((double)i0 + 0.5, tb.delta[0], tb.pmin[0]) * iE;
-    const double vy = fma((double)i1 + 0.5, tb.delta[1], tb.pmin[1]) * iE;
-    const double vz = fma((double)i2 + 0.5, tb.delta[2], tb.pmin[2]) * iE;
+    const double vx = cell_centre(i0, tb.delta[0], tb.pmin[0]) * iE;
+    const double vy = cell_centre(i1, tb.delta[1], tb.pmin[1]) * iE;
+    const double vz = cell_centre(i2, tb.delta[2], tb.pmin[2]) * iE;
     const double k0 = vp.dt / tb.delta[0], k1 = vp.dt / tb.delta[1], k2 = vp.dt / tb.delta[2];
     const double Q = tb.charge;
     const size_t np = (size_t)tb.np;

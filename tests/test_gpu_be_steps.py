@@ -265,6 +265,30 @@ def test_be_steps_on_degenerate_momentum_grids(n, nx, asym):
     assert np.all(np.abs(D.cpu().numpy() - D_ref) <= 1e-14 * np.abs(D_ref))
 
 
+def test_be_steps_massless_species_with_a_centre_that_is_zero_only_up_to_rounding():
+    """A massless species on an odd grid whose box edges are not dyadic: the centre cell's momentum is ~1e-16, not 0, so
+    E_p ~ 1e-16 and v = p / E_p is decided by the last bit of the centre.  The kernels must form the centre exactly as the
+    1/E and v tables (and the oracle) do -- pmin + (i + 1/2) delta in two roundings; a fused form fails here."""
+    rbg = _rbg()
+    box = [1.8258518432329411, 1.966972915376824, 1.6607711616229521]
+    for n, nx in (((3, 7, 5), 7), ((5, 2, 6), 300)):                    # general kernels (odd cell count) / symmetric-grid kernels
+        prob = dict(nx=nx, species=[dict(mass=0.0, charge=-1.0, stat=0, g=1.0)],
+                    grids=[dict(n=list(n), pmin=[-b for b in box], pmax=list(box))], processes=[], hbar=1.0)
+        rng = np.random.default_rng(5)
+        f = rng.random(nx * int(np.prod(n))) + 0.05
+        E = rng.normal(size=(nx, 3)); B = rng.normal(size=(nx, 3))
+        col = rbg.Collision(prob)
+        fd = torch.from_numpy(f).cuda()
+        M, _, _ = col.moments(fd)
+        V = col.vlasov_step(fd, 0.03, torch.from_numpy(E).cuda(), torch.from_numpy(B).cuda())
+        torch.cuda.synchronize()
+        M_ref, _, _ = bs.moments(prob, f)
+        scale = np.maximum(M_ref[..., 0:1], M_ref[..., 4:5]) * 16.0
+        assert np.all(np.abs(M.cpu().numpy() - M_ref) <= 1e-12 * scale)
+        V_ref = bs.vlasov_upfd(prob, f, 0.03, E, B)
+        assert np.all(np.abs(V.cpu().numpy() - V_ref) <= 1e-14 * np.abs(V_ref))
+
+
 def test_be_steps_on_the_papers_35_cubed_grid_use_the_direct_kernels():
     """A 35^3 block (343 KB) does not fit in shared memory: moments and Vlasov fall back to their direct kernels."""
     rbg = _rbg()
