@@ -178,6 +178,45 @@ int rbg_collision_host(rbg_handle* h, const double* f_host, double* C_host, int 
 #define RBG_N_MOMENTS 14
 int rbg_moments(rbg_handle* h, const double* f_dev, double* M_dev, double* total_dev, double* em_dev, void* cuda_stream);
 
+/* The moments of ONE species without a handle and without a single device allocation by this library.
+ *
+ * Who this is for.  Everything else in this header goes through rbg_create, which calls cudaMalloc for its per-species
+ * tables.  Some programs cannot do that at the point where they need the moments: a solver that has handed all of HBM to
+ * its own pool at start-up (a further cudaMalloc then fails, or takes memory the pool believed it had), a time-step loop
+ * that must not stall (cudaMalloc / cudaFree synchronise the whole device), or a plug-in running inside a host
+ * application that forbids device allocations after initialisation.  Such a caller already owns f and a place for the
+ * result; the only other memory the kernel needs is the species' 1/E_p table (8 bytes per momentum cell), and here that
+ * table lives in a fixed array compiled into the library (`static __device__`, RBG_MOMENTS_STATIC_MAX_CELLS doubles =
+ * 512 KB), which every GPU that loads librbg.so holds from module load until the process exits.
+ *
+ * What it computes.  The same 14 midpoint sums as rbg_moments for a species of mass `mass` on momentum grid `grid`
+ * (Eq. 5-6 and 9): f_dev is [n_cells][n0*n1*n2] doubles (one species' block of the usual layout),
+ * M_dev is [n_cells][RBG_N_MOMENTS] doubles in rbg_moments' order.  Both are device pointers on the CURRENT device,
+ * caller-owned, M_dev overwritten.  Two launches on cuda_stream (fill the table, then reduce), asynchronous.  The table
+ * holds the same bits as the one rbg_create builds, and the reduction is rbg_moments' unstaged kernel, so the result is
+ * identical to rbg_moments where that call takes its unstaged kernel and agrees with its staged kernels to rounding
+ * (a different summation order: within 1e-12 of the same sums over |f|).
+ * No species totals and no (rho, J): with one species the caller has them already (Q n, Q j).
+ *
+ * Limits and errors.  grid->n[0]*n[1]*n[2] must not exceed RBG_MOMENTS_STATIC_MAX_CELLS: a larger grid is refused with
+ * RBG_E_UNSUPPORTED and a message naming both numbers (it is never truncated).  Non-positive counts, pmax <= pmin,
+ * negative mass, n_cells < 0 or null pointers give RBG_E_INVALID_ARG; n_cells == 0 is a no-op.  The text is read with
+ * rbg_last_error(NULL).  The call makes no cudaMalloc, cudaFree, cudaMemcpy or other allocating runtime call.
+ *
+ * First call on a device.  The array's device address differs per GPU and is not known to host code until asked for, so
+ * the first call made with a given device current looks it up (cudaGetSymbolAddress, which also makes the runtime load
+ * this library's code onto that device if it has not yet) and remembers it for later calls.  Make that first call during
+ * your own set-up, outside any stream capture.
+ *
+ * Sharing.  There is one array per GPU, shared by every call from every thread, and it keeps whatever the previous call
+ * wrote.  Each call rewrites the cells it is about to read before it reads them, in stream order, so back-to-back calls on
+ * ONE stream are safe whatever their grids.  Two calls that can run on the GPU at the same time (different streams, or
+ * different host threads on different streams) race on the table unless species mass and grid are identical: order them
+ * with an event, or keep this entry point on one stream. */
+#define RBG_MOMENTS_STATIC_MAX_CELLS 65536
+int rbg_moments_static(const rbg_momentum_grid* grid, double mass, int n_cells, const double* f_dev, double* M_dev,
+                       void* cuda_stream);
+
 /* One first-order UPFD (unconditionally positivity-preserving finite difference) step of the drift term, Eq. 25 with
  * Eq. 28-30, all three directions at once (reading R23):
  *   f_out(x) = [ f/3 + dt Sum_d |v_d| f(x - sign(v_d) dx_d e_d) / dx_d ] / [ 1/3 + dt Sum_d |v_d| / dx_d ],  v = p/E_p.

@@ -10,5 +10,5 @@ from __future__ import annotations
 from .binding import (  # noqa: F401
     Collision, RbgError, KIND_CONST, KIND_COULOMB_SCREENED, KIND_TCHAN_S2, KIND_ISO_DSIGMA, KIND_QCD_Q1Q2, KIND_QCD_Q1Q1, KIND_QCD_Q1QB1,
     KIND_QCD_Q1QB1_Q2QB2, KIND_QCD_QQB_GG, KIND_QCD_QG, KIND_QCD_GG, load_library, probe_alu_peak,
-    exported_symbols, selftest_math, selfcheck_failures, use_checked_build,
+    exported_symbols, selftest_math, selfcheck_failures, use_checked_build, moments_static, MOMENTS_STATIC_MAX_CELLS,
 )

@@ -64,6 +64,7 @@ _SIGNATURES = {
                                        C.c_uint64, C.c_void_p]),
     "rbg_collision_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_uint64]),
     "rbg_moments": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "rbg_moments_static": (C.c_int, [C.POINTER(_MomentumGrid), C.c_double, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
     "rbg_drift_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "rbg_drift_step_pfl": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.POINTER(C.c_double), C.c_void_p]),
     "rbg_vlasov_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]),
@@ -142,6 +143,37 @@ def _stream_ptr(stream):
         import torch
         return C.c_void_p(torch.cuda.current_stream().cuda_stream)
     return C.c_void_p(getattr(stream, "cuda_stream", stream))
+
+
+MOMENTS_STATIC_MAX_CELLS = 65536
+
+
+def moments_static(grid: dict, mass: float, f, out=None, stream=None):
+    """rbg_moments_static: the 14 moments of one species, M[n_cells, 14], with no handle and no device allocation inside
+    the library -- for programs that cannot let a library call cudaMalloc where they need the moments (all of HBM already
+    in their own pool, a time-step loop that must not hit cudaMalloc's device-wide synchronisation, a host application
+    that forbids allocations after start-up).  The species' 1/E_p table sits in a fixed 512 KB array inside librbg.so, so
+    the momentum grid may have at most MOMENTS_STATIC_MAX_CELLS cells (larger: RbgError, nothing is truncated).
+
+    ``grid`` = dict(n, pmin, pmax); ``f`` = that species' block, a contiguous float64 CUDA tensor of n_cells * prod(n)
+    elements on the current device.  Pass ``out`` (float64 CUDA, n_cells * 14 elements) to keep this wrapper from allocating
+    as well; without it the result tensor comes from torch's allocator.  The first call on a device looks up the array's
+    address: make it before any stream capture.  Calls share the array, so keep them on one stream (include/rbg.h)."""
+    import torch
+    npc = int(np.prod(grid["n"]))
+    if not (isinstance(f, torch.Tensor) and f.is_cuda and f.dtype == torch.float64 and f.is_contiguous()
+            and npc > 0 and f.numel() % npc == 0):
+        raise RbgError("f must be a contiguous float64 CUDA tensor holding whole spatial cells of this momentum grid")
+    n_cells = f.numel() // npc
+    if out is None:
+        out = torch.empty((n_cells, N_MOMENTS), dtype=torch.float64, device=f.device)
+    elif not (isinstance(out, torch.Tensor) and out.is_cuda and out.dtype == torch.float64 and out.is_contiguous()
+              and out.numel() == n_cells * N_MOMENTS and out.device == f.device):
+        raise RbgError(f"out must be a contiguous float64 CUDA tensor with {n_cells * N_MOMENTS} elements on f's device")
+    g = _MomentumGrid((C.c_int * 3)(*grid["n"]), (C.c_double * 3)(*grid["pmin"]), (C.c_double * 3)(*grid["pmax"]))
+    _check(load_library().rbg_moments_static(C.byref(g), float(mass), int(n_cells), C.c_void_p(f.data_ptr()),
+                                             C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+    return out
 
 
 class Collision:

@@ -823,6 +823,107 @@ int rbg_moments(rbg_handle* h, const double* f_dev, double* M_dev, double* total
     return RBG_OK;
 }
 
+}  // extern "C" (re-opened below)
+
+// ---- rbg_moments_static: the moments of one species for callers that must not allocate device memory -----------------
+// Everything this entry point needs besides the caller's f and M is the species' 1/E_p table, and that lives here, in the
+// library image, instead of in a cudaMalloc'ed buffer.  Every GPU that loads the library carries these 512 KB until the
+// process exits; every call shares them.
+//
+// In host code `g_static_inv_energy` is NOT a device address: it names a host-side shadow the runtime uses as a lookup
+// key.  Handing it to a kernel would make the kernel read and write wherever that host address happens to point.  The
+// address a kernel may use is per device and comes from cudaGetSymbolAddress, asked for once per device with that device
+// current (static_table_for_current_device below).
+static __device__ __align__(256) double g_static_inv_energy[RBG_MOMENTS_STATIC_MAX_CELLS];
+
+namespace {
+
+// 1/E_p of every momentum-cell centre, the same roundings in the same order as the host loop of rbg_create (this file is
+// compiled with -fmad=false, and the double-precision sqrt and divide of the device are correctly rounded), so the table
+// holds the bits rbg_create would have uploaded.  Every entry in [0, n0 n1 n2) is overwritten: nothing is assumed about
+// what the previous call left in the array.
+__global__ void __launch_bounds__(256)
+inv_energy_fill_kernel(double* __restrict__ table, int n0, int n1, int n2, double pmin0, double pmin1, double pmin2,
+                       double delta0, double delta1, double delta2, double msq) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    const int nyz = n1 * n2;
+    if (j >= n0 * nyz) return;
+    const int i0 = j / nyz, r = j - i0 * nyz, i1 = r / n2, i2 = r - i1 * n2;
+    const double px = rbg::cell_centre(i0, delta0, pmin0);
+    const double py = rbg::cell_centre(i1, delta1, pmin1);
+    const double pz = rbg::cell_centre(i2, delta2, pmin2);
+    const double E = sqrt(((px * px + py * py) + pz * pz) + msq);
+    table[j] = E > 0.0 ? 1.0 / E : 0.0;
+}
+
+// Device address of g_static_inv_energy on the CURRENT device, looked up on the first call made with that device current
+// and remembered.  cudaGetSymbolAddress initialises the context / loads this module on the device if that has not happened
+// yet, which is why the first call belongs in the caller's set-up phase and outside any stream capture.
+enum { STATIC_MAX_DEVICES = 64 };
+std::mutex g_static_mu;
+double* g_static_table[STATIC_MAX_DEVICES] = {};
+
+int static_table_for_current_device(double** table) {
+    int dev = -1;
+    RBG_CUDA(nullptr, cudaGetDevice(&dev));
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES)
+        return fail(nullptr, RBG_E_UNSUPPORTED, "rbg_moments_static: device ordinal " + std::to_string(dev) + " is beyond the " +
+                                                std::to_string((int)STATIC_MAX_DEVICES) + " this entry point keeps an address for");
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_table[dev]) {
+        void* p = nullptr;
+        RBG_CUDA(nullptr, cudaGetSymbolAddress(&p, g_static_inv_energy));
+        if (!p) return fail(nullptr, RBG_E_CUDA, "rbg_moments_static: cudaGetSymbolAddress returned a null address");
+        g_static_table[dev] = static_cast<double*>(p);
+    }
+    *table = g_static_table[dev];
+    return RBG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int rbg_moments_static(const rbg_momentum_grid* grid, double mass, int n_cells, const double* f_dev, double* M_dev,
+                       void* cuda_stream) {
+    if (!grid || !f_dev || !M_dev) return fail(nullptr, RBG_E_INVALID_ARG, "rbg_moments_static: null argument");
+    if (!(mass >= 0.0)) return fail(nullptr, RBG_E_INVALID_ARG, "rbg_moments_static: negative mass");
+    if (n_cells < 0) return fail(nullptr, RBG_E_INVALID_ARG, "rbg_moments_static: n_cells must be >= 0");
+    double cells = 1.0;
+    for (int d = 0; d < 3; ++d) {
+        if (grid->n[d] <= 0) return fail(nullptr, RBG_E_INVALID_ARG, "rbg_moments_static: momentum grid counts must be positive");
+        if (!(grid->pmax[d] > grid->pmin[d])) return fail(nullptr, RBG_E_INVALID_ARG, "rbg_moments_static: pmax must exceed pmin");
+        cells *= (double)grid->n[d];
+    }
+    if (cells > (double)RBG_MOMENTS_STATIC_MAX_CELLS)
+        return fail(nullptr, RBG_E_UNSUPPORTED,
+                    "rbg_moments_static: the momentum grid has " + std::to_string((long long)cells) + " cells, the built-in table holds " +
+                    std::to_string((int)RBG_MOMENTS_STATIC_MAX_CELLS) +
+                    " (RBG_MOMENTS_STATIC_MAX_CELLS); larger grids need rbg_create + rbg_moments, which allocate");
+    if (n_cells == 0) return RBG_OK;
+    double* table = nullptr;
+    const int rc = static_table_for_current_device(&table);
+    if (rc != RBG_OK) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    rbg::SpeciesTables tb;
+    std::memset(&tb, 0, sizeof tb);
+    for (int d = 0; d < 3; ++d) {
+        tb.pmin[d] = grid->pmin[d];
+        tb.delta[d] = (grid->pmax[d] - grid->pmin[d]) / (double)grid->n[d];
+        tb.n[d] = grid->n[d];
+    }
+    tb.np = (int)cells;
+    tb.mass = mass;
+    tb.iE = table;                 // the device address, never the symbol
+    tb.v = nullptr;                // the moment sums do not read the velocity table
+    inv_energy_fill_kernel<<<(tb.np + 255) / 256, 256, 0, st>>>(table, tb.n[0], tb.n[1], tb.n[2], tb.pmin[0], tb.pmin[1], tb.pmin[2],
+                                                                tb.delta[0], tb.delta[1], tb.delta[2], mass * mass);
+    RBG_CUDA(nullptr, cudaGetLastError());
+    rbg::moments_direct_kernel<<<n_cells, 128, 0, st>>>(f_dev, tb, n_cells, M_dev);
+    RBG_CUDA(nullptr, cudaGetLastError());
+    return RBG_OK;
+}
+
 int rbg_drift_step(rbg_handle* h, const double* f_dev, double* f_out_dev, const rbg_drift_params* p, void* cuda_stream) {
     if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
     if (!f_dev || !f_out_dev || !p) return fail(h, RBG_E_INVALID_ARG, "null argument");
