@@ -31,8 +31,10 @@
  *   - Determinism: the result of rbg_collision / _update / _evolve / _host is a pure function of (f, the rbg_create
  *     arguments, n_samples, seed), bit for bit: it does not depend on the stream, on any rbg_set_option knob (CTA
  *     size, tile size, samples per lane, gather path) or on how spatial cells are partitioned across calls or GPUs
- *     (the sample stream is keyed by the global cell index; a lane always sums the even 32-sample blocks and the odd
- *     ones separately, in ascending order).  rbg_collision_symmetric uses atomics: reproducible to rounding only.
+ *     (the sample stream is keyed by the global cell index; lane l of the warp that owns a momentum cell adds its samples
+ *     n = l, l + 32, l + 64, ... in ascending order into ONE accumulator, whatever the samples-per-lane setting, and the 32
+ *     lane sums are then combined by a fixed xor-shuffle tree: offsets 16, 8, 4, 2, 1).  rbg_collision_symmetric uses
+ *     atomics: reproducible to rounding only.
  */
 #ifndef RBG_H_
 #define RBG_H_
@@ -265,12 +267,19 @@ int rbg_n_roles(const rbg_handle* h);
 uint64_t rbg_sample_evals(const rbg_handle* h, int n_samples);
 /* Kernels launched by the most recent rbg_collision* call on this handle. */
 int rbg_last_launch_count(const rbg_handle* h);
-/* Launch geometry / gather path knobs (results do not depend on them; 0 = automatic).  key:
- * "warps_per_cta" (1..32), "p1_per_cta" (momentum cells per CTA, >= 1), "samples_per_lane"
- * (1 or 2: samples a lane evaluates per loop iteration; CTAs of more than 12 warps -- 16 with RBG_FP32_KINEMATICS -- use 1),
- * "gather" (1 shared memory, 2 global/L2), "moments_path" / "vlasov_path" (1: rbg_moments / rbg_vlasov_step use their general staged
- * kernel even where the symmetric-grid kernel applies), "sym_tables" (1: rbg_collision_symmetric accumulates the deposits of a
- * CTA in shared-memory tables and flushes them at its end, instead of one global atomic per deposit).  Returns RBG_E_INVALID_ARG for an unknown key or value. */
+/* Launch geometry / kernel path knobs (0 = automatic).  Two groups of keys.
+ * (i) Results do NOT depend on these, bit for bit (rbg_collision / _update / _evolve / _host):
+ *   "warps_per_cta" (1..32), "p1_per_cta" (momentum cells per CTA, >= 1), "samples_per_lane" (1 or 2: samples a lane
+ *   evaluates per loop iteration; CTAs of more than 12 warps -- 16 with RBG_FP32_KINEMATICS -- use 1), "gather" (1 shared
+ *   memory, 2 global/L2).
+ * (ii) These select a kernel with different arithmetic, so results agree with the other setting (and with the oracle) to
+ *   rounding only, and are bit-identical only for a fixed setting:
+ *   "moments_path" / "vlasov_path" (1: rbg_moments / rbg_vlasov_step use their general staged kernel even where the
+ *   symmetric-grid kernel applies; the symmetric-grid kernels read a 1/E table of one octant, pair the cells at +p and -p
+ *   before multiplying, and pre-scale the fields: moments within 1e-12 of the sums over |f|, a Vlasov step within 1e-14
+ *   relative), "sym_tables" (1: rbg_collision_symmetric accumulates the deposits of a CTA in shared-memory tables and
+ *   flushes them at its end, instead of one global atomic per deposit: another order of atomic additions).
+ * Returns RBG_E_INVALID_ARG for an unknown key or value. */
 int rbg_set_option(rbg_handle* h, const char* key, int value);
 /* Text of the last error on this handle (or of the last failed rbg_create if h is NULL). */
 const char* rbg_last_error(const rbg_handle* h);

@@ -43,7 +43,7 @@ def collision_cases():
             ("collision: fp32 kinematics, cooperative float staging", 2, dict(nx=2, np_side=8, n_samples=40), True, ()),
             ("collision: quantum statistics, t-channel kind, 5 species", 3, dict(nx=1, np_side=6, n_samples=32), False, ()),
             ("collision: Table III kinds with inelastic roles (three tables)", 7, dict(nx=2, np_side=4, n_samples=16), False, ()),
-            ("collision: 2 samples per lane, 16 warps", 4, dict(nx=2, np_side=8, n_samples=70), False, (("samples_per_lane", 2),)),
+            ("collision: 2 samples per lane, 12 warps", 4, dict(nx=2, np_side=8, n_samples=70), False, (("samples_per_lane", 2),)),
             ("collision: 1 sample per lane, 32 warps", 4, dict(nx=2, np_side=8, n_samples=70), False, (("warps_per_cta", 32),)),
             ("collision: t-channel importance sampler", 2, dict(nx=2, np_side=8, n_samples=40, sampler=1), False, ())):
         w = workloads.make(cfg, **kw)
