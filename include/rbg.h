@@ -25,6 +25,8 @@
  *     the work queued on `cuda_stream` has completed.  The handle owns only its own scratch.
  *   - Calls that take a stream are asynchronous on that stream (a cudaStream_t passed as void*;
  *     NULL = the legacy default stream).  rbg_collision_host is synchronous.
+ *   - Overlap: an output buffer must not share a byte with the f it is computed from (every kernel reads f at cells other
+ *     than the one it writes); all entry points compare the byte ranges and return RBG_E_INVALID_ARG on any overlap.
  *   - Errors: every int-returning entry point returns RBG_OK (0) or a negative RBG_E_* code; the
  *     text is available from rbg_last_error().  No exception crosses this boundary.  There is no
  *     CPU fallback: anything the CUDA path does not support is an error, never a slow path.
@@ -139,7 +141,7 @@ int rbg_collision(rbg_handle* h, const double* f_dev, double* C_dev, int n_sampl
  * splitting reads (1/3) df/dt = C, so a caller reproducing it passes 3 * (the time step), as
  * rbg_be_step does; the same holds for rbg_collision_evolve.  *neg_flag_dev (one int in device memory, zeroed by the
  * caller) is incremented by the number of cells with f_out < 0; f_out is stored unclamped (policy is the caller's).
- * f_out_dev must not alias f_dev. */
+ * f_out_dev must not overlap f_dev, not even partly (RBG_E_INVALID_ARG). */
 int rbg_collision_update(rbg_handle* h, const double* f_dev, double* f_out_dev, double dt, int* neg_flag_dev,
                          int n_samples, uint64_t seed, void* cuda_stream);
 
@@ -225,7 +227,7 @@ int rbg_moments_static(const rbg_momentum_grid* grid, double mass, int n_cells, 
  * The spatial grid is the (nx, ny, nz) of rbg_create, ix = (i_x ny + i_y) nz + i_z.  bc[d]: 1 periodic, 0 wall; a wall
  * reflects with probability zeta in [0,1]: the value beyond it is zeta * f(wall cell, p_d -> -p_d),
  * which needs momentum grids symmetric about 0 when zeta != 0 (else RBG_E_UNSUPPORTED); zeta = 0 absorbs.
- * f_out_dev must not alias f_dev.  Needs the whole spatial domain in this handle (ix_offset == 0): across GPUs the
+ * f_out_dev must not overlap f_dev, not even partly (RBG_E_INVALID_ARG).  Needs the whole spatial domain in this handle (ix_offset == 0): across GPUs the
  * stencil would need the paper's ghost-layer exchange, which is out of scope. */
 typedef struct { double dt; double dx[3]; int bc[3]; double zeta; } rbg_drift_params;
 int rbg_drift_step(rbg_handle* h, const double* f_dev, double* f_out_dev, const rbg_drift_params* p, void* cuda_stream);
@@ -240,7 +242,7 @@ int rbg_drift_step_pfl(rbg_handle* h, const double* f_dev, double* f_out_dev, do
 /* One first-order UPFD step of the Vlasov term, Eq. 26 with Eq. 34, all three directions at once:
  *   f_out(p) = [ f/3 + dt Sum_d |F_d| f(p - sign(F_d) dp_d e_d) / dp_d ] / [ 1/3 + dt Sum_d |F_d| / dp_d ],
  * F = Q (E + v x B) with the species' charge and the fields of the spatial cell, E_dev and B_dev being
- * [Nx][3] doubles; periodic in every momentum direction.  f_out_dev must not alias f_dev. */
+ * [Nx][3] doubles; periodic in every momentum direction.  f_out_dev must not overlap f_dev, not even partly (RBG_E_INVALID_ARG). */
 int rbg_vlasov_step(rbg_handle* h, const double* f_dev, double* f_out_dev, double dt, const double* E_dev,
                     const double* B_dev, void* cuda_stream);
 

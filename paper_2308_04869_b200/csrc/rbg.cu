@@ -5,9 +5,11 @@
 // marshals.  Shares no code with oracle/.
 #include "../../include/rbg.h"
 
+#include <array>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <map>
 #include <mutex>
 #include <set>
 #include <type_traits>
@@ -54,6 +56,7 @@ struct rbg_handle {
     // options
     int opt_warps = 0, opt_p1_per_cta = 0, opt_gather = 0, opt_spl = 0, opt_moments_path = 0, opt_vlasov_path = 0, opt_sym_tables = 0;
     int last_launches = 0;
+    std::map<std::array<int, 4>, int> tile_cache;      // tile size chosen by run_roles per (role, cells, n_samples, warps)
     // per-species device tables for the moment / drift / Vlasov kernels: 1/E_p and v = p/E_p per momentum cell
     std::vector<double*> tab_iE, tab_v;
     double* charges_dev = nullptr;
@@ -72,6 +75,13 @@ namespace {
 int fail(rbg_handle* h, int code, const std::string& msg) {
     if (h) h->err = msg; else g_create_error = msg;
     return code;
+}
+
+// Do the byte ranges [a, a + na) and [b, b + nb) share a byte?  Every kernel here reads f at cells other than the one it
+// writes (gathers, stencil neighbours), so an output that overlaps the input even partly would be read half-updated.
+bool ranges_overlap(const void* a, size_t na, const void* b, size_t nb) {
+    const uintptr_t pa = reinterpret_cast<uintptr_t>(a), pb = reinterpret_cast<uintptr_t>(b);
+    return pa < pb + nb && pb < pa + na;
 }
 
 // Makes the handle's device current for the duration of an entry point and restores the caller's on every exit path.
@@ -246,7 +256,12 @@ int run_roles(rbg_handle* h, const double* f, double* out, bool update, double d
         // 100 GB/s) and then takes ceil(T / warps) rounds of one p1 per warp (a round of n_samples samples per warp at
         // about 5.7e8 samples/s per SM); the grid of nx * tiles CTAs runs in ceil(nx * tiles / SMs) waves.  Take the
         // tiling with the smallest waves * (rounds + staging), preferring larger tiles on near-ties.  T <= 512.
+        // The search takes up to 4096 candidates with several 64-bit divisions each, and its inputs never change inside a
+        // time-step loop (rbg_collision_evolve), so its result is kept per (role, cells in the sweep, n_samples, warps).
         int T = h->opt_p1_per_cta;
+        const std::array<int, 4> tile_key{(int)ir, ncell, n_samples, warps};
+        const auto cached = T <= 0 ? h->tile_cache.find(tile_key) : h->tile_cache.end();
+        if (cached != h->tile_cache.end()) T = cached->second;
         if (T <= 0) {
             size_t tab_bytes = 0;
             for (int i = 1; i < 4; ++i) {
@@ -263,6 +278,7 @@ int run_roles(rbg_handle* h, const double* f, double* out, bool update, double d
                 const double cost = (double)((ctas + h->sm_count - 1) / h->sm_count) * ((double)((Tt + warps - 1) / warps) + staging);
                 if (best_cost < 0.0 || cost < 0.995 * best_cost) { best_cost = cost; T = Tt; }
             }
+            h->tile_cache[tile_key] = T;
         }
         T = std::max(1, std::min(T, np1));
         // shared memory: [16 B mbarrier][T doubles][one f table per distinct species among slots 2, 3, 4, 16-B aligned]
@@ -327,7 +343,8 @@ int run(rbg_handle* h, const double* f, double* out, bool update, double dt, int
         void* stream) {
     if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
     if (!f || !out) return fail(h, RBG_E_INVALID_ARG, "null buffer");
-    if (f == out) return fail(h, RBG_E_INVALID_ARG, "output must not alias f");
+    if (ranges_overlap(f, h->f_elems * sizeof(double), out, h->f_elems * sizeof(double)))
+        return fail(h, RBG_E_INVALID_ARG, "the output buffer overlaps f (the kernels gather f at other cells while they write)");
     if (n_samples <= 0) return fail(h, RBG_E_INVALID_ARG, "n_samples must be positive");
     if (update && !neg_flag) return fail(h, RBG_E_INVALID_ARG, "null neg_flag_dev");
     cudaStream_t st = (cudaStream_t)stream;
@@ -514,7 +531,8 @@ int rbg_collision_update(rbg_handle* h, const double* f_dev, double* f_out_dev, 
 int rbg_collision_symmetric(rbg_handle* h, const double* f_dev, double* C_dev, int n_samples, uint64_t seed, void* cuda_stream) {
     if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
     if (!f_dev || !C_dev) return fail(h, RBG_E_INVALID_ARG, "null buffer");
-    if (f_dev == C_dev) return fail(h, RBG_E_INVALID_ARG, "output must not alias f");
+    if (ranges_overlap(f_dev, h->f_elems * sizeof(double), C_dev, h->f_elems * sizeof(double)))
+        return fail(h, RBG_E_INVALID_ARG, "C_dev overlaps f_dev (the kernels gather f at other cells while they deposit)");
     if (n_samples <= 0) return fail(h, RBG_E_INVALID_ARG, "n_samples must be positive");
     if (h->flags & RBG_FP32_KINEMATICS) return fail(h, RBG_E_UNSUPPORTED, "rbg_collision_symmetric is fp64 only");
     for (const Role& r : h->roles)
@@ -596,8 +614,7 @@ int rbg_collision_evolve(rbg_handle* h, double* f_dev, double* scratch_dev, doub
     if (n_steps < 0) return fail(h, RBG_E_INVALID_ARG, "n_steps must be >= 0");
     if (!f_dev || !scratch_dev) return fail(h, RBG_E_INVALID_ARG, "null buffer");
     const size_t bytes = h->f_elems * sizeof(double);
-    const char *a = (const char*)f_dev, *b = (const char*)scratch_dev;
-    if (a < b + bytes && b < a + bytes) return fail(h, RBG_E_INVALID_ARG, "scratch_dev overlaps f_dev");
+    if (ranges_overlap(f_dev, bytes, scratch_dev, bytes)) return fail(h, RBG_E_INVALID_ARG, "scratch_dev overlaps f_dev");
     DeviceGuard guard(h->device);
     double *cur = f_dev, *nxt = scratch_dev;
     int launches = 0;
@@ -615,6 +632,8 @@ int rbg_collision_evolve(rbg_handle* h, double* f_dev, double* scratch_dev, doub
 int rbg_collision_host(rbg_handle* h, const double* f_host, double* C_host, int n_samples, uint64_t seed) {
     if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
     if (!f_host || !C_host) return fail(h, RBG_E_INVALID_ARG, "null buffer");
+    if (ranges_overlap(f_host, h->f_elems * sizeof(double), C_host, h->f_elems * sizeof(double)))
+        return fail(h, RBG_E_INVALID_ARG, "C_host overlaps f_host (chunks of C are copied out while later chunks of f are still being read)");
     if (n_samples <= 0) return fail(h, RBG_E_INVALID_ARG, "n_samples must be positive");
     DeviceGuard guard(h->device);
     if (h->scratch_elems < h->f_elems) {
@@ -635,27 +654,34 @@ int rbg_collision_host(rbg_handle* h, const double* f_host, double* C_host, int 
     chunks = std::min(chunks, h->nx);
     cudaStream_t s_in = h->host_streams[0], s_k = h->host_streams[1], s_out = h->host_streams[2];
     const bool fp32 = (h->flags & RBG_FP32_KINEMATICS) != 0;
-    for (int c = 0; c < chunks; ++c) {
-        const int x0 = (int)((long)h->nx * c / chunks), x1 = (int)((long)h->nx * (c + 1) / chunks);
-        for (int s = 0; s < h->n_species; ++s) {
-            const size_t o = h->sp_off[s] + (size_t)x0 * h->np[s], n = (size_t)(x1 - x0) * h->np[s];
-            RBG_CUDA(h, cudaMemcpyAsync(h->scratch_f + o, f_host + o, n * sizeof(double), cudaMemcpyHostToDevice, s_in));
+    // The pipeline queues copies into and out of the CALLER's host buffers on three streams.  Whatever happens, this call
+    // returns only after all three have drained: after an error return the caller may free or reuse f_host / C_host at
+    // once, and no DMA may still be running on them then.
+    auto pipeline = [&]() -> int {
+        for (int c = 0; c < chunks; ++c) {
+            const int x0 = (int)((long)h->nx * c / chunks), x1 = (int)((long)h->nx * (c + 1) / chunks);
+            for (int s = 0; s < h->n_species; ++s) {
+                const size_t o = h->sp_off[s] + (size_t)x0 * h->np[s], n = (size_t)(x1 - x0) * h->np[s];
+                RBG_CUDA(h, cudaMemcpyAsync(h->scratch_f + o, f_host + o, n * sizeof(double), cudaMemcpyHostToDevice, s_in));
+            }
+            RBG_CUDA(h, cudaEventRecord(h->host_events[2 * c], s_in));
+            RBG_CUDA(h, cudaStreamWaitEvent(s_k, h->host_events[2 * c], 0));
+            const int rc = fp32 ? run_roles<float>(h, h->scratch_f, h->scratch_c, false, 0.0, nullptr, n_samples, seed, s_k, x0, x1 - x0)
+                                : run_roles<double>(h, h->scratch_f, h->scratch_c, false, 0.0, nullptr, n_samples, seed, s_k, x0, x1 - x0);
+            if (rc != RBG_OK) return rc;
+            RBG_CUDA(h, cudaEventRecord(h->host_events[2 * c + 1], s_k));
+            RBG_CUDA(h, cudaStreamWaitEvent(s_out, h->host_events[2 * c + 1], 0));
+            for (int s = 0; s < h->n_species; ++s) {
+                const size_t o = h->sp_off[s] + (size_t)x0 * h->np[s], n = (size_t)(x1 - x0) * h->np[s];
+                RBG_CUDA(h, cudaMemcpyAsync(C_host + o, h->scratch_c + o, n * sizeof(double), cudaMemcpyDeviceToHost, s_out));
+            }
         }
-        RBG_CUDA(h, cudaEventRecord(h->host_events[2 * c], s_in));
-        RBG_CUDA(h, cudaStreamWaitEvent(s_k, h->host_events[2 * c], 0));
-        const int rc = fp32 ? run_roles<float>(h, h->scratch_f, h->scratch_c, false, 0.0, nullptr, n_samples, seed, s_k, x0, x1 - x0)
-                            : run_roles<double>(h, h->scratch_f, h->scratch_c, false, 0.0, nullptr, n_samples, seed, s_k, x0, x1 - x0);
-        if (rc != RBG_OK) { cudaDeviceSynchronize(); return rc; }
-        RBG_CUDA(h, cudaEventRecord(h->host_events[2 * c + 1], s_k));
-        RBG_CUDA(h, cudaStreamWaitEvent(s_out, h->host_events[2 * c + 1], 0));
-        for (int s = 0; s < h->n_species; ++s) {
-            const size_t o = h->sp_off[s] + (size_t)x0 * h->np[s], n = (size_t)(x1 - x0) * h->np[s];
-            RBG_CUDA(h, cudaMemcpyAsync(C_host + o, h->scratch_c + o, n * sizeof(double), cudaMemcpyDeviceToHost, s_out));
-        }
-    }
-    RBG_CUDA(h, cudaStreamSynchronize(s_out));
-    RBG_CUDA(h, cudaStreamSynchronize(s_k));
-    RBG_CUDA(h, cudaStreamSynchronize(s_in));
+        return RBG_OK;
+    };
+    const int rc = pipeline();
+    const cudaError_t d_out = cudaStreamSynchronize(s_out), d_k = cudaStreamSynchronize(s_k), d_in = cudaStreamSynchronize(s_in);
+    if (rc != RBG_OK) return rc;                       // the pipeline's own message stands
+    RBG_CUDA(h, d_out); RBG_CUDA(h, d_k); RBG_CUDA(h, d_in);
     return RBG_OK;
 }
 
@@ -755,6 +781,12 @@ StagedGeometry staged_geometry(const rbg_handle* h, int s, const double* fs, siz
 int rbg_moments(rbg_handle* h, const double* f_dev, double* M_dev, double* total_dev, double* em_dev, void* cuda_stream) {
     if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
     if (!f_dev || !M_dev) return fail(h, RBG_E_INVALID_ARG, "null buffer");
+    {
+        const size_t fb = h->f_elems * sizeof(double), cellb = (size_t)h->nx * rbg::N_MOMENTS * sizeof(double);
+        if (ranges_overlap(f_dev, fb, M_dev, (size_t)h->n_species * cellb) || (total_dev && ranges_overlap(f_dev, fb, total_dev, cellb)) ||
+            (em_dev && ranges_overlap(f_dev, fb, em_dev, (size_t)h->nx * 4 * sizeof(double))))
+            return fail(h, RBG_E_INVALID_ARG, "an output buffer of rbg_moments overlaps f_dev");
+    }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     DeviceGuard guard(h->device);
     h->last_launches = 0;
@@ -901,6 +933,8 @@ int rbg_moments_static(const rbg_momentum_grid* grid, double mass, int n_cells, 
                     std::to_string((int)RBG_MOMENTS_STATIC_MAX_CELLS) +
                     " (RBG_MOMENTS_STATIC_MAX_CELLS); larger grids need rbg_create + rbg_moments, which allocate");
     if (n_cells == 0) return RBG_OK;
+    if (ranges_overlap(f_dev, (size_t)n_cells * (size_t)cells * sizeof(double), M_dev, (size_t)n_cells * rbg::N_MOMENTS * sizeof(double)))
+        return fail(nullptr, RBG_E_INVALID_ARG, "rbg_moments_static: M_dev overlaps f_dev");
     double* table = nullptr;
     const int rc = static_table_for_current_device(&table);
     if (rc != RBG_OK) return rc;
@@ -927,7 +961,8 @@ int rbg_moments_static(const rbg_momentum_grid* grid, double mass, int n_cells, 
 int rbg_drift_step(rbg_handle* h, const double* f_dev, double* f_out_dev, const rbg_drift_params* p, void* cuda_stream) {
     if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
     if (!f_dev || !f_out_dev || !p) return fail(h, RBG_E_INVALID_ARG, "null argument");
-    if (f_dev == f_out_dev) return fail(h, RBG_E_INVALID_ARG, "output must not alias f (the stencil reads neighbours)");
+    if (ranges_overlap(f_dev, h->f_elems * sizeof(double), f_out_dev, h->f_elems * sizeof(double)))
+        return fail(h, RBG_E_INVALID_ARG, "f_out_dev overlaps f_dev (the stencil reads neighbours)");
     if (!(p->dt >= 0.0)) return fail(h, RBG_E_INVALID_ARG, "dt must be >= 0");
     if (h->ix_offset != 0) return fail(h, RBG_E_UNSUPPORTED, "the drift stencil needs the whole spatial domain on one GPU (no ghost-layer exchange)");
     rbg::DriftParams dp;
@@ -963,7 +998,8 @@ int rbg_drift_step(rbg_handle* h, const double* f_dev, double* f_out_dev, const 
 int rbg_drift_step_pfl(rbg_handle* h, const double* f_dev, double* f_out_dev, double dt, const double* dx, void* cuda_stream) {
     if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
     if (!f_dev || !f_out_dev || !dx) return fail(h, RBG_E_INVALID_ARG, "null argument");
-    if (f_dev == f_out_dev) return fail(h, RBG_E_INVALID_ARG, "output must not alias f (the stencil reads neighbours)");
+    if (ranges_overlap(f_dev, h->f_elems * sizeof(double), f_out_dev, h->f_elems * sizeof(double)))
+        return fail(h, RBG_E_INVALID_ARG, "f_out_dev overlaps f_dev (the stencil reads neighbours)");
     if (!(dt >= 0.0)) return fail(h, RBG_E_INVALID_ARG, "dt must be >= 0");
     if (h->ix_offset != 0) return fail(h, RBG_E_UNSUPPORTED, "the drift stencil needs the whole spatial domain on one GPU (no ghost-layer exchange)");
     rbg::DriftParams dp;
@@ -993,7 +1029,8 @@ int rbg_vlasov_step(rbg_handle* h, const double* f_dev, double* f_out_dev, doubl
                     void* cuda_stream) {
     if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
     if (!f_dev || !f_out_dev || !E_dev || !B_dev) return fail(h, RBG_E_INVALID_ARG, "null buffer");
-    if (f_dev == f_out_dev) return fail(h, RBG_E_INVALID_ARG, "output must not alias f (the stencil reads neighbours)");
+    if (ranges_overlap(f_dev, h->f_elems * sizeof(double), f_out_dev, h->f_elems * sizeof(double)))
+        return fail(h, RBG_E_INVALID_ARG, "f_out_dev overlaps f_dev (the stencil reads neighbours)");
     if (!(dt >= 0.0)) return fail(h, RBG_E_INVALID_ARG, "dt must be >= 0");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     DeviceGuard guard(h->device);
@@ -1059,8 +1096,7 @@ int rbg_be_step(rbg_handle* h, double* f_dev, double* scratch_dev, const rbg_be_
     if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
     if (!f_dev || !scratch_dev || !p) return fail(h, RBG_E_INVALID_ARG, "null argument");
     const size_t bytes = h->f_elems * sizeof(double);
-    const char *a = (const char*)f_dev, *b = (const char*)scratch_dev;
-    if (a < b + bytes && b < a + bytes) return fail(h, RBG_E_INVALID_ARG, "scratch_dev overlaps f_dev");
+    if (ranges_overlap(f_dev, bytes, scratch_dev, bytes)) return fail(h, RBG_E_INVALID_ARG, "scratch_dev overlaps f_dev");
     if (p->do_vlasov && (!E_dev || !B_dev)) return fail(h, RBG_E_INVALID_ARG, "do_vlasov needs E_dev and B_dev");
     if (p->do_collision && !neg_flag_dev) return fail(h, RBG_E_INVALID_ARG, "do_collision needs neg_flag_dev");
     // everything the sub-steps would refuse is refused here, before the first launch touches f_dev

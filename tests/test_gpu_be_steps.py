@@ -112,6 +112,16 @@ def test_be_step_argument_errors():
     f = torch.from_numpy(w["f"]).cuda()
     with pytest.raises(rbg.RbgError):
         col.drift_step(f, 0.1, (1.0, 1.0, 1.0), out=f)               # aliasing
+    # partial overlap: the output starts one element before the end of f
+    n = col.f_elems
+    buf = torch.zeros(2 * n, dtype=torch.float64, device="cuda")
+    buf[:n] = f
+    EB = torch.zeros((1, 3), dtype=torch.float64, device="cuda")
+    for call in (lambda: col.drift_step(buf[:n], 0.1, (1.0, 1.0, 1.0), out=buf[n - 1:2 * n - 1]),
+                 lambda: col.drift_step_pfl(buf[:n], 0.1, (1.0, 1.0, 1.0), out=buf[n - 1:2 * n - 1]),
+                 lambda: col.vlasov_step(buf[:n], 0.1, EB, EB, out=buf[1:n + 1])):
+        with pytest.raises(rbg.RbgError, match="overlaps"):
+            call()
     with pytest.raises(rbg.RbgError):
         col.drift_step(f, 0.1, (0.0, 1.0, 1.0))                      # dx = 0
     with pytest.raises(rbg.RbgError):

@@ -182,6 +182,30 @@ def test_fused_update_and_negativity_flag():
         col.collision_update(f, 1e-3, 8, 1, out=f)          # f_out must not alias f
 
 
+def test_outputs_that_overlap_f_partly_are_refused():
+    """include/rbg.h, "Overlap": the byte ranges are compared, so an output that starts inside f (or ends inside it) is an
+    error just like out == f; buffers that merely touch are fine."""
+    rbg = _rbg()
+    w = workloads.make(1, nx=2, np_side=6, n_samples=8)
+    col = rbg.Collision(w["problem"])
+    n = col.f_elems
+    buf = torch.zeros(3 * n, dtype=torch.float64, device="cuda")
+    buf[n:2 * n] = torch.from_numpy(w["f"]).cuda()
+    f = buf[n:2 * n]
+    for lo in (n - 1, n + 1, 1, 2 * n - 1):                 # ends one element inside f / starts one element inside f / ...
+        out = buf[lo:lo + n]
+        for call in (lambda: col.collision(f, 8, 1, out=out), lambda: col.collision_update(f, 1e-3, 8, 1, out=out),
+                     lambda: col.collision_symmetric(f, 8, 1, out=out), lambda: col.collision_evolve(f, 1e-3, 1, 8, 1, scratch=out)):
+            with pytest.raises(rbg.RbgError, match="overlaps"):
+                call()
+    ref = col.collision(f, 8, 1).clone()
+    for lo in (0, 2 * n):                                   # adjacent, not overlapping
+        assert torch.equal(col.collision(f, 8, 1, out=buf[lo:lo + n]), ref)
+    host = np.zeros(2 * n)
+    with pytest.raises(rbg.RbgError, match="overlaps"):
+        col.collision_host(host[:n], 8, 1, out=host[n - 1:2 * n - 1])
+
+
 def test_host_entry_point_matches_device_entry_point():
     w = workloads.make(1, nx=2, np_side=8, n_samples=64)
     C_dev, col = gpu_C(w["problem"], w["f"], w["n_samples"], w["seed"])
