@@ -40,6 +40,8 @@
 #include <limits>
 #include <string>
 #include <type_traits>
+#include <map>
+#include <utility>
 #include <vector>
 #ifdef _OPENMP
 #include <omp.h>
@@ -695,16 +697,29 @@ void* orc_create(int nx, int n_species, const Species* sp, const Grid* grid, int
         Role r; r.kind = p.kind; std::memcpy(r.par, p.par, sizeof r.par); r.process = i; r.sampler = p.sampler;
         r.gab = sp[p.a].g * sp[p.b].g;
         r.sym_override = p.sym;
-        auto add = [&](int s1, int s2, int s3, int s4) {
-            r.s[0] = s1; r.s[1] = s2; r.s[2] = s3; r.s[3] = s4;
-            r.sym = p.sym < 0 ? (s3 == s4 ? 0.5 : 1.0) : p.sym;
-            H->roles.push_back(r); H->role_off.push_back(roff); roff += (size_t)nx * H->np[s1];
-        };
-        add(p.a, p.b, p.c, p.d);
-        if (p.b != p.a) add(p.b, p.a, p.d, p.c);
-        if (!elastic) {
-            add(p.c, p.d, p.a, p.b);
-            if (p.d != p.c) add(p.d, p.c, p.b, p.a);
+        // Eq. 19 lists, for every species, the processes it takes part in: C_X receives the process once
+        // for every DISTINCT way X appears among its external legs.  The legs are numbered 0 = a, 1 = b (one side of the
+        // reaction), 2 = c, 3 = d (the other side).  VIEW[v] is the reaction re-labelled with leg v as the grid particle
+        // (slot 1): slot 2 is v's companion on its own side, slots 3 and 4 are the far side taken in the order that keeps
+        // (p1 - p3)^2 equal to the t of the process as written (a<->c and b<->d are the t-channel partners).
+        static const int VIEW[4][4] = {{0, 1, 2, 3}, {1, 0, 3, 2}, {2, 3, 0, 1}, {3, 2, 1, 0}};
+        const int leg_species[4] = {p.a, p.b, p.c, p.d};
+        for (int v = 0; v < 4; ++v) {
+            const int companion = VIEW[v][1];
+            // a view is redundant when it describes the same integral as an earlier one:
+            //  - its companion leg has already been viewed and carries the same species (the p2 integral of that view
+            //    already runs over every partner of that species);
+            //  - it looks from the far side of a reaction that is its own reverse (elastic: gain and loss of the
+            //    near-side views are already the two directions of the reaction)
+            if (companion < v && leg_species[companion] == leg_species[v]) continue;
+            if (v >= 2 && elastic) continue;
+            for (int slot = 0; slot < 4; ++slot) r.s[slot] = leg_species[VIEW[v][slot]];
+            // 1/2 "when all incident particles are of the same type"; the incident pair of a view is its far side
+            const bool identical_pair = r.s[2] == r.s[3];
+            r.sym = p.sym >= 0 ? p.sym : (identical_pair ? 0.5 : 1.0);
+            H->roles.push_back(r);
+            H->role_off.push_back(roff);
+            roff += (size_t)nx * H->np[r.s[0]];
         }
     }
     H->role_off.push_back(roff);
@@ -757,21 +772,37 @@ int orc_collision_symmetric(void* h, const double* f, double* C, double* mag, in
     for (size_t s = 0; s < H->sp.size(); ++s)
         for (int ix = ix_begin; ix < ix_end; ix += ix_stride)
             for (size_t j = 0; j < H->np[s]; ++j) { C[H->sp_off[s] + (size_t)ix * H->np[s] + j] = 0.0; mag[H->sp_off[s] + (size_t)ix * H->np[s] + j] = 0.0; }
-    auto dp3 = [&](int s) {
-        const Grid& g = H->grid[s];
-        return ((g.pmax[0] - g.pmin[0]) / g.n[0]) * ((g.pmax[1] - g.pmin[1]) / g.n[1]) * ((g.pmax[2] - g.pmin[2]) / g.n[2]);
-    };
+    // DESIGN.md section 4c.  A sample of a role is one reaction {1, 2} <-> {3, 4} with net rate (gain - loss) as seen by
+    // slots 1 and 2; slots 3 and 4 see the opposite sign.  Each of the four slots is, by itself, an unbiased estimator of
+    // the collision term of the species in that slot, once (i) divided by that species' momentum-cell volume instead of
+    // the grid particle's, (ii) given the identical-particle factor of ITS incident pair, which is the pair across the
+    // reaction from the slot, and (iii) averaged with all other (role, slot) estimators of the same species and process.
+    // Momentum-cell volume per species:
+    std::vector<double> cell_volume(H->sp.size());
+    for (size_t sidx = 0; sidx < H->sp.size(); ++sidx) {
+        double v = 1.0;
+        for (int d = 0; d < 3; ++d) v *= (H->grid[sidx].pmax[d] - H->grid[sidx].pmin[d]) / H->grid[sidx].n[d];
+        cell_volume[sidx] = v;
+    }
+    // (iii) how many (role, slot) estimators each process has per species, counted once over the finished role list
+    std::map<std::pair<int, int>, int> estimators;      // (process, species) -> count
+    for (const Role& r2 : H->roles)
+        for (int slot = 0; slot < 4; ++slot)
+            if ((slot_mask >> slot) & 1) ++estimators[std::make_pair(r2.process, r2.s[slot])];
+    struct SlotRule { double sign; int across[2]; };    // sign of the slot's net rate; the two slots across the reaction
+    static const SlotRule RULE[4] = {{+1.0, {2, 3}}, {+1.0, {2, 3}}, {-1.0, {0, 1}}, {-1.0, {0, 1}}};
     for (int ir = 0; ir < (int)H->roles.size(); ++ir) {
         const Role& role = H->roles[ir];
         SymSink sink; sink.C = C; sink.mag = mag;
-        for (int k = 0; k < 4; ++k) {
-            int m = 0;                                  // (role, slot) pairs of this process carrying species s_k
-            for (const Role& r2 : H->roles)
-                if (r2.process == role.process)
-                    for (int k2 = 0; k2 < 4; ++k2) m += ((slot_mask >> k2) & 1) && r2.s[k2] == role.s[k];
-            const int oa = k < 2 ? 2 : 0;               // the opposite pair
-            const double symk = role.sym_override >= 0 ? role.sym_override : (role.s[oa] == role.s[oa + 1] ? 0.5 : 1.0);
-            sink.fac[k] = ((slot_mask >> k) & 1) ? (k < 2 ? 1.0 : -1.0) * symk * (dp3(role.s[0]) / dp3(role.s[k])) / (double)m : 0.0;
+        for (int slot = 0; slot < 4; ++slot) {
+            sink.fac[slot] = 0.0;
+            if (!((slot_mask >> slot) & 1)) continue;
+            const int species_here = role.s[slot];
+            const bool identical_incident = role.s[RULE[slot].across[0]] == role.s[RULE[slot].across[1]];
+            const double pair_factor = role.sym_override >= 0 ? role.sym_override : (identical_incident ? 0.5 : 1.0);
+            const double volume_ratio = cell_volume[role.s[0]] / cell_volume[species_here];
+            const int count = estimators[std::make_pair(role.process, species_here)];
+            sink.fac[slot] = RULE[slot].sign * pair_factor * volume_ratio / (double)count;
         }
         const long np1 = (long)H->np[role.s[0]];
         const long ncell = (ix_end - ix_begin + ix_stride - 1) / ix_stride;
