@@ -102,6 +102,7 @@ def lib():
         L.orc_update.argtypes = [C.c_size_t, dp, dp, C.c_double, dp]
         L.orc_philox4x32_10.argtypes = [C.POINTER(C.c_uint32)] * 3
         L.orc_direction.argtypes = [C.POINTER(C.c_uint32), C.c_int, dp]
+        L.orc_direction_by_eye.argtypes = [C.POINTER(C.c_uint32), C.c_int, dp]
         _lib = L
     return _lib
 
@@ -119,6 +120,15 @@ def direction(words, use_float=False):
     x = (C.c_uint32 * 4)(*[int(w) for w in words])
     out = np.zeros(3)
     lib().orc_direction(x, int(use_float), _dp(out))
+    return out
+
+
+def direction_by_eye(words, use_float=False):
+    """The same lattice point as direction(), from the definition of a unit vector with the C library's cosl / sinl
+    (not used by the chain; the readable twin of O6)."""
+    x = (C.c_uint32 * 4)(*[int(w) for w in words])
+    out = np.zeros(3)
+    lib().orc_direction_by_eye(x, int(use_float), _dp(out))
     return out
 
 

@@ -236,6 +236,29 @@ template <typename R> inline void direction(uint32_t x3, uint32_t k24, R nh[3]) 
     nh[0] = st * cphi; nh[1] = st * sphi; nh[2] = nz;
 }
 
+// O6 BY EYE -- not part of the chain, never called by the estimator.  direction() above reaches its lattice point through
+// minimax polynomials, an octant fold and (double chain) an angle split chosen so that an implementation can tabulate it;
+// none of that can be checked against the paper by reading it.  This is the same lattice point straight from the
+// definition of a unit vector, n = (sin(theta) cos(phi), sin(theta) sin(phi), cos(theta)), with the C library's cosl / sinl
+// in extended precision (x86-64 long double: 64-bit significand, so the result is the exact value rounded once, for the
+// purposes of a 4e-16 comparison):
+//   cos(theta) = (x3 | 1) 2^-31 - 1                    (double chain; float chain: ((x3 >> 8) | 1) 2^-23 - 1)
+//   phi        = ((k24 >> 2) + 1/2) 2 pi / 2^22        (double chain; float chain: (k24 + 1/2) 2 pi / 2^24)
+// tests/test_oracle_kinematics.py compares the two on every octant boundary and on random words.  The chain cannot use
+// this form itself: libm results differ by an ulp between machines and the kernels must reproduce every cell-index
+// decision bit for bit.
+template <typename R> inline void direction_by_eye(uint32_t x3, uint32_t k24, double nh[3]) {
+    const long double PI_L = 3.14159265358979323846264338327950288L;
+    const bool dbl = sizeof(R) == 8;
+    const long double ct = dbl ? (long double)(x3 | 1u) / 2147483648.0L - 1.0L : (long double)((x3 >> 8) | 1u) / 8388608.0L - 1.0L;
+    const long double phi = dbl ? ((long double)(k24 >> 2) + 0.5L) * (2.0L * PI_L / 4194304.0L)
+                                : ((long double)k24 + 0.5L) * (2.0L * PI_L / 16777216.0L);
+    const long double st = sqrtl(1.0L - ct * ct);
+    nh[0] = (double)(st * cosl(phi));
+    nh[1] = (double)(st * sinl(phi));
+    nh[2] = (double)ct;
+}
+
 // S2 (t-channel sampler): a word -> uniform real in (0,1) on the half-integer lattice, exact in both types:
 // double (x + 1/2) 2^-32, float ((x >> 8) + 1/2) 2^-24.  uhalf(~x) = 1 - uhalf(x) exactly.
 template <typename R> inline R uhalf(uint32_t x);
@@ -637,6 +660,12 @@ void orc_direction(const uint32_t x[4], int use_float, double out[3]) {
     const uint32_t k24 = ((x[0] & 255u) << 16) | ((x[1] & 255u) << 8) | (x[2] & 255u);
     if (use_float) { float nh[3]; direction<float>(x[3], k24, nh); for (int d = 0; d < 3; ++d) out[d] = nh[d]; }
     else { double nh[3]; direction<double>(x[3], k24, nh); for (int d = 0; d < 3; ++d) out[d] = nh[d]; }
+}
+
+// O6 by eye (see direction_by_eye): the same words through the textbook definition and the C library.
+void orc_direction_by_eye(const uint32_t x[4], int use_float, double out[3]) {
+    const uint32_t k24 = ((x[0] & 255u) << 16) | ((x[1] & 255u) << 8) | (x[2] & 255u);
+    if (use_float) direction_by_eye<float>(x[3], k24, out); else direction_by_eye<double>(x[3], k24, out);
 }
 
 void* orc_create(int nx, int n_species, const Species* sp, const Grid* grid, int n_process, const Process* pr,

@@ -165,3 +165,31 @@ def test_direction_against_library_trigonometry():
                 wm = [hi[0] | (mirror >> 16), hi[1] | ((mirror >> 8) & 255), hi[2] | (mirror & 255), x3]
                 gm = oracle.direction(wm, use_float)
                 assert gm[0] == got[0] and gm[1] == -got[1] and gm[2] == got[2]
+
+
+def test_direction_polynomial_path_against_its_by_eye_twin():
+    """O6 once more, in the oracle's own language: direction() (polynomials, octant fold, the 9 + 10-bit angle split of the
+    double chain) against direction_by_eye() (the definition of a unit vector with cosl / sinl of the same lattice angle,
+    oracle/rbg_oracle.cpp) at the tolerance of the mpmath pin above, 4e-16 in double and 3e-7 in float: every octant
+    boundary, both neighbours of each, the ends of the 2^10 blocks of the angle split, and random words."""
+    rng = np.random.default_rng(11)
+    ks = set()
+    for o in range(9):
+        for d in (-2, -1, 0, 1, 2):
+            ks.add(min(max(o * 2 ** 21 + d, 0), 2 ** 24 - 1))
+    for hi in (0, 1, 255, 256, 511):                       # the split a = alpha(hi) + beta(lo): first / last lo of a block
+        for lo in (0, 1, 1022, 1023):
+            ks.add(((hi << 10) | lo) << 2)
+    ks = sorted(ks) + [int(v) for v in rng.integers(0, 2 ** 24, 3000)]
+    worst = {False: 0.0, True: 0.0}
+    for k in ks:
+        for x3 in [0, 1, 2 ** 31 - 1, 2 ** 31, 2 ** 32 - 1, int(rng.integers(0, 2 ** 32))]:
+            words = [k >> 16, (k >> 8) & 255, k & 255, x3]
+            for use_float, tol in ((False, 4e-16), (True, 3e-7)):
+                got, want = oracle.direction(words, use_float), oracle.direction_by_eye(words, use_float)
+                err = float(np.max(np.abs(got - want)))
+                worst[use_float] = max(worst[use_float], err)
+                assert err <= tol, (k, x3, use_float, got, want)
+                assert got[2] == want[2]                     # cos(theta) is exact on both paths
+    assert worst[False] > 0.0 and worst[True] > 1e-9         # the two paths really are different arithmetic
+
