@@ -265,6 +265,14 @@ int rbg_be_step(rbg_handle* h, double* f_dev, double* scratch_dev, const rbg_be_
 size_t rbg_f_elems(const rbg_handle* h);
 /* Number of roles (a process seen from one grid species; a+b with a != b gives two). */
 int rbg_n_roles(const rbg_handle* h);
+/* Role r (0 <= r < rbg_n_roles) as rbg_create expanded it from the process list (Eq. 19; DESIGN.md
+ * section 3): species[0..3] = the species of the grid particle 1, its sampled partner 2 and the other pair 3, 4;
+ * *sym = the symmetry factor applied (1/2 iff species 3 == species 4, unless the process overrides it); *cl, *cg = the
+ * degrees-of-freedom factors of the loss (1+2 -> 3+4) and gain (3+4 -> 1+2) directions (reading R21: 1 and 1 for an
+ * elastic process of kinds 0..3); *process = index into the process list.  Roles are in process order; within a process:
+ * seen from a, from b (if b != a), and for an inelastic process from c and from d (if d != c).  Out-parameters may be
+ * NULL.  Host-only query (no CUDA work); RBG_E_INVALID_ARG for a bad handle or index. */
+int rbg_role_info(const rbg_handle* h, int r, int species[4], double* sym, double* cl, double* cg, int* process);
 /* roles * Nx * Np * n_samples summed over roles: the "collision samples" one sweep evaluates. */
 uint64_t rbg_sample_evals(const rbg_handle* h, int n_samples);
 /* Kernels launched by the most recent rbg_collision* call on this handle. */

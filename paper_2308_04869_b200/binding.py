@@ -71,6 +71,8 @@ _SIGNATURES = {
     "rbg_be_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "rbg_f_elems": (C.c_size_t, [C.c_void_p]),
     "rbg_n_roles": (C.c_int, [C.c_void_p]),
+    "rbg_role_info": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_double), C.POINTER(C.c_double),
+                                C.POINTER(C.c_double), C.POINTER(C.c_int)]),
     "rbg_sample_evals": (C.c_uint64, [C.c_void_p, C.c_int]),
     "rbg_last_launch_count": (C.c_int, [C.c_void_p]),
     "rbg_set_option": (C.c_int, [C.c_void_p, C.c_char_p, C.c_int]),
@@ -220,6 +222,13 @@ class Collision:
 
     def sample_evals(self, n_samples: int) -> int:
         return int(load_library().rbg_sample_evals(self._h, int(n_samples)))
+
+    def role_info(self, r: int) -> dict:
+        """rbg_role_info: dict(s=(s1, s2, s3, s4), sym, cl, cg, process) of role r as the library expanded it."""
+        s4 = (C.c_int * 4)()
+        sym, cl, cg, proc = C.c_double(), C.c_double(), C.c_double(), C.c_int()
+        _check(load_library().rbg_role_info(self._h, int(r), s4, C.byref(sym), C.byref(cl), C.byref(cg), C.byref(proc)), self._h)
+        return dict(s=tuple(s4), sym=sym.value, cl=cl.value, cg=cg.value, process=proc.value)
 
     def last_launch_count(self) -> int:
         return int(load_library().rbg_last_launch_count(self._h))

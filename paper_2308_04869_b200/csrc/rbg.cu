@@ -104,17 +104,20 @@ template <typename R>
 rbg::RoleParams<R> make_role_params(const rbg_handle& H, const Role& r) {
     rbg::RoleParams<R> k;
     std::memset(&k, 0, sizeof k);
-    double m[4];
-    for (int i = 0; i < 4; ++i) m[i] = H.species[r.s[i]].mass;
-    const double msum = m[0] + m[1], m34 = m[2] + m[3], md = m[2] - m[3];
+    // masses of the four slots and their squares (each square rounded once, as DESIGN.md section 4 states the constants)
+    double m[4], q[4];
+    for (int i = 0; i < 4; ++i) { m[i] = H.species[r.s[i]].mass; q[i] = m[i] * m[i]; }
     k.m1 = (R)m[0]; k.m2 = (R)m[1];
-    k.msq1 = (R)(m[0] * m[0]); k.msq2 = (R)(m[1] * m[1]);
+    k.msq1 = (R)q[0]; k.msq2 = (R)q[1];
     k.m1m2 = (R)(m[0] * m[1]);
-    k.msum2 = (R)(msum * msum);
-    k.Mth = (R)(msum * msum - m34 * m34);
-    k.Mdf = (R)(md * md);
-    k.dm34 = (R)(m[2] * m[2] - m[3] * m[3]);
-    k.msqsum = (R)((m[0] * m[0] + m[1] * m[1]) + (m[2] * m[2] + m[3] * m[3]));
+    // thresholds: (m1 + m2)^2, and its distance to (m3 + m4)^2 (0 for an elastic role); (m3 - m4)^2 and m3^2 - m4^2
+    const double in_pair = m[0] + m[1], out_pair = m[2] + m[3], out_split = m[2] - m[3];
+    const double in_pair2 = in_pair * in_pair;
+    k.msum2 = (R)in_pair2;
+    k.Mth = (R)(in_pair2 - out_pair * out_pair);
+    k.Mdf = (R)(out_split * out_split);
+    k.dm34 = (R)(q[2] - q[3]);
+    k.msqsum = (R)((q[0] + q[1]) + (q[2] + q[3]));
     const rbg_momentum_grid& g1 = H.grids[r.s[0]];
     const rbg_momentum_grid& g2 = H.grids[r.s[1]];
     const rbg_momentum_grid& g3 = H.grids[r.s[2]];
@@ -139,13 +142,15 @@ rbg::RoleParams<R> make_role_params(const rbg_handle& H, const Role& r) {
     k.twomD2 = (R)(2.0 * (r.par[1] * r.par[1]));
     const double g2c = r.par[0] * r.par[0];
     k.g4 = (R)(g2c * g2c);
-    // Table III prefactors (d_F = C_A = 3, C_F = 4/3, d_A = 8), times g^4 = par0^4
-    const double dF = 3.0, CA = 3.0, CF = 4.0 / 3.0, dA = 8.0, g4d = g2c * g2c;
-    k.qA = (R)(8.0 * g4d * dF * dF * CF * CF / dA);
-    k.qB = (R)(16.0 * g4d * dF * CF * (CF - CA / 2.0));
-    k.qC = (R)(8.0 * g4d * dF * CF * CF);
-    k.qD = (R)(8.0 * g4d * dF * CF * CA);
-    k.qG = (R)(16.0 * g4d * dA * CA * CA);
+    // Table III prefactors: the colour factors of SU(N_c = 3) (PAPER.md:671 quotes d_F = C_A = 3, C_F = 4/3, d_A = 8; here
+    // from N_c: d_F = C_A = N_c, d_A = N_c^2 - 1, C_F = d_A / (2 N_c)), each times g^4 = par0^4 at the end
+    const double Nc = 3.0, dF = Nc, CA = Nc, dA = Nc * Nc - 1.0, CF = dA / (2.0 * Nc);
+    const double g4d = g2c * g2c, dFCF = dF * CF;
+    k.qA = (R)(g4d * (8.0 * dFCF * dFCF / dA));
+    k.qB = (R)(g4d * (16.0 * dFCF * (CF - 0.5 * CA)));
+    k.qC = (R)(g4d * (8.0 * dFCF * CF));
+    k.qD = (R)(g4d * (8.0 * dFCF * CA));
+    k.qG = (R)(g4d * (16.0 * dA * (CA * CA)));
     k.qcd = r.kind >= RBG_M2_QCD_Q1Q2 ? r.kind - RBG_M2_QCD_Q1Q2 : 0;
     k.rho = (R)(r.cg / r.cl);
     k.symV2 = (H.hbar * H.hbar) * (r.sym * V2) * r.cl;     // hbar^2 c of Eq. 16, c = 1
@@ -687,6 +692,17 @@ int rbg_collision_host(rbg_handle* h, const double* f_host, double* C_host, int 
 
 size_t rbg_f_elems(const rbg_handle* h) { return h ? h->f_elems : 0; }
 int rbg_n_roles(const rbg_handle* h) { return h ? (int)h->roles.size() : 0; }
+int rbg_role_info(const rbg_handle* h, int r, int species[4], double* sym, double* cl, double* cg, int* process) {
+    if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
+    if (r < 0 || r >= (int)h->roles.size()) { h->err = "rbg_role_info: role index out of range"; return RBG_E_INVALID_ARG; }
+    const Role& R = h->roles[r];
+    if (species) for (int i = 0; i < 4; ++i) species[i] = R.s[i];
+    if (sym) *sym = R.sym;
+    if (cl) *cl = R.cl;
+    if (cg) *cg = R.cg;
+    if (process) *process = R.process;
+    return RBG_OK;
+}
 uint64_t rbg_sample_evals(const rbg_handle* h, int n_samples) {
     if (!h) return 0;
     uint64_t t = 0;
