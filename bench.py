@@ -55,10 +55,26 @@ DOUBLE_CHAIN_V3_SAVING = 23.0
 # the same count for the t-channel importance sampler (steps S1-S7), kinds 1 and 2
 FLOPS_PER_SAMPLE_TCHANNEL = {1: 185.0, 2: 187.0}
 FP64_LANES_PER_SM = 64          # FMA/clk/SM; confirmed by the live probe
-# dram__bytes_read.sum + dram__bytes_write.sum of one role launch at full size, from the committed `ncu --set full`
-# captures (file named beside each); null for workloads without a capture.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {2: (32.91e6 + 2.41e6, "profiles/r2_collision.md, capture C"),
-                                4: (2183821056.0 + 2080522496.0, "profiles/r2_collision.md, capture D")}
+
+
+def ncu_traffic(group, key):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture, profiles/traffic.json
+    (written by hand from the capture named in profiles/traffic.md).  The file carries the digest of the library sources it
+    was captured on; on any other build the number is not this build's, and (None, reason) is returned instead of a stale
+    constant."""
+    path = ROOT / "profiles" / "traffic.json"
+    try:
+        t = json.loads(path.read_text())
+    except (OSError, ValueError):
+        return None, "profiles/traffic.json missing or unreadable"
+    from paper_2308_04869_b200.build import _digest
+    if t.get("digest") != _digest():
+        return None, (f"profiles/traffic.json was captured on build {str(t.get('digest'))[:12]}, this is build {_digest()[:12]}: "
+                      "no ncu capture of this build")
+    e = t.get(group, {}).get(str(key))
+    if not e:
+        return None, f"no capture for {group}/{key} in profiles/traffic.json"
+    return float(e["dram_bytes_read"]) + float(e["dram_bytes_write"]), f"bytes per launch (dram read + write; {e['source']})"
 
 
 def flops_per_sweep(problem, n_samples, fp32=False):
@@ -178,12 +194,6 @@ def config_block(w, args, world):
 
 
 # ---- the NEXT-4 kernels -----------------------------------------------------------------------------------------
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the NEXT-4 kernels on config 4 at full size, from the committed
-# `ncu --set full` captures (profiles/r2_be_steps.md; drift_pfl: profiles/r1d_be_steps_and_qgp.md, capture F); null otherwise.
-NCU_TRAFFIC_BE_CFG4 = {"moments": 2.097e9 + 7.4e6, "drift": 2.495e9 + 2.071e9, "vlasov": 2.099e9 + 2.042e9,
-                       "drift_pfl": 5.233e9 + 2.083e9}
-
-
 def hbm_peak():
     try:
         peaks = json.loads((ROOT / "MEASURED_PEAKS.json").read_text())
@@ -198,11 +208,16 @@ def run_be_steps(args):
     are 8 B per cell for the moments (f read once) and 16 B per cell for each stencil (f read once, f_out written once);
     peak = MEASURED_PEAKS.json hbm_gbs (sustained copy bandwidth), else the profiling guide's fallback 6500 GB/s."""
     import torch
-    import paper_2308_04869_b200 as rbg
     if int(os.environ.get("RANK", "0")) != 0:
         return
     torch.cuda.set_device(0)
-    w = workloads.make(args.config, nx=args.nx)
+    print(json.dumps(measure_be_steps(args, args.config, args.nx, args.steps, cpu_baseline=not args.no_cpu_baseline)))
+
+
+def measure_be_steps(args, cfg, nx_override, steps, cpu_baseline, e2e=True):
+    import torch
+    import paper_2308_04869_b200 as rbg
+    w = workloads.make(cfg, nx=nx_override)
     prob = w["problem"]
     nx = prob["nx"]
     side = round(nx ** (1.0 / 3.0))
@@ -238,44 +253,49 @@ def run_be_steps(args):
                 fn()
             torch.cuda.synchronize()
             ts = []
-            for _ in range(args.steps):
+            for _ in range(steps):
                 flush.fill_(1)
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 e0.record(stream); fn(); e1.record(stream)
                 torch.cuda.synchronize()
                 ts.append(e0.elapsed_time(e1))
-            launches += col.last_launch_count() * args.steps
+            launches += col.last_launch_count() * steps
             ms = sum(ts) / len(ts)
             gbs = bytes_per_cell * cells / (ms * 1e-3) / 1e9
             res[name] = {"ms": ms, "algorithmic_bytes_per_cell": bytes_per_cell, "achieved_gbs": gbs, "frac": gbs / peak,
-                         "traffic": NCU_TRAFFIC_BE_CFG4.get(name) if (args.config == 4 and args.nx is None and not args.opt) else None}
+                         "traffic": None, "traffic_unit": "not a full-size default run"}
+            if nx_override is None and not args.opt:
+                res[name]["traffic"], res[name]["traffic_unit"] = ncu_traffic(f"be_cfg{cfg}", name)
     clocks = cs.summary()
     t_step = sum(r["ms"] for k, r in res.items() if k != "drift_pfl") * 1e-3
-    # e2e: host buffers in, host buffers out, for the three calls of one step
-    f_host = torch.from_numpy(w["f"]).pin_memory()
-    o_host = torch.empty_like(f_host).pin_memory()
-    t0 = time.perf_counter()
-    fd = f_host.cuda(non_blocking=True)
-    M, tot, em = col.moments(fd)
-    o1 = col.drift_step(fd, 0.01, dx)
-    o2 = col.vlasov_step(o1, 0.01, E, B)
-    o_host.copy_(o2, non_blocking=True); em_h = em.cpu()
-    torch.cuda.synchronize()
-    t_e2e = time.perf_counter() - t0
     dom = max(("drift", "vlasov"), key=lambda k: res[k]["ms"])
     kern_name = {"drift": "rbg::drift_upfd_kernel", "vlasov": "rbg::vlasov_sym_kernel / rbg::vlasov_upfd_kernel"}[dom]
-    line = {"metric": "be_step_phase_space_cells_per_s", "value": cells / t_step, "unit": "cells/s", "n_gpus": 1, "steps": args.steps,
+    line = {"metric": "be_step_phase_space_cells_per_s", "value": cells / t_step, "unit": "cells/s", "n_gpus": 1, "steps": steps,
             "warmup": max(args.warmup, 3), "ms_per_step": t_step * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": w["name"] + " [moments + UPFD drift + UPFD Vlasov, NEXT-4]", "cfg": args.config, "nxyz": list(nxyz),
+            "config": {"workload": w["name"] + " [moments + UPFD drift + UPFD Vlasov, NEXT-4]", "cfg": cfg, "nxyz": list(nxyz),
                        "cells": cells, "f_bytes": int(w["f"].nbytes), "l2": "L2 flushed (256 MB write) between timed iterations"},
             "clocks": clocks, "gpu_launches": launches,
-            "e2e": {"value": cells / t_e2e, "unit": "cells/s", "h2d_bytes_per_step": int(w["f"].nbytes),
-                    "d2h_bytes_per_step": int(w["f"].nbytes) + int(em.numel() * 8), "ms_per_step": t_e2e * 1e3},
             "roofline": {"bound": "hbm", "achieved": res[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s", "frac": res[dom]["frac"],
-                         "traffic": res[dom]["traffic"], "kernel": kern_name, "peak_source": peak_src},
+                         "traffic": res[dom]["traffic"], "traffic_unit": res[dom]["traffic_unit"], "kernel": kern_name,
+                         "peak_source": peak_src},
             "kernels": res}
-    if not args.no_cpu_baseline:
+    if e2e:
+        # e2e: host buffers in, host buffers out, for the three calls of one step
+        f_host = torch.from_numpy(w["f"]).pin_memory()
+        o_host = torch.empty_like(f_host).pin_memory()
+        t0 = time.perf_counter()
+        fd = f_host.cuda(non_blocking=True)
+        M, tot, em = col.moments(fd)
+        o1 = col.drift_step(fd, 0.01, dx)
+        o2 = col.vlasov_step(o1, 0.01, E, B)
+        o_host.copy_(o2, non_blocking=True); em_h = em.cpu()
+        torch.cuda.synchronize()
+        t_e2e = time.perf_counter() - t0
+        line["e2e"] = {"value": cells / t_e2e, "unit": "cells/s", "h2d_bytes_per_step": int(w["f"].nbytes),
+                       "d2h_bytes_per_step": int(w["f"].nbytes) + int(em.numel() * 8), "ms_per_step": t_e2e * 1e3}
+        del f_host, o_host, fd, o1, o2
+    if cpu_baseline:
         from oracle import be_steps as bs
         ncell = max(1, min(nx, 8))
         sub = dict(prob, nx=ncell)
@@ -287,7 +307,9 @@ def run_be_steps(args):
         dt = time.perf_counter() - t0
         line["cpu_baseline"] = {"value": fsub.size / dt, "unit": "cells/s", "cores": 1, "kind": "oracle",
                                 "sample": f"{ncell} of {nx} spatial cells as an {ncell}x1x1 periodic box, every species and momentum cell"}
-    print(json.dumps(line))
+    del f, out, flush, col, E, B
+    torch.cuda.empty_cache()
+    return line
 
 
 # ---- launcher -------------------------------------------------------------------------------------------------------
@@ -469,10 +491,11 @@ def roofline_of(rbg, torch, res, args, local, probe_cache):
         probe_cache["ctx"] = {"dfma_3_distinct_operands_tflops": rbg.probe_alu_peak(3, 1 << 16) * 2 / 1e12,
                               "widemul_u32_gops": rbg.probe_alu_peak(4, 1 << 16) / 1e9}
     sym = args.estimator == "symmetric"
-    traffic = NCU_TRAFFIC_BYTES_PER_LAUNCH.get(w["cfg"]) if (args.nx is None and not args.sampler and not sym and not args.opt) else None
+    traffic = (None, "not a full-size default run of the standard estimator")
+    if args.nx is None and not args.sampler and not sym and not args.opt:
+        traffic = ncu_traffic("collision", w["cfg"])
     return {"bound": "alu", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s", "frac": achieved / peak_nominal,
-            "traffic": traffic[0] if traffic else None,
-            "traffic_unit": f"bytes per launch (dram read + write, {traffic[1]})" if traffic else None,
+            "traffic": traffic[0], "traffic_unit": traffic[1],
             "peak_source": f"{sms} SM x {lanes} FMA/clk x 2 x {max_mhz:.0f} MHz ({'FP32' if w['fp32'] else 'FP64'} FMA pipe; DESIGN.md section 8)",
             "peak_probe_tflops": probe, "frac_of_probe": achieved / probe, "probe_context": probe_cache["ctx"],
             # FP64 chain: a DFMA whose three operands are distinct registers is limited by register-file operand bandwidth
@@ -480,6 +503,68 @@ def roofline_of(rbg, torch, res, args, local, probe_cache):
             "frac_of_3_operand_dfma_rate": None if w["fp32"] else achieved / probe_cache["ctx"]["dfma_3_distinct_operands_tflops"],
             "kernel": "rbg::collision_symmetric_kernel" if sym else "rbg::collision_role_kernel", "launch_ms": t_launch * 1e3,
             "flops_per_sample": res["fl_rank"] / res["n_evals_rank"]}
+
+
+def evolve_measure(rbg, torch, w, n_steps, n_evals_per_step):
+    """The paper's collision-dominated run: n Euler steps f <- f + dt C[f] in place, every step a full sweep with its own
+    seed (rbg_collision_evolve); wall clock around the call, device synchronised on both sides."""
+    col = rbg.Collision(w["problem"], fp32_kinematics=w["fp32"])
+    fe = torch.from_numpy(w["f"]).cuda()
+    dt_e = w["dt"] if w["dt"] > 0 else 1e-3
+    col.collision_evolve(fe, dt_e, 3, w["n_samples"], w["seed"])             # warm-up
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    _, negf = col.collision_evolve(fe, dt_e, n_steps, w["n_samples"], w["seed"])
+    torch.cuda.synchronize()
+    t_ev = time.perf_counter() - t0
+    return {"steps": n_steps, "seconds": t_ev, "ms_per_step": 1e3 * t_ev / n_steps, "dt": dt_e,
+            "samples_per_s": n_evals_per_step * n_steps / t_ev,
+            "negative_cells_counted": int(negf.item()), "f_finite": bool(torch.isfinite(fe).all())}
+
+
+def next_block(rbg, torch, args, local, probe_cache):
+    """The rows SURVEY.md section 8(f) marks "next", each at full size and timed like the headline (3 warm-up sweeps, L2
+    flushed between timed sweeps, CUDA events, clocks sampled during the timed region), so that the driver's own N = 1 run
+    carries them: the paper's QGP sweep (workload 7, 70 roles, Table III kinds, inelastic roles), the conservative
+    estimator on the headline workload, the t-channel importance sampler on config 2, the paper's own collision test
+    (config 6: one Euler step, and 2 500 steps of rbg_collision_evolve), and the moments / drift / Vlasov kernels against
+    the HBM roofline on config 4 and on workload 7's odd 11^3 grid."""
+    import copy
+
+    def collision(cfg, steps, **over):
+        a = copy.copy(args)
+        a.nx, a.opt, a.sampler, a.estimator = None, [], 0, "standard"
+        for k, v in over.items():
+            setattr(a, k, v)
+        r = time_config(rbg, torch, cfg, a, steps, 3, 0, 1, local, e2e=False)
+        roof = roofline_of(rbg, torch, r, a, local, probe_cache)
+        return r, {"workload": r["w"]["name"], "value": r["n_evals_total"] / r["t_step"], "unit": UNIT,
+                   "ms_per_step": r["t_step"] * 1e3, "steps": steps, "warmup": 3, "sample_evals_per_sweep": r["n_evals_total"],
+                   "gpu_launches_per_step": r["launches_per_step"], "dtype": "f32" if r["w"]["fp32"] else "f64",
+                   "roofline": {k: roof[k] for k in ("bound", "achieved", "peak", "unit", "frac", "flops_per_sample", "launch_ms",
+                                                     "kernel")},
+                   "clocks": r["clocks"]}
+
+    def be(cfg, steps):
+        a = copy.copy(args)
+        a.nx, a.opt = None, []
+        line = measure_be_steps(a, cfg, None, steps, cpu_baseline=False, e2e=False)
+        return {"workload": line["config"]["workload"], "cells": line["config"]["cells"], "ms_per_step": line["ms_per_step"],
+                "steps": steps, "warmup": line["warmup"], "gpu_launches": line["gpu_launches"], "clocks": line["clocks"],
+                "peak_gbs": line["roofline"]["peak"], "peak_source": line["roofline"]["peak_source"],
+                "kernels": {k: {kk: v[kk] for kk in ("ms", "achieved_gbs", "frac", "algorithmic_bytes_per_cell")}
+                            for k, v in line["kernels"].items() if k != "drift_pfl"}}
+
+    out = {}
+    _, out["qgp_workload7_sweep"] = collision(7, 2)
+    _, out["conservative_estimator_config4"] = collision(HEADLINE_CONFIG, 2, estimator="symmetric")
+    _, out["tchannel_sampler_config2"] = collision(2, 3, sampler=1)
+    r6, out["papers_collision_test_config6_euler_step"] = collision(6, 10)
+    out["papers_collision_test_config6_evolve"] = evolve_measure(rbg, torch, r6["w"], 2500, r6["n_evals_total"])
+    del r6
+    out["be_steps_config4"] = be(4, 5)
+    out["be_steps_workload7"] = be(7, 5)
+    return out
 
 
 def main():
@@ -498,6 +583,8 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="CPU wall time of the cpu_baseline leg (bounded sample)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-config-block", action="store_true", help="skip the per-config block (configs 1, 2, 3, 5) of the N = 1 line")
+    ap.add_argument("--no-next", action="store_true", help="skip the `next` object (SURVEY 8(f) rows: workload 7, conservative "
+                    "estimator, t-channel sampler, config 6 step + evolve, moments / drift / Vlasov) of the default N = 1 line")
     ap.add_argument("--block-steps", type=int, default=3, help="timed sweeps per config of the per-config block")
     ap.add_argument("--nx", type=int, default=None, help="override the number of spatial cells (profiling runs; "
                     "the JSON line then names the reduced workload)")
@@ -571,21 +658,10 @@ def main():
                                                                      "flops_per_sample", "launch_ms", "traffic")},
                                    "clocks": r["clocks"]}
             line["configs"] = block
+            if not args.no_next:
+                line["next"] = next_block(rbg, torch, args, local, probe_cache)
         if args.evolve_steps > 0 and world == 1:
-            # the paper's collision-dominated run: n Euler steps f <- f + dt C[f] in place, every step a full sweep with its
-            # own seed (rbg_collision_evolve); wall clock around the call, device synchronised on both sides
-            col = rbg.Collision(w["problem"], fp32_kinematics=w["fp32"])
-            fe = torch.from_numpy(w["f"]).cuda()
-            dt_e = w["dt"] if w["dt"] > 0 else 1e-3
-            col.collision_evolve(fe, dt_e, 3, w["n_samples"], w["seed"])             # warm-up
-            torch.cuda.synchronize()
-            t0 = time.perf_counter()
-            _, negf = col.collision_evolve(fe, dt_e, args.evolve_steps, w["n_samples"], w["seed"])
-            torch.cuda.synchronize()
-            t_ev = time.perf_counter() - t0
-            line["evolve"] = {"steps": args.evolve_steps, "seconds": t_ev, "ms_per_step": 1e3 * t_ev / args.evolve_steps, "dt": dt_e,
-                              "samples_per_s": res["n_evals_total"] * args.evolve_steps / t_ev,
-                              "negative_cells_counted": int(negf.item()), "f_finite": bool(torch.isfinite(fe).all())}
+            line["evolve"] = evolve_measure(rbg, torch, w, args.evolve_steps, res["n_evals_total"])
         if not args.no_cpu_baseline and world == 1:          # rank 0 at N = 1 only
             cb = oracle_leg(w, args.cpu_seconds)
             cb.pop("seconds")
