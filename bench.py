@@ -330,6 +330,7 @@ def self_launch(args):
     env = dict(os.environ)
     env.setdefault("NCCL_DEBUG", "INFO")                  # the communicator lines (nranks, NVLS) go to the log
     env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+    env.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")       # NCCL logs to stdout by default: stdout carries the JSON line only
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
            "--master-addr", "127.0.0.1", "--master-port", str(free_port()), str(Path(__file__).resolve()), *sys.argv[1:]]
     raise SystemExit(subprocess.run(cmd, env=env).returncode)
@@ -409,9 +410,11 @@ def time_config(rbg, torch, cfg, args, steps, warmup, rank, world, local, e2e=Tr
         else:
             col.collision(f, w["n_samples"], w["seed"], out=out, stream=stream)
 
+    import torch.distributed as dist
+    grouped = dist.is_available() and dist.is_initialized()      # N > 1, or N = 1 with --force-dist
+
     def barrier():
-        if world > 1:
-            import torch.distributed as dist
+        if grouped:
             dist.barrier()
         torch.cuda.synchronize()
 
@@ -432,8 +435,7 @@ def time_config(rbg, torch, cfg, args, steps, warmup, rank, world, local, e2e=Tr
     times_ms = [e0.elapsed_time(e1) for e0, e1 in ev]
     t_step = max_over_ranks(sum(times_ms) / len(times_ms)) * 1e-3
     total_evals = n_evals
-    if world > 1:
-        import torch.distributed as dist
+    if grouped:
         t = torch.tensor([float(n_evals)], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.SUM)
         total_evals = int(t.item())
@@ -446,14 +448,13 @@ def time_config(rbg, torch, cfg, args, steps, warmup, rank, world, local, e2e=Tr
         c_host = torch.empty_like(f_host).pin_memory()
 
         def host_call():
-            if sym or w["dt"] > 0:               # no host entry point for these: pinned copies around the device call
+            if sym:                              # no host entry point for this one: pinned copies around the device call
                 fd = f_host.cuda(non_blocking=True)
-                if sym:
-                    r = col.collision_symmetric(fd, w["n_samples"], w["seed"])
-                else:
-                    r, _ = col.collision_update(fd, w["dt"], w["n_samples"], w["seed"], neg_flag=flag)
+                r = col.collision_symmetric(fd, w["n_samples"], w["seed"])
                 c_host.copy_(r, non_blocking=True)
                 torch.cuda.synchronize()
+            elif w["dt"] > 0:
+                col.collision_update_host(f_host, w["dt"], w["n_samples"], w["seed"], out=c_host)
             else:
                 col.collision_host(f_host, w["n_samples"], w["seed"], out=c_host)
         host_call()                              # warm: allocates scratch
@@ -595,6 +596,8 @@ def main():
     ap.add_argument("--opt", action="append", default=[], help="librbg option key=value (launch geometry)")
     ap.add_argument("--evolve-steps", type=int, default=0, help="also time rbg_collision_evolve over this many explicit Euler steps "
                     "in place (the paper's collision test, config 6: 25 000 steps, PAPER.md:469-506) and add an `evolve` object")
+    ap.add_argument("--force-dist", action="store_true", help="N = 1: initialise the NCCL process group with one rank and run the "
+                    "same barrier / MAX / SUM reductions as N > 1 (exercises the multi-GPU plumbing on one GPU)")
     ap.add_argument("--launch-check", action="store_true", help="launcher / rank plumbing only (gloo, no GPU work)")
     args = ap.parse_args()
     if args.gpus < 1:
@@ -617,10 +620,16 @@ def main():
     if torch.cuda.device_count() <= local:
         raise SystemExit(f"bench.py: rank {rank} needs CUDA device {local}, only {torch.cuda.device_count()} visible")
     torch.cuda.set_device(local)
-    if world > 1:
+    grouped = world > 1 or args.force_dist
+    if grouped:
+        # --force-dist at N = 1: the same NCCL process group, barrier, MAX and SUM reductions as N > 1, with one rank, so
+        # that a one-GPU run executes the multi-GPU plumbing (the communicator lines go to stderr)
         import torch.distributed as dist
         os.environ.setdefault("NCCL_DEBUG", "INFO")
         os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+        os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")     # NCCL logs to stdout by default: stdout carries the JSON line only
+        if "MASTER_ADDR" not in os.environ:
+            os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(free_port()), RANK="0", WORLD_SIZE="1", LOCAL_RANK="0")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     warmup = max(args.warmup, 3)
@@ -637,11 +646,13 @@ def main():
                 "workload_detail": {"sample_evals_per_sweep": res["n_evals_total"], "f_bytes_per_rank": res["bytes"],
                                     "nx_per_rank": w["problem"]["nx"], "roles": len(wl.roles(w["problem"]))},
                 "clocks": res["clocks"], "gpu_launches": res["launches_per_step"] * args.steps,
+                "process_group": f"nccl, {world} rank(s)" if grouped else None,
                 "e2e": {"value": res["n_evals_total"] / res["t_e2e"], "unit": UNIT, "h2d_bytes_per_step": res["bytes"] * world,
                         "d2h_bytes_per_step": res["bytes"] * world, "ms_per_step": res["t_e2e"] * 1e3,
                         "matches_device_path": res["same"],
-                        "api": "rbg_collision_host (pinned host buffers in and out)" if (w["dt"] == 0 and args.estimator == "standard")
-                               else "pinned host -> device copy, device entry point, device -> pinned host copy"},
+                        "api": ("pinned host -> device copy, rbg_collision_symmetric, device -> pinned host copy" if args.estimator != "standard"
+                                else "rbg_collision_update_host (pinned host buffers in and out)" if w["dt"] > 0
+                                else "rbg_collision_host (pinned host buffers in and out)")},
                 "roofline": roofline_of(rbg, torch, res, args, local, probe_cache)}
         # ---- every other BASELINE config in the same record (N = 1 only) -------------------------------------------
         if (world == 1 and not args.no_config_block and args.config == HEADLINE_CONFIG and args.nx is None and not args.opt
@@ -667,7 +678,7 @@ def main():
             cb.pop("seconds")
             line["cpu_baseline"] = cb
         print(json.dumps(line))
-    if world > 1:
+    if grouped:
         import torch.distributed as dist
         dist.barrier()
         dist.destroy_process_group()

@@ -172,6 +172,13 @@ int rbg_collision_symmetric(rbg_handle* h, const double* f_dev, double* C_dev, i
  * C_host must not overlap. */
 int rbg_collision_host(rbg_handle* h, const double* f_host, double* C_host, int n_samples, uint64_t seed);
 
+/* The fused explicit update (rbg_collision_update, Eq. 27) with HOST buffers, pipelined over chunks of spatial
+ * cells exactly like rbg_collision_host: f_out_host = f_host + dt C[f_host], bit-identical to the device entry point.
+ * *neg_count_host (host int) is SET to the number of cells of f_out that are negative -- unlike the device
+ * flag it does not accumulate across calls.  Synchronous; f_out_host must not overlap f_host. */
+int rbg_collision_update_host(rbg_handle* h, const double* f_host, double* f_out_host, double dt, int* neg_count_host,
+                              int n_samples, uint64_t seed);
+
 /* ---- The steps either side of the collision term ---------------------------------
  * Moments of f per species and spatial cell (midpoint sums over the momentum grid, Int d3p -> Sum dp^3, c = 1):
  *   n = Int f, j^k = Int v^k f (Eq. 5-6), T^{mu nu} = Int d3p/p0 p^mu p^nu f (Eq. 9).

@@ -63,6 +63,7 @@ _SIGNATURES = {
     "rbg_collision_evolve": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int, C.c_void_p, C.c_int,
                                        C.c_uint64, C.c_void_p]),
     "rbg_collision_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_uint64]),
+    "rbg_collision_update_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.POINTER(C.c_int), C.c_int, C.c_uint64]),
     "rbg_moments": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "rbg_moments_static": (C.c_int, [C.POINTER(_MomentumGrid), C.c_double, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
     "rbg_drift_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
@@ -340,8 +341,15 @@ class Collision:
                                           C.c_void_p(neg_flag.data_ptr()), _stream_ptr(stream)), self._h)
         return f, neg_flag
 
+    def collision_update_host(self, f_host, dt: float, n_samples: int, seed: int, out=None):
+        """rbg_collision_update_host: (f + dt*C[f], number of negative cells), host buffers in and out."""
+        return self._host_call(f_host, n_samples, seed, out, dt)
+
     def collision_host(self, f_host, n_samples: int, seed: int, out=None):
         """rbg_collision_host: host buffers in, host buffers out (numpy float64 or pinned CPU tensors)."""
+        return self._host_call(f_host, n_samples, seed, out, None)
+
+    def _host_call(self, f_host, n_samples, seed, out, dt):
         import torch
         def ptr(a, name):
             if isinstance(a, torch.Tensor):
@@ -355,6 +363,11 @@ class Collision:
             return C.c_void_p(p)
         if out is None:
             out = torch.empty_like(f_host) if isinstance(f_host, torch.Tensor) else np.empty_like(f_host)
+        if dt is not None:
+            neg = C.c_int(0)
+            _check(load_library().rbg_collision_update_host(self._h, ptr(f_host, "f_host"), ptr(out, "out"), float(dt),
+                                                            C.byref(neg), int(n_samples), int(seed)), self._h)
+            return out, int(neg.value)
         _check(load_library().rbg_collision_host(self._h, ptr(f_host, "f_host"), ptr(out, "out"), int(n_samples),
                                                  int(seed)), self._h)
         return out

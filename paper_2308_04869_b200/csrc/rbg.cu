@@ -63,6 +63,7 @@ struct rbg_handle {
     double2* dir_tab = nullptr;          // direction table of the double chain (rbg::kDirTabEntries entries)
     // scratch for the host entry point
     double *scratch_f = nullptr, *scratch_c = nullptr;
+    int* scratch_flag = nullptr;         // negative-cell counter of rbg_collision_update_host
     size_t scratch_elems = 0;
     enum { HOST_CHUNKS_MAX = 16 };
     cudaStream_t host_streams[3] = {nullptr, nullptr, nullptr};      // copy-in, kernels, copy-out of rbg_collision_host
@@ -634,9 +635,12 @@ int rbg_collision_evolve(rbg_handle* h, double* f_dev, double* scratch_dev, doub
     return RBG_OK;
 }
 
-int rbg_collision_host(rbg_handle* h, const double* f_host, double* C_host, int n_samples, uint64_t seed) {
+// Host-buffer sweep shared by rbg_collision_host (update = false: C into C_host) and rbg_collision_update_host (update =
+// true: f + dt C into C_host, *neg_count_host = cells left negative).
+static int host_sweep(rbg_handle* h, const double* f_host, double* C_host, bool update, double dt, int* neg_count_host,
+                      int n_samples, uint64_t seed) {
     if (!h) return fail(nullptr, RBG_E_INVALID_ARG, "null handle");
-    if (!f_host || !C_host) return fail(h, RBG_E_INVALID_ARG, "null buffer");
+    if (!f_host || !C_host || (update && !neg_count_host)) return fail(h, RBG_E_INVALID_ARG, "null buffer");
     if (ranges_overlap(f_host, h->f_elems * sizeof(double), C_host, h->f_elems * sizeof(double)))
         return fail(h, RBG_E_INVALID_ARG, "C_host overlaps f_host (chunks of C are copied out while later chunks of f are still being read)");
     if (n_samples <= 0) return fail(h, RBG_E_INVALID_ARG, "n_samples must be positive");
@@ -647,6 +651,7 @@ int rbg_collision_host(rbg_handle* h, const double* f_host, double* C_host, int 
         RBG_CUDA(h, cudaMalloc(&h->scratch_c, h->f_elems * sizeof(double)));
         h->scratch_elems = h->f_elems;
     }
+    if (update && !h->scratch_flag) RBG_CUDA(h, cudaMalloc(&h->scratch_flag, sizeof(int)));
     if (!h->host_streams[0]) {
         for (int i = 0; i < 3; ++i) RBG_CUDA(h, cudaStreamCreateWithFlags(&h->host_streams[i], cudaStreamNonBlocking));
         for (int i = 0; i < 2 * rbg_handle::HOST_CHUNKS_MAX; ++i) RBG_CUDA(h, cudaEventCreateWithFlags(&h->host_events[i], cudaEventDisableTiming));
@@ -662,7 +667,9 @@ int rbg_collision_host(rbg_handle* h, const double* f_host, double* C_host, int 
     // The pipeline queues copies into and out of the CALLER's host buffers on three streams.  Whatever happens, this call
     // returns only after all three have drained: after an error return the caller may free or reuse f_host / C_host at
     // once, and no DMA may still be running on them then.
+    int neg_count = 0;
     auto pipeline = [&]() -> int {
+        if (update) RBG_CUDA(h, cudaMemsetAsync(h->scratch_flag, 0, sizeof(int), s_k));
         for (int c = 0; c < chunks; ++c) {
             const int x0 = (int)((long)h->nx * c / chunks), x1 = (int)((long)h->nx * (c + 1) / chunks);
             for (int s = 0; s < h->n_species; ++s) {
@@ -671,8 +678,8 @@ int rbg_collision_host(rbg_handle* h, const double* f_host, double* C_host, int 
             }
             RBG_CUDA(h, cudaEventRecord(h->host_events[2 * c], s_in));
             RBG_CUDA(h, cudaStreamWaitEvent(s_k, h->host_events[2 * c], 0));
-            const int rc = fp32 ? run_roles<float>(h, h->scratch_f, h->scratch_c, false, 0.0, nullptr, n_samples, seed, s_k, x0, x1 - x0)
-                                : run_roles<double>(h, h->scratch_f, h->scratch_c, false, 0.0, nullptr, n_samples, seed, s_k, x0, x1 - x0);
+            const int rc = fp32 ? run_roles<float>(h, h->scratch_f, h->scratch_c, update, dt, h->scratch_flag, n_samples, seed, s_k, x0, x1 - x0)
+                                : run_roles<double>(h, h->scratch_f, h->scratch_c, update, dt, h->scratch_flag, n_samples, seed, s_k, x0, x1 - x0);
             if (rc != RBG_OK) return rc;
             RBG_CUDA(h, cudaEventRecord(h->host_events[2 * c + 1], s_k));
             RBG_CUDA(h, cudaStreamWaitEvent(s_out, h->host_events[2 * c + 1], 0));
@@ -681,13 +688,25 @@ int rbg_collision_host(rbg_handle* h, const double* f_host, double* C_host, int 
                 RBG_CUDA(h, cudaMemcpyAsync(C_host + o, h->scratch_c + o, n * sizeof(double), cudaMemcpyDeviceToHost, s_out));
             }
         }
+        // the count is complete once the kernels of the last chunk have run (stream order on s_k)
+        if (update) RBG_CUDA(h, cudaMemcpyAsync(&neg_count, h->scratch_flag, sizeof(int), cudaMemcpyDeviceToHost, s_k));
         return RBG_OK;
     };
     const int rc = pipeline();
     const cudaError_t d_out = cudaStreamSynchronize(s_out), d_k = cudaStreamSynchronize(s_k), d_in = cudaStreamSynchronize(s_in);
     if (rc != RBG_OK) return rc;                       // the pipeline's own message stands
     RBG_CUDA(h, d_out); RBG_CUDA(h, d_k); RBG_CUDA(h, d_in);
+    if (update) *neg_count_host = neg_count;
     return RBG_OK;
+}
+
+int rbg_collision_host(rbg_handle* h, const double* f_host, double* C_host, int n_samples, uint64_t seed) {
+    return host_sweep(h, f_host, C_host, false, 0.0, nullptr, n_samples, seed);
+}
+
+int rbg_collision_update_host(rbg_handle* h, const double* f_host, double* f_out_host, double dt, int* neg_count_host,
+                              int n_samples, uint64_t seed) {
+    return host_sweep(h, f_host, f_out_host, true, dt, neg_count_host, n_samples, seed);
 }
 
 size_t rbg_f_elems(const rbg_handle* h) { return h ? h->f_elems : 0; }
@@ -738,7 +757,7 @@ const char* rbg_last_error(const rbg_handle* h) { return h ? h->err.c_str() : g_
 void rbg_destroy(rbg_handle* h) {
     if (!h) return;
     DeviceGuard guard(h->device);
-    cudaFree(h->scratch_f); cudaFree(h->scratch_c);
+    cudaFree(h->scratch_f); cudaFree(h->scratch_c); cudaFree(h->scratch_flag);
     for (cudaStream_t st : h->host_streams) if (st) cudaStreamDestroy(st);
     for (cudaEvent_t ev : h->host_events) if (ev) cudaEventDestroy(ev);
     for (double* p : h->tab_iE) cudaFree(p);

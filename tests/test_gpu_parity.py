@@ -215,6 +215,34 @@ def test_host_entry_point_matches_device_entry_point():
     assert np.array_equal(col.collision_host(pinned, w["n_samples"], w["seed"]).numpy(), C_dev)
 
 
+def test_update_host_entry_point_matches_the_device_update():
+    """rbg_collision_update_host = rbg_collision_update with host buffers: same bits, and the count of negative cells is set
+    (not accumulated).  Two species, fp32 kinematics and fp64; a step large enough to drive cells negative; then a problem
+    above 128 MB so that the sweep is pipelined over two chunks and the count sums over them."""
+    rbg = _rbg()
+    for fp32 in (False, True):
+        w = workloads.make(2, nx=3, np_side=8, n_samples=32)
+        col = rbg.Collision(w["problem"], fp32_kinematics=fp32)
+        f = torch.from_numpy(w["f"]).cuda()
+        for dt in (1e-3, 5e4):
+            ref, flag = col.collision_update(f, dt, w["n_samples"], w["seed"])
+            torch.cuda.synchronize()
+            for _ in range(2):                                   # twice: the count must not accumulate
+                out, neg = col.collision_update_host(w["f"], dt, w["n_samples"], w["seed"])
+                assert np.array_equal(out, ref.cpu().numpy())
+                assert neg == int(flag.item()) == int(np.sum(out < 0))
+        assert neg > 0
+    w = workloads.make(2, nx=1201, np_side=20, n_samples=4)
+    assert w["f"].nbytes > (128 << 20)
+    col = rbg.Collision(w["problem"])
+    ref, flag = col.collision_update(torch.from_numpy(w["f"]).cuda(), 3e4, w["n_samples"], w["seed"])
+    out, neg = col.collision_update_host(torch.from_numpy(w["f"]).pin_memory(), 3e4, w["n_samples"], w["seed"])
+    assert torch.equal(out, ref.cpu()) and neg == int(flag.item()) and neg > 0
+    with pytest.raises(rbg.RbgError, match="overlaps"):
+        buf = np.zeros(2 * col.f_elems)
+        col.collision_update_host(buf[:col.f_elems], 1e-3, 4, 1, out=buf[1:col.f_elems + 1])
+
+
 def test_host_entry_point_pipelined_over_cell_chunks_is_bit_identical():
     """rbg_collision_host pipelines copy-in / kernels / copy-out over chunks of spatial cells once f exceeds 128 MB
     (include/rbg.h); two species so that every chunk is two H2D copies, an odd cell count so that the chunks are unequal.
