@@ -621,6 +621,7 @@ def main():
         raise SystemExit(f"bench.py: rank {rank} needs CUDA device {local}, only {torch.cuda.device_count()} visible")
     torch.cuda.set_device(local)
     grouped = world > 1 or args.force_dist
+    json_out = sys.stdout
     if grouped:
         # --force-dist at N = 1: the same NCCL process group, barrier, MAX and SUM reductions as N > 1, with one rank, so
         # that a one-GPU run executes the multi-GPU plumbing (the communicator lines go to stderr)
@@ -630,6 +631,11 @@ def main():
         os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")     # NCCL logs to stdout by default: stdout carries the JSON line only
         if "MASTER_ADDR" not in os.environ:
             os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(free_port()), RANK="0", WORLD_SIZE="1", LOCAL_RANK="0")
+        # NCCL writes its version banner (and, without NCCL_DEBUG_FILE, its log) to file descriptor 1.  stdout must carry the one
+        # JSON line and nothing else, so for the rest of this process fd 1 points at stderr and the line goes to the saved stdout.
+        sys.stdout.flush()
+        json_out = os.fdopen(os.dup(1), "w")
+        os.dup2(2, 1)
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     warmup = max(args.warmup, 3)
@@ -677,7 +683,7 @@ def main():
             cb = oracle_leg(w, args.cpu_seconds)
             cb.pop("seconds")
             line["cpu_baseline"] = cb
-        print(json.dumps(line))
+        print(json.dumps(line), file=json_out, flush=True)
     if grouped:
         import torch.distributed as dist
         dist.barrier()
